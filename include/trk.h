@@ -1,0 +1,172 @@
+/* trk.h -- C ABI of the B200-native Exa.TrkX inference hot path.
+ *
+ * One call runs the five stages of PAPER.md line 85 (section 2.2.2) on the device:
+ *   S1 embedding MLP -> S2 fixed-radius graph in the latent space -> S3 filter MLP + cut ->
+ *   S4 interaction-network GNN edge scores -> S5 weakly-connected components (track labels).
+ * The lifecycle mirrors the paper's backend: "loading the full
+ * pipeline, performing inference, and setting the GPU device ID" == trk_create / trk_infer /
+ * trk_destroy, with constants preloaded once and intermediates kept on the device (lines 77, 115).
+ * Every architectural number comes from the caller (BASELINE.json configs); DESIGN.md lists the
+ * readings of the paper this header relies on (C-7..C-17).
+ *
+ * Conventions
+ *   - plain C99, no torch types; "HOST"/"DEVICE" says where a pointer must live.
+ *   - all indices int32, hit features fp32 (r/1000, phi/pi, z/1000), row-major everywhere.
+ *   - every function returns trk_status; no exception crosses the ABI; trk_last_error() gives text.
+ *   - trk_infer and the trk_stage_* calls only enqueue work on `cuda_stream` (a cudaStream_t cast
+ *     to void*, NULL = legacy default stream): they never allocate, never synchronise, and may be
+ *     captured into a CUDA graph.  Host-detectable errors return before anything is enqueued.
+ *   - a ctx serves one in-flight call at a time (stream-ordered); several ctxs on several streams
+ *     are the analogue of several model instances.
+ *   - there is no CPU fallback: trk_create fails with TRK_ERR_UNSUPPORTED_DEVICE off sm_100.
+ */
+#ifndef TRK_H_
+#define TRK_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct trk_ctx trk_ctx; /* opaque: one "model instance" */
+
+typedef enum {
+  TRK_OK = 0,
+  TRK_ERR_INVALID_ARG = 1,      /* NULL pointer, negative size, non-monotone offsets, bad enum   */
+  TRK_ERR_SHAPE = 2,            /* MLP dims inconsistent with each other or with the hyperparameters */
+  TRK_ERR_CAPACITY = 3,         /* a call exceeds max_hits / max_events / an output capacity      */
+  TRK_ERR_CUDA = 4,             /* CUDA runtime or driver error (text in trk_last_error)          */
+  TRK_ERR_OOM = 5,              /* workspace allocation failed in trk_create                      */
+  TRK_ERR_UNSUPPORTED_DEVICE = 6 /* device is not compute capability 10.x                         */
+} trk_status;
+
+enum { TRK_FP32 = 0, TRK_BF16 = 1 };             /* trk_config.precision                          */
+enum { TRK_FILTER_RAW = 0, TRK_FILTER_EMB = 1 }; /* trk_config.filter_input (reading C-10)        */
+
+/* A stack of Linear layers.  weight[l] is HOST fp32 [dims[l+1]][dims[l]] (out, in) row-major,
+ * bias[l] is HOST fp32 [dims[l+1]].  trk_create copies everything; the caller may free at return. */
+typedef struct {
+  int32_t n_layers;
+  const int32_t* dims;          /* HOST, n_layers + 1 entries, e.g. {3,1024,1024,1024,12}         */
+  const float* const* weight;   /* HOST array of n_layers HOST pointers                            */
+  const float* const* bias;     /* HOST array of n_layers HOST pointers                            */
+} trk_mlp;
+
+typedef struct {
+  uint32_t struct_size;         /* = sizeof(trk_config), for versioning                            */
+  int32_t device;               /* CUDA device ordinal, fixed for the ctx lifetime */
+  int32_t precision;            /* TRK_FP32: SIMT fp32 everywhere.  TRK_BF16: tcgen05 GEMMs with bf16
+                                   operands (weights/activations rounded RNE) and fp32 accumulation;
+                                   needs hidden widths that are multiples of 64 and H in {64,128}.  */
+  /* S1: embedding MLP, ReLU between layers, none on the output. dims[0] == 3.                     */
+  trk_mlp embed;
+  /* S2: for every hit i the K nearest hits j of the same event with outer(i,j) and d2 <= r^2, d2 in
+   * fp64 from the fp32 embedding (k ascending, no FMA); outer <=> (r,|z|,index) lexicographically
+   * larger; ties in d2 -> lower index (readings C-7..C-9, C-11).  1 <= frnn_k <= 128.             */
+  float frnn_radius;
+  int32_t frnn_k;
+  const float* grid_proj;       /* HOST fp32 [d_e][grid_dims] with orthonormal columns used only to
+                                   bin hits (any such matrix gives the same graph, reading C-21);
+                                   NULL = the first grid_dims latent coordinates                    */
+  int32_t grid_dims;            /* 1..3                                                             */
+  /* S3: score = sigmoid(MLP([u_src ; u_dst])), u = embedding row (TRK_FILTER_EMB) or raw hit row
+   * (TRK_FILTER_RAW); kept iff score > filter_cut (strict); kept edges stay in (src,dst) order.    */
+  trk_mlp filter;               /* dims[0] == 2*u, last dim == 1                                    */
+  int32_t filter_input;
+  float filter_cut;
+  /* S4: interaction network of DESIGN.md "S4" (reading C-12): all five MLPs have 2 layers.        */
+  int32_t gnn_hidden;           /* H                                                                */
+  int32_t gnn_iters;            /* T, weights shared across iterations                              */
+  int32_t gnn_layernorm;        /* 1: ReLU(LayerNorm(.)) after every GNN Linear but the last (eps 1e-5,
+                                   no affine, reading C-13); 0: plain ReLU                          */
+  trk_mlp node_enc;             /* 3  -> H -> H                                                     */
+  trk_mlp edge_enc;             /* 4  -> H -> H   on (dr, dphi wrapped to (-1,1], dz, deta)         */
+  trk_mlp edge_net;             /* 3H -> H -> H   on [h_src ; h_dst ; e], residual                  */
+  trk_mlp node_net;             /* 3H -> H -> H   on [h ; sum_in e ; sum_out e], residual           */
+  trk_mlp edge_dec;             /* 3H -> H -> 1   on [h_src ; h_dst ; e], then sigmoid              */
+  /* S5: keep edges with gnn score > gnn_cut (strict); label = smallest hit index of the component. */
+  float gnn_cut;
+  /* Workspace is sized once from these; nothing is allocated later.                               */
+  int64_t max_hits;             /* N summed over the events of one call                             */
+  int64_t max_events;
+  int64_t max_cand_edges;       /* S2 output capacity; max_hits*frnn_k can never overflow           */
+  int64_t max_kept_edges;       /* S3 output capacity (data dependent)                              */
+} trk_config;
+
+typedef struct {
+  int32_t n_events;
+  const int32_t* event_offsets; /* HOST, n_events+1 entries, [0] == 0, non-decreasing; N = last     */
+  const float* hits;            /* DEVICE fp32 [N][3]                                               */
+} trk_batch;
+
+/* Outputs: all DEVICE, caller-owned, NULL = not wanted (counts and labels are required).
+ * Edges are global hit indices, sorted by (src, dst).  If a capacity is too small the list is
+ * truncated deterministically (lowest (src,dst) first), counts[3] is set to 1 and labels are the
+ * components of the truncated graph.                                                              */
+typedef struct {
+  int32_t* labels;              /* [N]                                                              */
+  int32_t* counts;              /* [4] = {E_c, E_k, E_t (edges passing gnn_cut), overflow flag}     */
+  int32_t* edge_src;            /* [edge_capacity] kept (S3) edges                                  */
+  int32_t* edge_dst;
+  float* edge_score;            /* [edge_capacity] S4 sigmoid scores of the kept edges              */
+  int64_t edge_capacity;
+  int32_t* cand_src;            /* [cand_capacity] S2 edges                                         */
+  int32_t* cand_dst;
+  float* cand_score;            /* [cand_capacity] S3 sigmoid scores                                */
+  int64_t cand_capacity;
+  float* embedding;             /* [N][d_e] S1 output                                               */
+} trk_result;
+
+trk_status trk_create(const trk_config* cfg, trk_ctx** out);
+trk_status trk_infer(trk_ctx* ctx, const trk_batch* batch, const trk_result* result, void* cuda_stream);
+trk_status trk_destroy(trk_ctx* ctx);
+
+/* The served request (spacepoints in, track candidates out) with HOST
+ * buffers: copies hits H2D, runs trk_infer on the ctx's own stream, copies labels (and, when the
+ * pointers are non-NULL, counts[4]) D2H and synchronises.  hits_host/labels_host should be pinned. */
+trk_status trk_infer_host(trk_ctx* ctx, int32_t n_events, const int32_t* event_offsets,
+                          const float* hits_host, int32_t* labels_host, int32_t* counts_host);
+
+const char* trk_status_string(trk_status s);
+const char* trk_last_error(const trk_ctx* ctx); /* ctx may be NULL: error of the last failed trk_create */
+int64_t trk_workspace_bytes(const trk_ctx* ctx);
+/* Number of kernels of this library launched by the most recent trk_infer on ctx (host-side count). */
+int64_t trk_last_launch_count(const trk_ctx* ctx);
+
+/* Stage hooks: run ONE stage on caller-supplied DEVICE inputs (BASELINE.json north_star: "each
+ * stage fed the oracle's own inputs for that stage").  Same kernels as trk_infer.  Unless noted
+ * all pointers are DEVICE; sizes are HOST scalars and must respect the ctx capacities.            */
+
+/* S1: emb fp32 [n][d_e]. */
+trk_status trk_stage_embed(trk_ctx* ctx, const float* hits, int64_t n, float* emb, void* cuda_stream);
+/* S2: writes src/dst [<= capacity] sorted by (src,dst), rowptr [n+1], count[2] = {E_c, overflow}.
+ * event_offsets is HOST. */
+trk_status trk_stage_frnn(trk_ctx* ctx, const float* emb, const float* hits, const int32_t* event_offsets,
+                          int32_t n_events, int32_t* src, int32_t* dst, int32_t* rowptr, int64_t capacity,
+                          int32_t* count, void* cuda_stream);
+/* S3: score fp32 [n_edges] for the given edges; feat is the embedding [n][d_e] or the hits [n][3]
+ * according to filter_input.  n is the number of rows of feat. */
+trk_status trk_stage_filter(trk_ctx* ctx, const float* feat, int64_t n, const int32_t* src, const int32_t* dst,
+                            int64_t n_edges, float* score, void* cuda_stream);
+/* S3 tail: stable compaction of the edges with score > filter_cut; count[2] = {E_k, overflow}. */
+trk_status trk_stage_compact(trk_ctx* ctx, const int32_t* src, const int32_t* dst, const float* score,
+                             int64_t n_edges, int32_t* out_src, int32_t* out_dst, int64_t capacity,
+                             int32_t* count, void* cuda_stream);
+/* S4: score fp32 [n_edges] = sigmoid(GNN logit).  Edges must be sorted by (src,dst). */
+trk_status trk_stage_gnn(trk_ctx* ctx, const float* hits, int64_t n, const int32_t* src, const int32_t* dst,
+                         int64_t n_edges, float* score, void* cuda_stream);
+/* S5: labels int32 [n]; edges with score > cut are kept. */
+trk_status trk_stage_cc(trk_ctx* ctx, int64_t n, const int32_t* src, const int32_t* dst, const float* score,
+                        int64_t n_edges, float cut, int32_t* labels, void* cuda_stream);
+
+/* Kernel hook for tests/bench: out = act(A W^T + bias) through the ctx-independent tcgen05 GEMM.
+ * A DEVICE bf16 [m][k] (k % 64 == 0), W DEVICE bf16 [n][k] (n % 16 == 0, n <= 1024 ... see DESIGN.md),
+ * bias DEVICE fp32 [n], out DEVICE bf16 [m][n]; relu != 0 applies ReLU. */
+trk_status trk_gemm_bf16(const void* a, const void* w, const float* bias, void* out, int64_t m, int32_t n,
+                         int32_t k, int32_t relu, void* cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TRK_H_ */

@@ -1,0 +1,177 @@
+// Shared declarations of the trk library (CUDA path).  No code here is shared with oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <cuda_bf16.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "trk.h"
+
+namespace trk {
+
+constexpr int kMaxEmbDim = 16;      // d_e is padded to a multiple of 4, at most 16
+constexpr int kMaxEvents = 1024;    // event offsets travel as a kernel parameter
+constexpr int64_t kMaxCells = 1 << 21;  // FRNN grid cells summed over the events of a call
+constexpr int kFilterChunkRows = 128 * 148;  // S3 rows per pass: one 128-row tile per SM and N-tile column
+
+// One Linear layer resident on the device.
+struct DevLinear {
+  int in = 0, out = 0;
+  float* w_f32 = nullptr;           // [out][in]
+  float* b_f32 = nullptr;           // [out]
+  __nv_bfloat16* w_bf16 = nullptr;  // [out_pad][in_pad] K-major, zero padded (bf16 mode only)
+  int in_pad = 0, out_pad = 0;
+};
+
+struct DevMlp {
+  std::vector<DevLinear> layers;
+};
+
+// Device-side FRNN grid parameters (written by a 1-thread kernel, read by the others).
+struct GridParams {
+  float origin[3];
+  float inv_cell[3];
+  int dims[3];
+  int cells_per_event;
+};
+
+struct EventOffsets {
+  int32_t v[kMaxEvents + 1];
+};
+
+struct Workspace {
+  char* base = nullptr;
+  size_t bytes = 0;
+};
+
+}  // namespace trk
+
+struct trk_ctx {
+  trk_config cfg;                   // scalar hyperparameters (pointers inside are not kept)
+  int device = 0;
+  int sm_count = 148;
+  int d_e = 0, d_e_pad = 0;         // embedding width and its padding to a multiple of 4
+  int filter_u = 0;                 // width of one endpoint's filter input
+  int H = 0;
+  cudaStream_t own_stream = nullptr;
+  std::string last_error;
+  int64_t launch_count = 0;
+
+  trk::DevMlp embed, filter, node_enc, edge_enc, edge_net, node_net, edge_dec;
+  float* grid_proj = nullptr;       // [d_e_pad][3] device
+  int grid_dims = 3;
+  int grid_max = 32;                // cells per axis and event (32, 16 or 8 by max_events)
+
+  // stacked bf16 weights of the split first layers (bf16 mode): [2H][H] = [W1[:, :H] ; W1[:, H:2H]]
+  __nv_bfloat16* edge_net_wab = nullptr;
+  __nv_bfloat16* edge_net_wc = nullptr;    // [H][H] = W1[:, 2H:3H]
+  __nv_bfloat16* edge_dec_wab = nullptr;
+  __nv_bfloat16* edge_dec_wc = nullptr;
+  __nv_bfloat16* filter_w1_pad = nullptr;  // [1024][64] = W1 zero padded in K
+
+  trk::Workspace ws;
+  // ---- workspace carve-up (device pointers into ws.base) ----
+  int32_t* ev_of_hit = nullptr;     // [max_hits] event id per hit
+  float* emb = nullptr;             // [max_hits][d_e]
+  // S1 / S3 activations
+  void* act0 = nullptr;             // bf16 or fp32 [rows][width]
+  void* act1 = nullptr;
+  void* act_in = nullptr;           // S3 gathered input rows
+  float* partial = nullptr;         // [chunk][4] fused last-layer partial dots
+  int64_t act_rows = 0;
+  // S2
+  float* proj = nullptr;            // [max_hits][3]
+  int32_t* bbox = nullptr;          // [6] ordered-int min/max
+  trk::GridParams* grid = nullptr;
+  int32_t* cell_of_hit = nullptr;   // [max_hits]
+  int32_t* cell_count = nullptr;    // [max_cells+1]
+  int32_t* cell_start = nullptr;    // [max_cells+1]
+  int32_t* cell_fill = nullptr;     // [max_cells]
+  float* semb = nullptr;            // [max_hits][d_e_pad] sorted by cell
+  float4* smeta = nullptr;          // [max_hits] (r, |z|, idx bits, cell bits)
+  int32_t* slots = nullptr;         // [max_hits][K]
+  int32_t* deg = nullptr;           // [max_hits+1]
+  int32_t* rowptr = nullptr;        // [max_hits+1]
+  int32_t* scan_tmp = nullptr;      // block sums for scans
+  int64_t max_cells = 0;
+  // edges
+  int32_t* cand_src = nullptr;      // [max_cand_edges]
+  int32_t* cand_dst = nullptr;
+  float* cand_score = nullptr;
+  int32_t* kept_src = nullptr;      // [max_kept_edges]
+  int32_t* kept_dst = nullptr;
+  float* kept_score = nullptr;
+  int32_t* counts = nullptr;        // [8] device: {E_c, E_k, E_t, overflow, ...}
+  int32_t* flag_scan = nullptr;     // [max_cand_edges] compaction offsets
+  // S4
+  void* X = nullptr;                // [max_hits][3H]  (h | m_in | m_out)  bf16 or fp32
+  void* E = nullptr;                // [max_kept_edges][H]
+  void* T1 = nullptr;               // [max(max_hits,max_kept_edges)][H]
+  float* PAB = nullptr;             // [max_hits][2H] fp32 per-node halves of the split first layer
+  float* cat = nullptr;             // fp32 mode: [max(E,N)][3H]
+  int32_t* in_rowptr = nullptr;     // [max_hits+1] CSR by dst
+  int32_t* in_perm = nullptr;       // [max_kept_edges]
+  int32_t* in_fill = nullptr;       // [max_hits]
+  int32_t* out_rowptr = nullptr;    // [max_hits+1] CSR by src (edges are src-sorted)
+  // S5
+  int32_t* parent = nullptr;        // [max_hits]
+};
+
+namespace trk {
+
+// ---- error plumbing ----
+trk_status fail(trk_ctx* ctx, trk_status s, const std::string& msg);
+#define TRK_CUDA(ctx, expr)                                                                   \
+  do {                                                                                        \
+    cudaError_t _e = (expr);                                                                  \
+    if (_e != cudaSuccess)                                                                    \
+      return ::trk::fail((ctx), TRK_ERR_CUDA, std::string(#expr) + ": " + cudaGetErrorString(_e)); \
+  } while (0)
+#define TRK_TRY(expr)                   \
+  do {                                  \
+    trk_status _s = (expr);             \
+    if (_s != TRK_OK) return _s;        \
+  } while (0)
+
+// Every kernel launch of the library goes through this so that launches can be counted.
+#define TRK_LAUNCH(ctx, kernel, grid, block, smem, stream, ...)                 \
+  do {                                                                           \
+    kernel<<<(grid), (block), (smem), (stream)>>>(__VA_ARGS__);                  \
+    (ctx)->launch_count++;                                                       \
+    cudaError_t _e = cudaPeekAtLastError();                                      \
+    if (_e != cudaSuccess)                                                       \
+      return ::trk::fail((ctx), TRK_ERR_CUDA, std::string(#kernel) + ": " + cudaGetErrorString(_e)); \
+  } while (0)
+
+inline int64_t ceil_div(int64_t a, int64_t b) { return (a + b - 1) / b; }
+
+// ---- util_kernels.cu ----
+trk_status exclusive_scan_i32(trk_ctx* ctx, const int32_t* in, int32_t* out, int64_t n, int32_t* tmp, cudaStream_t st);
+trk_status fill_i32(trk_ctx* ctx, int32_t* p, int32_t v, int64_t n, cudaStream_t st);
+trk_status compact_edges(trk_ctx* ctx, const int32_t* src, const int32_t* dst, const float* score, const int32_t* n_dev,
+                         int64_t n_cap, float cut, int32_t* out_src, int32_t* out_dst, int64_t out_cap, int32_t* count_out,
+                         int32_t* overflow_flag, cudaStream_t st);
+
+// ---- frnn.cu ----
+trk_status frnn_build(trk_ctx* ctx, const float* emb, const float* hits, int64_t n, int32_t n_events, int32_t* src,
+                      int32_t* dst, int32_t* rowptr_out, int64_t capacity, int32_t* count_out, int32_t* overflow_flag,
+                      cudaStream_t st);
+
+trk_status set_event_ids(trk_ctx* ctx, const int32_t* offsets_host, int n_events, int64_t n, cudaStream_t st);
+
+// ---- cc.cu ----
+trk_status cc_labels(trk_ctx* ctx, int64_t n, const int32_t* src, const int32_t* dst, const float* score,
+                     const int32_t* n_edges_dev, int64_t n_edges_cap, float cut, int32_t* labels, int32_t* pass_count,
+                     cudaStream_t st);
+
+// ---- nn_fp32.cu / nn_bf16.cu: S1, S3, S4 ----
+trk_status embed_forward(trk_ctx* ctx, const float* hits, int64_t n, float* emb, cudaStream_t st);
+trk_status filter_forward(trk_ctx* ctx, const float* feat, const int32_t* src, const int32_t* dst,
+                          const int32_t* n_edges_dev, int64_t n_edges_cap, float* score, cudaStream_t st);
+trk_status gnn_forward(trk_ctx* ctx, const float* hits, int64_t n, const int32_t* src, const int32_t* dst,
+                       const int32_t* n_edges_dev, int64_t n_edges_cap, float* score, cudaStream_t st);
+
+}  // namespace trk

@@ -1,0 +1,355 @@
+// S2: fixed-radius nearest-neighbour graph in the latent space (the paper used the
+// FRNN CUDA package, line 87).  Definition (readings C-7..C-9, C-11, C-21):
+//   edge i -> j  iff  same event, outer(i,j), d2(i,j) <= r^2, and j is among the K smallest (d2, j).
+// d2 is accumulated in fp64 from the fp32 embedding, k ascending, with separate multiply and add
+// (__dsub_rn/__dmul_rn/__dadd_rn forbid FMA contraction), so accept and rank decisions are exact
+// functions of the inputs and the edge list is unique.
+//
+// Search structure (an implementation detail that cannot change the result): hits are binned on
+// g <= 3 coordinates of P^T e (P has orthonormal columns, so projected distance <= true distance)
+// into a per-event grid with cell edge >= r; a query looks at the 3^g neighbouring cells.  Hits
+// are counting-sorted by cell so a row of 3 x-adjacent cells is one contiguous candidate range.
+// One warp serves one query: lanes stride over the candidates, accepted ones are appended to a
+// shared-memory buffer via ballot, and a warp bitonic sort on (d2, j) prunes to the K nearest
+// whenever the buffer fills; a final sort on j gives the (src, dst) output order.
+#include "common.cuh"
+
+namespace trk {
+namespace {
+
+__device__ __forceinline__ int float_to_ordered(float f) {
+  int i = __float_as_int(f);
+  return i >= 0 ? i : i ^ 0x7fffffff;
+}
+__device__ __forceinline__ float ordered_to_float(int i) { return __int_as_float(i >= 0 ? i : i ^ 0x7fffffff); }
+
+__global__ void frnn_reset_kernel(int32_t* __restrict__ bbox, int32_t* __restrict__ cell_count, int64_t n_cells_plus1) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < 3) {
+    bbox[i] = 0x7fffffff;          // min
+    bbox[3 + i] = (int)0x80000000; // max
+  }
+  if (i < n_cells_plus1) cell_count[i] = 0;
+}
+
+// proj[i] = P^T e_i  (or the first g coordinates), and the global bounding box.
+__global__ void frnn_project_kernel(const float* __restrict__ emb, int d_e, const float* __restrict__ P, int g,
+                                    float* __restrict__ proj, int32_t* __restrict__ bbox, int64_t n) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  float p[3] = {0.f, 0.f, 0.f};
+  if (i < n) {
+    const float* e = emb + i * d_e;
+    if (P) {
+      for (int k = 0; k < d_e; ++k) {
+        float v = e[k];
+        for (int a = 0; a < g; ++a) p[a] = fmaf(v, P[k * 3 + a], p[a]);
+      }
+    } else {
+      for (int a = 0; a < g; ++a) p[a] = e[a];
+    }
+    proj[i * 3 + 0] = p[0];
+    proj[i * 3 + 1] = p[1];
+    proj[i * 3 + 2] = p[2];
+  }
+  // warp-reduce then one atomic per warp and axis
+  for (int a = 0; a < 3; ++a) {
+    int lo = i < n ? float_to_ordered(p[a]) : 0x7fffffff;
+    int hi = i < n ? float_to_ordered(p[a]) : (int)0x80000000;
+    for (int o = 16; o > 0; o >>= 1) {
+      lo = min(lo, __shfl_xor_sync(0xffffffffu, lo, o));
+      hi = max(hi, __shfl_xor_sync(0xffffffffu, hi, o));
+    }
+    if ((threadIdx.x & 31) == 0) {
+      atomicMin(&bbox[a], lo);
+      atomicMax(&bbox[3 + a], hi);
+    }
+  }
+}
+
+__global__ void frnn_grid_setup_kernel(const int32_t* __restrict__ bbox, float radius, int g, int G, GridParams* __restrict__ gp) {
+  if (threadIdx.x != 0 || blockIdx.x != 0) return;
+  // cell edge >= r with slack for the fp32 rounding of the projection (|p| of order 1..10, error ~1e-6)
+  const float cell_min = radius * 1.001f + 1e-5f;
+  int cells = 1;
+  for (int a = 0; a < 3; ++a) {
+    if (a >= g) {
+      gp->origin[a] = 0.f;
+      gp->inv_cell[a] = 0.f;
+      gp->dims[a] = 1;
+      continue;
+    }
+    float lo = ordered_to_float(bbox[a]), hi = ordered_to_float(bbox[3 + a]);
+    if (!(hi >= lo)) { lo = 0.f; hi = 0.f; }
+    float extent = hi - lo;
+    float cell = fmaxf(cell_min, extent / (float)G * 1.0001f);
+    int d = (int)floorf(extent / cell) + 1;
+    d = max(1, min(d, G));
+    gp->origin[a] = lo;
+    gp->inv_cell[a] = 1.0f / cell;
+    gp->dims[a] = d;
+    cells *= d;
+  }
+  gp->cells_per_event = cells;
+}
+
+__device__ __forceinline__ void cell_coords(const GridParams& gp, const float* p, int c[3]) {
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    int v = (int)floorf((p[a] - gp.origin[a]) * gp.inv_cell[a]);
+    c[a] = max(0, min(v, gp.dims[a] - 1));   // clamping is monotone, so neighbours stay neighbours
+  }
+}
+
+__global__ void frnn_count_kernel(const float* __restrict__ proj, const int32_t* __restrict__ ev_of_hit,
+                                  const GridParams* __restrict__ gpp, int32_t* __restrict__ cell_of_hit,
+                                  int32_t* __restrict__ cell_count, int64_t n) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const GridParams gp = *gpp;
+  int c[3];
+  cell_coords(gp, proj + i * 3, c);
+  int cell = ev_of_hit[i] * gp.cells_per_event + (c[2] * gp.dims[1] + c[1]) * gp.dims[0] + c[0];
+  cell_of_hit[i] = cell;
+  atomicAdd(&cell_count[cell], 1);
+}
+
+// Sorted records: semb[pos][D] and smeta[pos] = (r, |z|, index, cell).
+__global__ void frnn_scatter_kernel(const float* __restrict__ emb, const float* __restrict__ hits, int d_e, int d_pad,
+                                    const int32_t* __restrict__ cell_of_hit, const int32_t* __restrict__ cell_start,
+                                    int32_t* __restrict__ cell_fill, float* __restrict__ semb, float4* __restrict__ smeta,
+                                    int64_t n) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const int cell = cell_of_hit[i];
+  const int pos = cell_start[cell] + atomicAdd(&cell_fill[cell], 1);
+  for (int k = 0; k < d_pad; ++k) semb[(int64_t)pos * d_pad + k] = k < d_e ? emb[i * d_e + k] : 0.f;
+  smeta[pos] = make_float4(hits[i * 3 + 0], fabsf(hits[i * 3 + 2]), __int_as_float((int)i), __int_as_float(cell));
+}
+
+// ---- warp-level bitonic sort of n (power of two) entries held in shared memory ----
+// by_index = false: key (d2 bits, idx);  true: key idx only.
+__device__ __forceinline__ void warp_bitonic(unsigned long long* d2, int* idx, int n, bool by_index, int lane) {
+  for (int k = 2; k <= n; k <<= 1) {
+    for (int j = k >> 1; j > 0; j >>= 1) {
+      for (int t = lane; t < n; t += 32) {
+        const int l = t ^ j;
+        if (l > t) {
+          const unsigned long long a = d2[t], b = d2[l];
+          const int ia = idx[t], ib = idx[l];
+          const bool a_gt_b = by_index ? (ia > ib) : (a > b || (a == b && ia > ib));
+          const bool up = (t & k) == 0;
+          if (a_gt_b == up) {
+            d2[t] = b; d2[l] = a;
+            idx[t] = ib; idx[l] = ia;
+          }
+        }
+      }
+      __syncwarp();
+    }
+  }
+}
+
+constexpr unsigned long long kInfBits = 0x7ff0000000000000ull;
+constexpr int kWarpsPerBlock = 4;
+
+template <int D4, int CAP>
+__global__ void __launch_bounds__(kWarpsPerBlock * 32)
+frnn_search_kernel(const float* __restrict__ semb, const float4* __restrict__ smeta, const int32_t* __restrict__ cell_start,
+                   const GridParams* __restrict__ gpp, double r2, int K, int32_t* __restrict__ slots, int32_t* __restrict__ deg,
+                   int64_t n) {
+  constexpr int D = D4 * 4;
+  __shared__ unsigned long long s_d2[kWarpsPerBlock][CAP];
+  __shared__ int s_idx[kWarpsPerBlock][CAP];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int64_t q = (int64_t)blockIdx.x * kWarpsPerBlock + warp;
+  if (q >= n) return;
+  unsigned long long* bd2 = s_d2[warp];
+  int* bidx = s_idx[warp];
+  const GridParams gp = *gpp;
+
+  const float4 qm = smeta[q];
+  const float q_r = qm.x, q_az = qm.y;
+  const int q_i = __float_as_int(qm.z);
+  int cell = __float_as_int(qm.w);
+  const int ev = cell / gp.cells_per_event;
+  cell -= ev * gp.cells_per_event;
+  const int cx = cell % gp.dims[0];
+  const int cy = (cell / gp.dims[0]) % gp.dims[1];
+  const int cz = cell / (gp.dims[0] * gp.dims[1]);
+  double qe[D];
+#pragma unroll
+  for (int k4 = 0; k4 < D4; ++k4) {
+    const float4 v = reinterpret_cast<const float4*>(semb + q * D)[k4];
+    qe[k4 * 4 + 0] = (double)v.x; qe[k4 * 4 + 1] = (double)v.y; qe[k4 * 4 + 2] = (double)v.z; qe[k4 * 4 + 3] = (double)v.w;
+  }
+
+  int count = 0;  // warp-uniform number of buffered candidates
+  for (int t = lane; t < CAP; t += 32) { bd2[t] = kInfBits; bidx[t] = 0x7fffffff; }
+  __syncwarp();
+
+  const int x0 = max(cx - 1, 0), x1 = min(cx + 1, gp.dims[0] - 1);
+  for (int dz = -1; dz <= 1; ++dz) {
+    const int z = cz + dz;
+    if (z < 0 || z >= gp.dims[2]) continue;
+    for (int dy = -1; dy <= 1; ++dy) {
+      const int y = cy + dy;
+      if (y < 0 || y >= gp.dims[1]) continue;
+      const int row = ev * gp.cells_per_event + (z * gp.dims[1] + y) * gp.dims[0];
+      const int lo = cell_start[row + x0], hi = cell_start[row + x1 + 1];
+      for (int base = lo; base < hi; base += 32) {
+        const int pos = base + lane;
+        bool ok = false;
+        double d2 = 0.0;
+        int c_i = 0;
+        if (pos < hi) {
+          const float4 cm = smeta[pos];
+          c_i = __float_as_int(cm.z);
+          // outer(i,j): (r_i, |z_i|, i) < (r_j, |z_j|, j)
+          const bool outer = (q_r < cm.x) || (q_r == cm.x && (q_az < cm.y || (q_az == cm.y && q_i < c_i)));
+          if (outer) {
+            const float4* ce = reinterpret_cast<const float4*>(semb + (int64_t)pos * D);
+#pragma unroll
+            for (int k4 = 0; k4 < D4; ++k4) {
+              const float4 v = ce[k4];
+              double t;
+              t = __dsub_rn(qe[k4 * 4 + 0], (double)v.x); d2 = __dadd_rn(d2, __dmul_rn(t, t));
+              t = __dsub_rn(qe[k4 * 4 + 1], (double)v.y); d2 = __dadd_rn(d2, __dmul_rn(t, t));
+              t = __dsub_rn(qe[k4 * 4 + 2], (double)v.z); d2 = __dadd_rn(d2, __dmul_rn(t, t));
+              t = __dsub_rn(qe[k4 * 4 + 3], (double)v.w); d2 = __dadd_rn(d2, __dmul_rn(t, t));
+            }
+            ok = d2 <= r2;
+          }
+        }
+        const unsigned m = __ballot_sync(0xffffffffu, ok);
+        if (m) {
+          if (count + 32 > CAP) {  // make room: keep the K nearest so far
+            warp_bitonic(bd2, bidx, CAP, false, lane);
+            for (int t = K + lane; t < CAP; t += 32) { bd2[t] = kInfBits; bidx[t] = 0x7fffffff; }
+            __syncwarp();
+            count = min(count, K);
+          }
+          if (ok) {
+            const int slot = count + __popc(m & ((1u << lane) - 1u));
+            bd2[slot] = (unsigned long long)__double_as_longlong(d2);
+            bidx[slot] = c_i;
+          }
+          count += __popc(m);
+          __syncwarp();
+        }
+      }
+    }
+  }
+  if (count > K) {
+    warp_bitonic(bd2, bidx, CAP, false, lane);
+    for (int t = K + lane; t < CAP; t += 32) { bd2[t] = kInfBits; bidx[t] = 0x7fffffff; }
+    __syncwarp();
+    count = K;
+  }
+  // order the kept neighbours by index; unused entries hold INT_MAX and sort to the end
+  int nsort = 32;
+  while (nsort < count) nsort <<= 1;
+  warp_bitonic(bd2, bidx, nsort, true, lane);
+  for (int t = lane; t < count; t += 32) slots[(int64_t)q_i * K + t] = bidx[t];
+  if (lane == 0) deg[q_i] = count;
+}
+
+__global__ void frnn_emit_kernel(const int32_t* __restrict__ slots, const int32_t* __restrict__ rowptr, int K,
+                                 int32_t* __restrict__ src, int32_t* __restrict__ dst, int32_t* __restrict__ rowptr_out,
+                                 int64_t capacity, int32_t* __restrict__ count_out, int32_t* __restrict__ overflow_flag, int64_t n) {
+  // one warp per hit
+  const int lane = threadIdx.x & 31;
+  const int64_t i = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  if (i > n) return;
+  if (i == n) {
+    if (lane == 0) {
+      const int64_t tot = rowptr[n];
+      *count_out = (int32_t)min(tot, capacity);
+      if (tot > capacity) *overflow_flag = 1;
+      if (rowptr_out) rowptr_out[n] = (int32_t)min(tot, capacity);
+    }
+    return;
+  }
+  const int64_t b = rowptr[i], e = rowptr[i + 1];
+  if (rowptr_out && lane == 0) rowptr_out[i] = (int32_t)min(b, capacity);
+  for (int64_t t = lane; t < e - b; t += 32) {
+    if (b + t < capacity) {
+      src[b + t] = (int32_t)i;
+      dst[b + t] = slots[i * K + t];
+    }
+  }
+}
+
+// Event offsets travel as a kernel parameter (by value), so trk_infer needs no staging copy and
+// stays graph-capturable.
+__global__ void event_of_hit_kernel(const __grid_constant__ EventOffsets offs, int n_events, int32_t* __restrict__ ev_of_hit, int64_t n) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  int lo = 0, hi = n_events;  // offsets[lo] <= i < offsets[hi]
+  while (hi - lo > 1) {
+    int mid = (lo + hi) >> 1;
+    if (offs.v[mid] <= i) lo = mid; else hi = mid;
+  }
+  ev_of_hit[i] = lo;
+}
+
+template <int D4>
+trk_status launch_search(trk_ctx* ctx, int K, double r2, int64_t n, cudaStream_t st) {
+  const unsigned blocks = (unsigned)ceil_div(n, kWarpsPerBlock);
+  if (K <= 32) {
+    TRK_LAUNCH(ctx, (frnn_search_kernel<D4, 64>), blocks, kWarpsPerBlock * 32, 0, st, ctx->semb, ctx->smeta, ctx->cell_start,
+               ctx->grid, r2, K, ctx->slots, ctx->deg, n);
+  } else if (K <= 64) {
+    TRK_LAUNCH(ctx, (frnn_search_kernel<D4, 128>), blocks, kWarpsPerBlock * 32, 0, st, ctx->semb, ctx->smeta, ctx->cell_start,
+               ctx->grid, r2, K, ctx->slots, ctx->deg, n);
+  } else {
+    TRK_LAUNCH(ctx, (frnn_search_kernel<D4, 256>), blocks, kWarpsPerBlock * 32, 0, st, ctx->semb, ctx->smeta, ctx->cell_start,
+               ctx->grid, r2, K, ctx->slots, ctx->deg, n);
+  }
+  return TRK_OK;
+}
+
+}  // namespace
+
+// ev_of_hit must already hold the event id of every hit (see set_event_ids in api.cu).
+trk_status frnn_build(trk_ctx* ctx, const float* emb, const float* hits, int64_t n, int32_t n_events, int32_t* src,
+                      int32_t* dst, int32_t* rowptr_out, int64_t capacity, int32_t* count_out, int32_t* overflow_flag,
+                      cudaStream_t st) {
+  const int K = ctx->cfg.frnn_k;
+  const int g = ctx->grid_dims;
+  const int G = ctx->grid_max;
+  const int64_t n_cells = (int64_t)n_events * G * G * G;
+  if (n_cells > ctx->max_cells) return fail(ctx, TRK_ERR_CAPACITY, "frnn: n_events exceeds max_events");
+  if (n <= 0) return fail(ctx, TRK_ERR_INVALID_ARG, "frnn: empty input");
+  const unsigned nb = (unsigned)ceil_div(n, 256);
+  // only the cells of this call's events are touched
+  TRK_LAUNCH(ctx, frnn_reset_kernel, (unsigned)ceil_div(n_cells + 1, 256), 256, 0, st, ctx->bbox, ctx->cell_count, n_cells + 1);
+  TRK_LAUNCH(ctx, frnn_project_kernel, nb, 256, 0, st, emb, ctx->d_e, ctx->grid_proj, g, ctx->proj, ctx->bbox, n);
+  TRK_LAUNCH(ctx, frnn_grid_setup_kernel, 1, 32, 0, st, ctx->bbox, ctx->cfg.frnn_radius, g, G, ctx->grid);
+  TRK_LAUNCH(ctx, frnn_count_kernel, nb, 256, 0, st, ctx->proj, ctx->ev_of_hit, ctx->grid, ctx->cell_of_hit, ctx->cell_count, n);
+  TRK_TRY(exclusive_scan_i32(ctx, ctx->cell_count, ctx->cell_start, n_cells, ctx->scan_tmp, st));
+  TRK_TRY(fill_i32(ctx, ctx->cell_fill, 0, n_cells, st));
+  TRK_LAUNCH(ctx, frnn_scatter_kernel, nb, 256, 0, st, emb, hits, ctx->d_e, ctx->d_e_pad, ctx->cell_of_hit, ctx->cell_start,
+             ctx->cell_fill, ctx->semb, ctx->smeta, n);
+  const double r = (double)ctx->cfg.frnn_radius;
+  const double r2 = r * r;
+  switch (ctx->d_e_pad / 4) {
+    case 1: TRK_TRY(launch_search<1>(ctx, K, r2, n, st)); break;
+    case 2: TRK_TRY(launch_search<2>(ctx, K, r2, n, st)); break;
+    case 3: TRK_TRY(launch_search<3>(ctx, K, r2, n, st)); break;
+    default: TRK_TRY(launch_search<4>(ctx, K, r2, n, st)); break;
+  }
+  TRK_TRY(exclusive_scan_i32(ctx, ctx->deg, ctx->rowptr, n, ctx->scan_tmp, st));
+  TRK_LAUNCH(ctx, frnn_emit_kernel, (unsigned)ceil_div((n + 1) * 32, 256), 256, 0, st, ctx->slots, ctx->rowptr, K, src, dst,
+             rowptr_out, capacity, count_out, overflow_flag, n);
+  return TRK_OK;
+}
+
+trk_status set_event_ids(trk_ctx* ctx, const int32_t* offsets_host, int n_events, int64_t n, cudaStream_t st) {
+  if (n <= 0) return TRK_OK;
+  EventOffsets offs;
+  for (int i = 0; i <= n_events; ++i) offs.v[i] = offsets_host[i];
+  TRK_LAUNCH(ctx, event_of_hit_kernel, (unsigned)ceil_div(n, 256), 256, 0, st, offs, n_events, ctx->ev_of_hit, n);
+  return TRK_OK;
+}
+
+}  // namespace trk

@@ -1,0 +1,138 @@
+// Graph bookkeeping for S4 message passing: the kept edge list is sorted by
+// (src, dst) and static over the T iterations, so both aggregations
+//     m_out_v = sum_{k: src(k)=v} e_k        m_in_v = sum_{k: dst(k)=v} e_k
+// are atomic-free segmented sums over a CSR built once per call: out-edges are already
+// contiguous; in-edges go through a dst-sorted permutation whose segments are ordered by edge
+// index, so the fp32 summation order is fixed and results are run-to-run identical
+// (PAPER.md line 164 identity check; reading C-14: fp32 accumulation).
+#include "common.cuh"
+#include "graph.cuh"
+
+namespace trk {
+namespace {
+
+__device__ __forceinline__ int64_t dev_count(const int32_t* n_dev, int64_t cap) {
+  return n_dev ? min((int64_t)max(*n_dev, 0), cap) : cap;
+}
+
+// rowptr[v] = first k with key[k] >= v, for sorted keys; rowptr[n_nodes] = n_edges.
+__global__ void rowptr_from_sorted_kernel(const int32_t* __restrict__ key, const int32_t* __restrict__ n_dev, int64_t cap,
+                                          int32_t* __restrict__ rowptr, int64_t n_nodes) {
+  const int64_t n_edges = dev_count(n_dev, cap);
+  const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (k > n_edges) return;
+  const int64_t prev = k == 0 ? -1 : key[k - 1];
+  const int64_t cur = k == n_edges ? n_nodes : key[k];
+  for (int64_t v = prev + 1; v <= cur; ++v) rowptr[v] = (int32_t)k;
+}
+
+__global__ void count_keys_kernel(const int32_t* __restrict__ key, const int32_t* __restrict__ n_dev, int64_t cap,
+                                  int32_t* __restrict__ count) {
+  const int64_t n_edges = dev_count(n_dev, cap);
+  const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (k < n_edges) atomicAdd(&count[key[k]], 1);
+}
+
+__global__ void place_keys_kernel(const int32_t* __restrict__ key, const int32_t* __restrict__ n_dev, int64_t cap,
+                                  const int32_t* __restrict__ rowptr, int32_t* __restrict__ fill, int32_t* __restrict__ perm) {
+  const int64_t n_edges = dev_count(n_dev, cap);
+  const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (k < n_edges) {
+    const int v = key[k];
+    perm[rowptr[v] + atomicAdd(&fill[v], 1)] = (int32_t)k;
+  }
+}
+
+// Each segment of perm is put in ascending edge order (segments are short: mean in-degree ~10).
+__global__ void sort_segments_kernel(const int32_t* __restrict__ rowptr, int32_t* __restrict__ perm, int64_t n_nodes) {
+  const int64_t v = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (v >= n_nodes) return;
+  const int b = rowptr[v], e = rowptr[v + 1];
+  for (int i = b + 1; i < e; ++i) {
+    const int x = perm[i];
+    int j = i - 1;
+    while (j >= b && perm[j] > x) {
+      perm[j + 1] = perm[j];
+      --j;
+    }
+    perm[j + 1] = x;
+  }
+}
+
+template <typename T>
+__device__ __forceinline__ float4 load4(const T* p);
+template <>
+__device__ __forceinline__ float4 load4<float>(const float* p) { return *reinterpret_cast<const float4*>(p); }
+template <>
+__device__ __forceinline__ float4 load4<__nv_bfloat16>(const __nv_bfloat16* p) {
+  const uint2 u = *reinterpret_cast<const uint2*>(p);
+  const __nv_bfloat162 a = *reinterpret_cast<const __nv_bfloat162*>(&u.x);
+  const __nv_bfloat162 b = *reinterpret_cast<const __nv_bfloat162*>(&u.y);
+  return make_float4(__low2float(a), __high2float(a), __low2float(b), __high2float(b));
+}
+template <typename T>
+__device__ __forceinline__ void store4(T* p, float4 v);
+template <>
+__device__ __forceinline__ void store4<float>(float* p, float4 v) { *reinterpret_cast<float4*>(p) = v; }
+template <>
+__device__ __forceinline__ void store4<__nv_bfloat16>(__nv_bfloat16* p, float4 v) {
+  __nv_bfloat162 a = __floats2bfloat162_rn(v.x, v.y), b = __floats2bfloat162_rn(v.z, v.w);
+  uint2 u;
+  u.x = *reinterpret_cast<unsigned*>(&a);
+  u.y = *reinterpret_cast<unsigned*>(&b);
+  *reinterpret_cast<uint2*>(p) = u;
+}
+
+// One warp per (node, direction): X[v][H + dir*H + :] = sum over the segment of E rows (fp32 accumulate).
+// H is a multiple of 4; lanes cover H/4 float4 columns in strides of 32.
+template <typename T>
+__global__ void __launch_bounds__(256)
+segment_sum_kernel(const T* __restrict__ E, int H, const int32_t* __restrict__ in_rowptr, const int32_t* __restrict__ in_perm,
+                   const int32_t* __restrict__ out_rowptr, T* __restrict__ X, int ldx, int64_t n_nodes) {
+  const int lane = threadIdx.x & 31;
+  const int64_t w = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  if (w >= 2 * n_nodes) return;
+  const int64_t v = w >> 1;
+  const int dir = (int)(w & 1);  // 0: in (dst == v, via perm), 1: out (src == v, contiguous)
+  const int32_t* rp = dir == 0 ? in_rowptr : out_rowptr;
+  const int b = rp[v], e = rp[v + 1];
+  for (int c = lane * 4; c < H; c += 128) {
+    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int k = b; k < e; ++k) {
+      const int64_t row = dir == 0 ? in_perm[k] : k;
+      const float4 x = load4<T>(E + row * H + c);
+      acc.x += x.x; acc.y += x.y; acc.z += x.z; acc.w += x.w;
+    }
+    store4<T>(X + v * ldx + H + dir * H + c, acc);
+  }
+}
+
+}  // namespace
+
+trk_status build_gnn_csr(trk_ctx* ctx, const int32_t* src, const int32_t* dst, const int32_t* n_edges_dev, int64_t n_edges_cap,
+                         int64_t n_nodes, cudaStream_t st) {
+  const unsigned eb = (unsigned)ceil_div(n_edges_cap + 1, 256);
+  TRK_LAUNCH(ctx, rowptr_from_sorted_kernel, eb, 256, 0, st, src, n_edges_dev, n_edges_cap, ctx->out_rowptr, n_nodes);
+  TRK_TRY(fill_i32(ctx, ctx->in_fill, 0, n_nodes + 1, st));
+  TRK_LAUNCH(ctx, count_keys_kernel, eb, 256, 0, st, dst, n_edges_dev, n_edges_cap, ctx->in_fill);
+  TRK_TRY(exclusive_scan_i32(ctx, ctx->in_fill, ctx->in_rowptr, n_nodes, ctx->scan_tmp, st));
+  TRK_TRY(fill_i32(ctx, ctx->in_fill, 0, n_nodes, st));
+  TRK_LAUNCH(ctx, place_keys_kernel, eb, 256, 0, st, dst, n_edges_dev, n_edges_cap, ctx->in_rowptr, ctx->in_fill, ctx->in_perm);
+  TRK_LAUNCH(ctx, sort_segments_kernel, (unsigned)ceil_div(n_nodes, 128), 128, 0, st, ctx->in_rowptr, ctx->in_perm, n_nodes);
+  return TRK_OK;
+}
+
+trk_status segment_sums(trk_ctx* ctx, const void* E, bool bf16, int64_t n_nodes, void* X, cudaStream_t st) {
+  const int H = ctx->H;
+  const unsigned blocks = (unsigned)ceil_div(2 * n_nodes * 32, 256);
+  if (bf16) {
+    TRK_LAUNCH(ctx, segment_sum_kernel<__nv_bfloat16>, blocks, 256, 0, st, (const __nv_bfloat16*)E, H, ctx->in_rowptr,
+               ctx->in_perm, ctx->out_rowptr, (__nv_bfloat16*)X, 3 * H, n_nodes);
+  } else {
+    TRK_LAUNCH(ctx, segment_sum_kernel<float>, blocks, 256, 0, st, (const float*)E, H, ctx->in_rowptr, ctx->in_perm,
+               ctx->out_rowptr, (float*)X, 3 * H, n_nodes);
+  }
+  return TRK_OK;
+}
+
+}  // namespace trk
