@@ -71,6 +71,8 @@ struct trk_ctx {
   __nv_bfloat16* edge_dec_wab = nullptr;
   __nv_bfloat16* edge_dec_wc = nullptr;
   __nv_bfloat16* filter_w1_pad = nullptr;  // [1024][64] = W1 zero padded in K
+  float filter_b_last = 0.f;               // bias of the filter's final Linear(W -> 1)
+  float edge_dec_b_last = 0.f;             // bias of the decoder's final Linear(H -> 1)
 
   trk::Workspace ws;
   // ---- workspace carve-up (device pointers into ws.base) ----
@@ -118,6 +120,10 @@ struct trk_ctx {
   int32_t* out_rowptr = nullptr;    // [max_hits+1] CSR by src (edges are src-sorted)
   // S5
   int32_t* parent = nullptr;        // [max_hits]
+  // trk_infer_host staging (device side)
+  float* io_hits = nullptr;         // [max_hits][3]
+  int32_t* io_labels = nullptr;     // [max_hits]
+  int32_t* io_counts = nullptr;     // [4]
 };
 
 namespace trk {
@@ -167,11 +173,5 @@ trk_status cc_labels(trk_ctx* ctx, int64_t n, const int32_t* src, const int32_t*
                      const int32_t* n_edges_dev, int64_t n_edges_cap, float cut, int32_t* labels, int32_t* pass_count,
                      cudaStream_t st);
 
-// ---- nn_fp32.cu / nn_bf16.cu: S1, S3, S4 ----
-trk_status embed_forward(trk_ctx* ctx, const float* hits, int64_t n, float* emb, cudaStream_t st);
-trk_status filter_forward(trk_ctx* ctx, const float* feat, const int32_t* src, const int32_t* dst,
-                          const int32_t* n_edges_dev, int64_t n_edges_cap, float* score, cudaStream_t st);
-trk_status gnn_forward(trk_ctx* ctx, const float* hits, int64_t n, const int32_t* src, const int32_t* dst,
-                       const int32_t* n_edges_dev, int64_t n_edges_cap, float* score, cudaStream_t st);
 
 }  // namespace trk

@@ -1,0 +1,341 @@
+// TRK_BF16 precision: S1, S3 and S4 with every dense layer on the tcgen05 tensor cores
+// (gemm_tc.cuh); layers whose K is 3 or 4 run on the plain ALUs in fp32 (they are <0.1% of the flops).
+//
+// S1   hits -> [SIMT 3->W] -> GEMM+ReLU ... -> GEMM (N padded to 16, fp32 out) = embedding
+// S3   per chunk of 18944 edges (one 128-row tile per SM and N-tile column, activations L2 resident):
+//        gather [e_src ; e_dst] -> bf16 [rows][64] (K zero-padded) -> GEMM+ReLU ... -> last hidden GEMM
+//        with the final Linear(W->1) folded into its epilogue as per-tile partial dots -> sigmoid
+// S4   the first layer of edge_net / edge_dec is split exactly:
+//        W1 [h_s ; h_d ; e] = Wa h_s + Wb h_d + Wc e
+//      so one per-node GEMM (N = 2H) produces PA|PB in fp32 and the per-edge GEMM has K = H only;
+//      the epilogue gathers PA[src] + PB[dst], applies LayerNorm+ReLU (+ residual) in registers.
+//      This halves the per-edge flops against the dense concat.
+#include <mutex>
+
+#include "common.cuh"
+#include "gemm_tc.cuh"
+#include "graph.cuh"
+#include "nn.cuh"
+
+namespace trk {
+namespace {
+
+using bf16 = __nv_bfloat16;
+
+// ---------------------------------------------------------------- tensor maps
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn get_encode_fn() {
+  static EncodeTiledFn fn = nullptr;
+  static std::once_flag once;
+  std::call_once(once, [] {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) == cudaSuccess &&
+        qres == cudaDriverEntryPointSuccess)
+      fn = reinterpret_cast<EncodeTiledFn>(p);
+  });
+  return fn;
+}
+
+// bf16 matrix [rows][k] with row stride ld (elements); box = 64 (k) x box_rows; 128-byte swizzle.
+trk_status make_tmap(trk_ctx* ctx, CUtensorMap* m, const void* base, int64_t rows, int k, int64_t ld, int box_rows) {
+  EncodeTiledFn fn = get_encode_fn();
+  if (!fn) return fail(ctx, TRK_ERR_CUDA, "cuTensorMapEncodeTiled entry point not found");
+  cuuint64_t dims[2] = {(cuuint64_t)k, (cuuint64_t)(rows > 0 ? rows : 1)};
+  cuuint64_t strides[1] = {(cuuint64_t)ld * 2};
+  cuuint32_t box[2] = {64u, (cuuint32_t)box_rows};
+  cuuint32_t estr[2] = {1u, 1u};
+  CUresult r = fn(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), dims, strides, box, estr,
+                  CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                  CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return fail(ctx, TRK_ERR_CUDA, "cuTensorMapEncodeTiled failed with code " + std::to_string((int)r));
+  return TRK_OK;
+}
+
+// A [a_rows][K] bf16 (row stride lda), W [n_pad][K] bf16 K-major; rows of the product resolved on the device.
+template <int BN, class Epi>
+trk_status launch_gemm(trk_ctx* ctx, const bf16* A, int64_t a_rows, int64_t lda, int K, const bf16* W, int n_pad, tc::Rows rows,
+                       const typename Epi::Params& ep, cudaStream_t st) {
+  if (rows.m_cap <= 0) return TRK_OK;
+  if (K % tc::BK != 0 || n_pad % BN != 0) return fail(ctx, TRK_ERR_SHAPE, "gemm: K must be a multiple of 64 and N of the tile");
+  static bool attr_set = false;
+  auto kern = tc::gemm_tc_kernel<BN, Epi>;
+  if (!attr_set) {
+    TRK_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::smem_bytes(BN)));
+    attr_set = true;
+  }
+  CUtensorMap ta, tb;
+  TRK_TRY(make_tmap(ctx, &ta, A, a_rows, K, lda, tc::BM));
+  TRK_TRY(make_tmap(ctx, &tb, W, n_pad, K, K, BN));
+  const int n_tiles = n_pad / BN;
+  const int64_t tiles = ceil_div(rows.m_cap, tc::BM) * n_tiles;
+  const unsigned grid = (unsigned)std::min<int64_t>(tiles, ctx->sm_count);
+  TRK_LAUNCH(ctx, kern, grid, tc::kThreads, tc::smem_bytes(BN), st, ta, tb, rows, n_tiles, K / tc::BK, ep);
+  return TRK_OK;
+}
+
+int pick_bn(int n_pad) { return n_pad % 256 == 0 ? 256 : (n_pad % 128 == 0 ? 128 : 64); }
+
+trk_status gemm_bias_act(trk_ctx* ctx, const bf16* A, int64_t a_rows, int64_t lda, const DevLinear& L, bf16* out, int ldo, int relu,
+                         tc::Rows rows, cudaStream_t st) {
+  tc::EpiBiasActBf16::Params ep{L.b_f32, out, ldo, relu};
+  switch (pick_bn(L.out_pad)) {
+    case 256: return launch_gemm<256, tc::EpiBiasActBf16>(ctx, A, a_rows, lda, L.in_pad, L.w_bf16, L.out_pad, rows, ep, st);
+    case 128: return launch_gemm<128, tc::EpiBiasActBf16>(ctx, A, a_rows, lda, L.in_pad, L.w_bf16, L.out_pad, rows, ep, st);
+    default: return launch_gemm<64, tc::EpiBiasActBf16>(ctx, A, a_rows, lda, L.in_pad, L.w_bf16, L.out_pad, rows, ep, st);
+  }
+}
+
+trk_status gemm_relu_dot(trk_ctx* ctx, const bf16* A, int64_t a_rows, int64_t lda, const DevLinear& L, const float* w_last,
+                         float* partial, int* n_tiles_out, tc::Rows rows, cudaStream_t st) {
+  const int bn = pick_bn(L.out_pad);
+  tc::EpiReluDot::Params ep{L.b_f32, w_last, partial, L.out_pad / bn};
+  *n_tiles_out = L.out_pad / bn;
+  switch (bn) {
+    case 256: return launch_gemm<256, tc::EpiReluDot>(ctx, A, a_rows, lda, L.in_pad, L.w_bf16, L.out_pad, rows, ep, st);
+    case 128: return launch_gemm<128, tc::EpiReluDot>(ctx, A, a_rows, lda, L.in_pad, L.w_bf16, L.out_pad, rows, ep, st);
+    default: return launch_gemm<64, tc::EpiReluDot>(ctx, A, a_rows, lda, L.in_pad, L.w_bf16, L.out_pad, rows, ep, st);
+  }
+}
+
+trk_status gemm_store_f32(trk_ctx* ctx, const bf16* A, int64_t a_rows, int64_t lda, int K, const bf16* W, int n_pad, float* out,
+                          tc::Rows rows, cudaStream_t st) {
+  tc::EpiStoreF32::Params ep{out, n_pad};
+  if (n_pad % 256 == 0) return launch_gemm<256, tc::EpiStoreF32>(ctx, A, a_rows, lda, K, W, n_pad, rows, ep, st);
+  return launch_gemm<128, tc::EpiStoreF32>(ctx, A, a_rows, lda, K, W, n_pad, rows, ep, st);
+}
+
+trk_status gemm_row_ln(trk_ctx* ctx, const bf16* A, int64_t a_rows, int64_t lda, int K, const bf16* W, tc::EpiRowLn::Params ep,
+                       tc::Rows rows, cudaStream_t st) {
+  if (ctx->H == 128) return launch_gemm<128, tc::EpiRowLn>(ctx, A, a_rows, lda, K, W, 128, rows, ep, st);
+  return launch_gemm<64, tc::EpiRowLn>(ctx, A, a_rows, lda, K, W, 64, rows, ep, st);
+}
+
+// ---------------------------------------------------------------- small SIMT kernels
+__device__ __forceinline__ int64_t rows_of(const int32_t* m_dev, int64_t m_off, int64_t m_cap) {
+  if (!m_dev) return m_cap;
+  int64_t m = (int64_t)*m_dev - m_off;
+  return m < 0 ? 0 : (m > m_cap ? m_cap : m);
+}
+
+// S1 first layer: out[m][n] = bf16(relu(W[n][0..3) . x[m] + b[n])), 8 columns per thread.
+__global__ void embed_first_layer_kernel(const float* __restrict__ hits, const float* __restrict__ W, const float* __restrict__ b,
+                                         bf16* __restrict__ out, int64_t M, int N) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int groups = N / 8;
+  const int64_t row = i / groups;
+  if (row >= M) return;
+  const int c0 = (int)(i % groups) * 8;
+  const float x0 = hits[row * 3], x1 = hits[row * 3 + 1], x2 = hits[row * 3 + 2];
+  float v[8];
+#pragma unroll
+  for (int j = 0; j < 8; ++j) {
+    const float* w = W + (int64_t)(c0 + j) * 3;
+    v[j] = fmaxf(fmaf(w[2], x2, fmaf(w[1], x1, fmaf(w[0], x0, b[c0 + j]))), 0.f);
+  }
+  *reinterpret_cast<uint4*>(out + row * N + c0) =
+      make_uint4(tc::pack_bf16(v[0], v[1]), tc::pack_bf16(v[2], v[3]), tc::pack_bf16(v[4], v[5]), tc::pack_bf16(v[6], v[7]));
+}
+
+// S3 input rows: out[m][0..64) = bf16([feat[src] ; feat[dst]]) zero padded; 8 columns per thread.
+__global__ void filter_gather_kernel(const float* __restrict__ feat, int u, const int32_t* __restrict__ src,
+                                     const int32_t* __restrict__ dst, const int32_t* __restrict__ m_dev, int64_t m_off, int64_t m_cap,
+                                     bf16* __restrict__ out) {
+  const int64_t M = rows_of(m_dev, m_off, m_cap);
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int64_t row = i >> 3;
+  if (row >= m_cap) return;
+  const int c0 = (int)(i & 7) * 8;
+  float v[8];
+#pragma unroll
+  for (int j = 0; j < 8; ++j) v[j] = 0.f;
+  if (row < M) {
+    const int64_t s = src[m_off + row], d = dst[m_off + row];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+      const int c = c0 + j;
+      if (c < u) v[j] = feat[s * u + c];
+      else if (c < 2 * u) v[j] = feat[d * u + (c - u)];
+    }
+  }
+  *reinterpret_cast<uint4*>(out + row * 64 + c0) =
+      make_uint4(tc::pack_bf16(v[0], v[1]), tc::pack_bf16(v[2], v[3]), tc::pack_bf16(v[4], v[5]), tc::pack_bf16(v[6], v[7]));
+}
+
+__global__ void filter_finish_kernel(const float* __restrict__ partial, int n_tiles, float b_last, const int32_t* __restrict__ m_dev,
+                                     int64_t m_off, int64_t m_cap, float* __restrict__ score) {
+  const int64_t M = rows_of(m_dev, m_off, m_cap);
+  const int64_t row = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (row >= M) return;
+  float s = b_last;
+  for (int t = 0; t < n_tiles; ++t) s += partial[row * n_tiles + t];
+  score[m_off + row] = 1.f / (1.f + __expf(-s));
+}
+
+// First GNN encoder layers (K = 3 node features or K = 4 edge features): one warp per row,
+// out[m] = bf16(ReLU(LayerNorm(W x + b))).  EDGE: x = edge_features(src[m], dst[m]).
+template <bool EDGE>
+__global__ void __launch_bounds__(256)
+encoder_first_layer_kernel(const float* __restrict__ hits, const int32_t* __restrict__ src, const int32_t* __restrict__ dst,
+                           const float* __restrict__ W, const float* __restrict__ b, int H, int use_ln,
+                           const int32_t* __restrict__ m_dev, int64_t m_cap, bf16* __restrict__ out) {
+  const int64_t M = rows_of(m_dev, 0, m_cap);
+  const int lane = threadIdx.x & 31;
+  const int64_t row = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  if (row >= M) return;
+  float x[4];
+  constexpr int K = EDGE ? 4 : 3;
+  if (EDGE) {
+    const float4 a = edge_features(hits, src[row], dst[row]);
+    x[0] = a.x; x[1] = a.y; x[2] = a.z; x[3] = a.w;
+  } else {
+    x[0] = hits[row * 3]; x[1] = hits[row * 3 + 1]; x[2] = hits[row * 3 + 2]; x[3] = 0.f;
+  }
+  float v[4];  // H <= 128: columns lane, lane+32, ...
+  float s = 0.f;
+  const int per = H / 32;
+  for (int j = 0; j < per; ++j) {
+    const int c = lane + 32 * j;
+    float a = b[c];
+#pragma unroll
+    for (int k = 0; k < K; ++k) a = fmaf(W[c * K + k], x[k], a);
+    v[j] = a;
+    s += a;
+  }
+  float mean = 0.f, rstd = 1.f;
+  if (use_ln) {
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    mean = s / (float)H;
+    float q = 0.f;
+    for (int j = 0; j < per; ++j) { const float d = v[j] - mean; q += d * d; }
+    for (int o = 16; o > 0; o >>= 1) q += __shfl_xor_sync(0xffffffffu, q, o);
+    rstd = rsqrtf(q / (float)H + 1e-5f);
+  }
+  for (int j = 0; j < per; ++j) out[row * H + lane + 32 * j] = __float2bfloat16_rn(fmaxf((v[j] - mean) * rstd, 0.f));
+}
+
+}  // namespace
+
+// ---------------------------------------------------------------- S1
+trk_status embed_forward_bf16(trk_ctx* ctx, const float* hits, int64_t n, float* emb, cudaStream_t st) {
+  const auto& L = ctx->embed.layers;
+  const int nl = (int)L.size();
+  bf16* bufs[2] = {(bf16*)ctx->act0, (bf16*)ctx->act1};
+  const int w0 = L[0].out;
+  TRK_LAUNCH(ctx, embed_first_layer_kernel, (unsigned)ceil_div(n * (w0 / 8), 256), 256, 0, st, hits, L[0].w_f32, L[0].b_f32, bufs[0], n,
+             w0);
+  int cur = 0;
+  tc::Rows rows{nullptr, 0, n};
+  for (int l = 1; l < nl - 1; ++l) {
+    TRK_TRY(gemm_bias_act(ctx, bufs[cur], ctx->act_rows, L[l].in_pad, L[l], bufs[cur ^ 1], L[l].out_pad, 1, rows, st));
+    cur ^= 1;
+  }
+  const DevLinear& last = L[nl - 1];
+  tc::EpiBiasF32Narrow::Params ep{last.b_f32, emb, ctx->d_e, ctx->d_e};
+  return launch_gemm<16, tc::EpiBiasF32Narrow>(ctx, bufs[cur], ctx->act_rows, last.in_pad, last.in_pad, last.w_bf16, 16, rows, ep, st);
+}
+
+// ---------------------------------------------------------------- S3
+trk_status filter_forward_bf16(trk_ctx* ctx, const float* feat, const int32_t* src, const int32_t* dst,
+                               const int32_t* n_edges_dev, int64_t n_edges_cap, float* score, cudaStream_t st) {
+  const auto& L = ctx->filter.layers;
+  const int nl = (int)L.size();
+  const int u = ctx->filter_u;
+  bf16* bufs[2] = {(bf16*)ctx->act0, (bf16*)ctx->act1};
+  bf16* gin = (bf16*)ctx->act_in;
+  for (int64_t off = 0; off < n_edges_cap; off += kFilterChunkRows) {
+    const int64_t cap = std::min<int64_t>(kFilterChunkRows, n_edges_cap - off);
+    tc::Rows rows{n_edges_dev, off, cap};
+    TRK_LAUNCH(ctx, filter_gather_kernel, (unsigned)ceil_div(cap * 8, 256), 256, 0, st, feat, u, src, dst, n_edges_dev, off, cap, gin);
+    const bf16* in = gin;
+    int64_t in_rows = kFilterChunkRows;
+    int cur = 0;
+    int n_tiles = 1;
+    for (int l = 0; l < nl - 1; ++l) {
+      // layer 0 reads the gathered rows (K padded to 64) against the K-padded copy of W1
+      DevLinear Ll = L[l];
+      if (l == 0) { Ll.w_bf16 = ctx->filter_w1_pad; Ll.in_pad = 64; }
+      const int64_t lda = l == 0 ? 64 : Ll.in_pad;
+      if (l == nl - 2) {
+        TRK_TRY(gemm_relu_dot(ctx, in, in_rows, lda, Ll, L[nl - 1].w_f32, ctx->partial, &n_tiles, rows, st));
+      } else {
+        TRK_TRY(gemm_bias_act(ctx, in, in_rows, lda, Ll, bufs[cur], Ll.out_pad, 1, rows, st));
+        in = bufs[cur];
+        in_rows = ctx->act_rows;
+        cur ^= 1;
+      }
+    }
+    TRK_LAUNCH(ctx, filter_finish_kernel, (unsigned)ceil_div(cap, 256), 256, 0, st, ctx->partial, n_tiles, ctx->filter_b_last,
+               n_edges_dev, off, cap, score);
+  }
+  return TRK_OK;
+}
+
+// ---------------------------------------------------------------- S4
+trk_status gnn_forward_bf16(trk_ctx* ctx, const float* hits, int64_t n, const int32_t* src, const int32_t* dst,
+                            const int32_t* n_edges_dev, int64_t n_edges_cap, float* score, cudaStream_t st) {
+  const int H = ctx->H;
+  const int ln = ctx->cfg.gnn_layernorm;
+  bf16* X = (bf16*)ctx->X;      // [n][3H]: h | m_in | m_out
+  bf16* E = (bf16*)ctx->E;      // [E][H]
+  bf16* T1 = (bf16*)ctx->T1;    // [max(n,E)][H]
+  float* PAB = ctx->PAB;        // [n][2H]
+  const int64_t x_rows = ctx->cfg.max_hits, e_rows = ctx->cfg.max_kept_edges, t_rows = std::max(x_rows, e_rows);
+  tc::Rows nrows{nullptr, 0, n};
+  tc::Rows erows{n_edges_dev, 0, n_edges_cap};
+  TRK_TRY(build_gnn_csr(ctx, src, dst, n_edges_dev, n_edges_cap, n, st));
+
+  // node encoder: 3 -> H (SIMT) -> H (GEMM, LNR) -> X[:, 0:H]
+  TRK_LAUNCH(ctx, encoder_first_layer_kernel<false>, (unsigned)ceil_div(n * 32, 256), 256, 0, st, hits, nullptr, nullptr,
+             ctx->node_enc.layers[0].w_f32, ctx->node_enc.layers[0].b_f32, H, ln, nullptr, n, T1);
+  {
+    tc::EpiRowLn::Params ep{ctx->node_enc.layers[1].b_f32, nullptr, nullptr, nullptr, ln, nullptr, 0, X, 3 * H, nullptr, 0.f, nullptr};
+    TRK_TRY(gemm_row_ln(ctx, T1, t_rows, H, H, ctx->node_enc.layers[1].w_bf16, ep, nrows, st));
+  }
+  if (n_edges_cap > 0) {
+    // edge encoder: 4 -> H (SIMT on the fly features) -> H (GEMM, LNR) -> E
+    TRK_LAUNCH(ctx, encoder_first_layer_kernel<true>, (unsigned)ceil_div(n_edges_cap * 32, 256), 256, 0, st, hits, src, dst,
+               ctx->edge_enc.layers[0].w_f32, ctx->edge_enc.layers[0].b_f32, H, ln, n_edges_dev, n_edges_cap, T1);
+    tc::EpiRowLn::Params ep{ctx->edge_enc.layers[1].b_f32, nullptr, nullptr, nullptr, ln, nullptr, 0, E, H, nullptr, 0.f, nullptr};
+    TRK_TRY(gemm_row_ln(ctx, T1, t_rows, H, H, ctx->edge_enc.layers[1].w_bf16, ep, erows, st));
+  }
+  for (int t = 0; t < ctx->cfg.gnn_iters; ++t) {
+    if (n_edges_cap > 0) {
+      // PA|PB = h [Wa ; Wb]^T per node, then e <- e + LNR(W2 LNR(Wc e + PA[src] + PB[dst] + b1) + b2)
+      TRK_TRY(gemm_store_f32(ctx, X, x_rows, 3 * H, H, ctx->edge_net_wab, 2 * H, PAB, nrows, st));
+      tc::EpiRowLn::Params e1{ctx->edge_net.layers[0].b_f32, PAB, src, dst, ln, nullptr, 0, T1, H, nullptr, 0.f, nullptr};
+      TRK_TRY(gemm_row_ln(ctx, E, e_rows, H, H, ctx->edge_net_wc, e1, erows, st));
+      tc::EpiRowLn::Params e2{ctx->edge_net.layers[1].b_f32, nullptr, nullptr, nullptr, ln, E, H, E, H, nullptr, 0.f, nullptr};
+      TRK_TRY(gemm_row_ln(ctx, T1, t_rows, H, H, ctx->edge_net.layers[1].w_bf16, e2, erows, st));
+    }
+    TRK_TRY(segment_sums(ctx, E, true, n, X, st));
+    // h <- h + LNR(W2 LNR(W1 [h ; m_in ; m_out] + b1) + b2): X is the concatenation already
+    tc::EpiRowLn::Params n1{ctx->node_net.layers[0].b_f32, nullptr, nullptr, nullptr, ln, nullptr, 0, T1, H, nullptr, 0.f, nullptr};
+    TRK_TRY(gemm_row_ln(ctx, X, x_rows, 3 * H, 3 * H, ctx->node_net.layers[0].w_bf16, n1, nrows, st));
+    tc::EpiRowLn::Params n2{ctx->node_net.layers[1].b_f32, nullptr, nullptr, nullptr, ln, X, 3 * H, X, 3 * H, nullptr, 0.f, nullptr};
+    TRK_TRY(gemm_row_ln(ctx, T1, t_rows, H, H, ctx->node_net.layers[1].w_bf16, n2, nrows, st));
+  }
+  if (n_edges_cap > 0) {
+    TRK_TRY(gemm_store_f32(ctx, X, x_rows, 3 * H, H, ctx->edge_dec_wab, 2 * H, PAB, nrows, st));
+    tc::EpiRowLn::Params d1{ctx->edge_dec.layers[0].b_f32, PAB, src, dst, ln, nullptr, 0, nullptr, 0,
+                            ctx->edge_dec.layers[1].w_f32, ctx->edge_dec_b_last, score};
+    TRK_TRY(gemm_row_ln(ctx, E, e_rows, H, H, ctx->edge_dec_wc, d1, erows, st));
+  }
+  return TRK_OK;
+}
+
+// ---------------------------------------------------------------- test hook
+trk_status gemm_bf16_hook(trk_ctx* ctx, const void* a, const void* w, const float* bias, void* out, int64_t m, int n, int k, int relu,
+                          cudaStream_t st) {
+  DevLinear L;
+  L.in = L.in_pad = k;
+  L.out = L.out_pad = n;
+  L.w_bf16 = (bf16*)w;
+  L.b_f32 = const_cast<float*>(bias);
+  return gemm_bias_act(ctx, (const bf16*)a, m, k, L, (bf16*)out, n, relu, tc::Rows{nullptr, 0, m}, st);
+}
+
+}  // namespace trk
