@@ -134,6 +134,13 @@ int64_t trk_workspace_bytes(const trk_ctx* ctx);
 /* Number of kernels of this library launched by the most recent trk_infer on ctx (host-side count). */
 int64_t trk_last_launch_count(const trk_ctx* ctx);
 
+/* Per-stage timing of trk_infer with CUDA events recorded on the call's stream at the stage
+ * boundaries (the analogue of perf_analyzer's latency breakdown).
+ * trk_profile_enable(ctx, 1) makes the following trk_infer calls record 6 events; trk_profile_stage_ms
+ * waits for the last one and writes the HOST array ms[5] = {S1, S2, S3 (incl. compaction), S4, S5}. */
+trk_status trk_profile_enable(trk_ctx* ctx, int32_t on);
+trk_status trk_profile_stage_ms(trk_ctx* ctx, float* ms);
+
 /* Stage hooks: run ONE stage on caller-supplied DEVICE inputs (BASELINE.json north_star: "each
  * stage fed the oracle's own inputs for that stage").  Same kernels as trk_infer.  Unless noted
  * all pointers are DEVICE; sizes are HOST scalars and must respect the ctx capacities.            */

@@ -19,7 +19,7 @@ TRK_FILTER_RAW, TRK_FILTER_EMB = 0, 1
 EXPORTS = [
     "trk_create", "trk_infer", "trk_destroy", "trk_infer_host", "trk_status_string", "trk_last_error",
     "trk_workspace_bytes", "trk_last_launch_count", "trk_stage_embed", "trk_stage_frnn", "trk_stage_filter",
-    "trk_stage_compact", "trk_stage_gnn", "trk_stage_cc", "trk_gemm_bf16",
+    "trk_stage_compact", "trk_stage_gnn", "trk_stage_cc", "trk_gemm_bf16", "trk_profile_enable", "trk_profile_stage_ms",
 ]
 
 _f32p = C.POINTER(C.c_float)
@@ -88,6 +88,8 @@ def lib():
     L.trk_stage_gnn.argtypes = [vp, vp, i64, vp, vp, i64, vp, vp]
     L.trk_stage_cc.argtypes = [vp, i64, vp, vp, vp, i64, C.c_float, vp, vp]
     L.trk_gemm_bf16.argtypes = [vp, vp, vp, vp, i64, i32, i32, i32, vp]
+    L.trk_profile_enable.argtypes = [vp, i32]
+    L.trk_profile_stage_ms.argtypes = [vp, _f32p]
     for name in EXPORTS:
         if getattr(L, name).restype is C.c_int:
             getattr(L, name).restype = C.c_int
@@ -188,6 +190,15 @@ class Trk:
     @property
     def last_launch_count(self):
         return lib().trk_last_launch_count(self._h)
+
+    def profile(self, on=True):
+        self._check(lib().trk_profile_enable(self._h, int(on)))
+
+    def stage_ms(self):
+        """{S1..S5: ms} of the last profiled infer (waits for it to finish)."""
+        ms = (C.c_float * 5)()
+        self._check(lib().trk_profile_stage_ms(self._h, ms))
+        return dict(zip(("s1_embed", "s2_frnn", "s3_filter", "s4_gnn", "s5_cc"), [float(v) for v in ms]))
 
     # ---- the call
     def infer(self, hits, event_offsets, *, want_edges=False, want_cand=False, want_embedding=False, out=None, stream=None):

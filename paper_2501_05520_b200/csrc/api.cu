@@ -232,6 +232,8 @@ trk_status trk_destroy(trk_ctx* ctx) {
     cudaStreamDestroy(ctx->own_stream);
   }
   cudaDeviceSynchronize();
+  for (auto& e : ctx->prof_ev)
+    if (e) cudaEventDestroy(e);
   for (DevMlp* m : {&ctx->embed, &ctx->filter, &ctx->node_enc, &ctx->edge_enc, &ctx->edge_net, &ctx->node_net, &ctx->edge_dec}) free_mlp(*m);
   cudaFree(ctx->grid_proj);
   cudaFree(ctx->edge_net_wab);
@@ -395,20 +397,30 @@ trk_status trk_infer(trk_ctx* ctx, const trk_batch* batch, const trk_result* res
   const trk_config& f = ctx->cfg;
   ctx->launch_count = 0;
   TRK_LAUNCH(ctx, zero_counts_kernel, 1, 32, 0, st, ctx->counts);
+  const bool prof = ctx->profiling && n > 0;
+  ctx->prof_valid = false;
+#define TRK_MARK(i) do { if (prof) TRK_CUDA(ctx, cudaEventRecord(ctx->prof_ev[i], st)); } while (0)
   if (n > 0) {
     TRK_TRY(set_event_ids(ctx, batch->event_offsets, batch->n_events, n, st));
+    TRK_MARK(0);
     TRK_TRY(embed_dispatch(ctx, batch->hits, n, ctx->emb, st));
+    TRK_MARK(1);
     TRK_TRY(frnn_build(ctx, ctx->emb, batch->hits, n, batch->n_events, ctx->cand_src, ctx->cand_dst, nullptr, f.max_cand_edges,
                        &ctx->counts[0], &ctx->counts[3], st));
+    TRK_MARK(2);
     const float* feat = f.filter_input == TRK_FILTER_EMB ? ctx->emb : batch->hits;
     const int64_t cand_cap = std::min<int64_t>(f.max_cand_edges, n * f.frnn_k);
     TRK_TRY(filter_dispatch(ctx, feat, ctx->cand_src, ctx->cand_dst, &ctx->counts[0], cand_cap, ctx->cand_score, st));
     TRK_TRY(compact_edges(ctx, ctx->cand_src, ctx->cand_dst, ctx->cand_score, &ctx->counts[0], cand_cap, f.filter_cut, ctx->kept_src,
                           ctx->kept_dst, f.max_kept_edges, &ctx->counts[1], &ctx->counts[3], st));
     const int64_t kept_cap = std::min<int64_t>(f.max_kept_edges, cand_cap);
+    TRK_MARK(3);
     TRK_TRY(gnn_dispatch(ctx, batch->hits, n, ctx->kept_src, ctx->kept_dst, &ctx->counts[1], kept_cap, ctx->kept_score, st));
+    TRK_MARK(4);
     TRK_TRY(cc_labels(ctx, n, ctx->kept_src, ctx->kept_dst, ctx->kept_score, &ctx->counts[1], kept_cap, f.gnn_cut, res->labels,
                       &ctx->counts[2], st));
+    TRK_MARK(5);
+    ctx->prof_valid = prof;
     if (res->embedding) TRK_CUDA(ctx, cudaMemcpyAsync(res->embedding, ctx->emb, (size_t)n * ctx->d_e * 4, cudaMemcpyDeviceToDevice, st));
     const size_t ne = (size_t)std::min<int64_t>(res->edge_capacity, kept_cap), nc = (size_t)std::min<int64_t>(res->cand_capacity, cand_cap);
     if (res->edge_src) TRK_CUDA(ctx, cudaMemcpyAsync(res->edge_src, ctx->kept_src, ne * 4, cudaMemcpyDeviceToDevice, st));
@@ -441,6 +453,23 @@ trk_status trk_infer_host(trk_ctx* ctx, int32_t n_events, const int32_t* event_o
   if (n > 0) TRK_CUDA(ctx, cudaMemcpyAsync(labels_host, ctx->io_labels, (size_t)n * 4, cudaMemcpyDeviceToHost, st));
   if (counts_host) TRK_CUDA(ctx, cudaMemcpyAsync(counts_host, ctx->io_counts, 16, cudaMemcpyDeviceToHost, st));
   TRK_CUDA(ctx, cudaStreamSynchronize(st));
+  return TRK_OK;
+}
+
+trk_status trk_profile_enable(trk_ctx* ctx, int32_t on) {
+  if (!ctx) return TRK_ERR_INVALID_ARG;
+  if (on && !ctx->prof_ev[0])
+    for (auto& e : ctx->prof_ev) TRK_CUDA(ctx, cudaEventCreate(&e));
+  ctx->profiling = on != 0;
+  ctx->prof_valid = false;
+  return TRK_OK;
+}
+
+trk_status trk_profile_stage_ms(trk_ctx* ctx, float* ms) {
+  if (!ctx || !ms) return TRK_ERR_INVALID_ARG;
+  if (!ctx->prof_valid) return fail(ctx, TRK_ERR_INVALID_ARG, "no profiled trk_infer call to read");
+  TRK_CUDA(ctx, cudaEventSynchronize(ctx->prof_ev[5]));
+  for (int i = 0; i < 5; ++i) TRK_CUDA(ctx, cudaEventElapsedTime(&ms[i], ctx->prof_ev[i], ctx->prof_ev[i + 1]));
   return TRK_OK;
 }
 

@@ -59,6 +59,9 @@ struct trk_ctx {
   cudaStream_t own_stream = nullptr;
   std::string last_error;
   int64_t launch_count = 0;
+  bool profiling = false;
+  cudaEvent_t prof_ev[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+  bool prof_valid = false;
 
   trk::DevMlp embed, filter, node_enc, edge_enc, edge_net, node_net, edge_dec;
   float* grid_proj = nullptr;       // [d_e_pad][3] device
