@@ -2,6 +2,7 @@
 // pipeline of PAPER.md line 85 and the per-stage hooks.
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <mutex>
 
@@ -111,14 +112,19 @@ void carve(trk_ctx* c, Carver& k) {
   int maxw = 64;
   for (auto& L : c->embed.layers) maxw = std::max(maxw, L.out_pad);
   for (auto& L : c->filter.layers) maxw = std::max(maxw, L.out_pad);
-  c->act_rows = (int64_t)std::max<size_t>(N, (size_t)kFilterChunkRows);
+  {
+    int64_t chunk = kFilterChunkRows;
+    if (const char* e = std::getenv("TRK_FILTER_CHUNK_TILES")) chunk = std::max<int64_t>(1, std::atoll(e)) * 128;  // tuning knob
+    c->filter_chunk = std::min<int64_t>(chunk, ((int64_t)EC + 127) / 128 * 128);
+  }
+  c->act_rows = (int64_t)std::max<size_t>(N, (size_t)c->filter_chunk);
   char* p;
   k.take(&c->ev_of_hit, N);
   k.take(&c->emb, N * c->d_e);
   k.take(&p, (size_t)c->act_rows * maxw * es); c->act0 = p;
   k.take(&p, (size_t)c->act_rows * maxw * es); c->act1 = p;
-  k.take(&p, (size_t)kFilterChunkRows * (bf ? 64 * 2 : 2 * c->filter_u * 4)); c->act_in = p;
-  k.take(&c->partial, (size_t)kFilterChunkRows * 16);
+  k.take(&p, (size_t)c->filter_chunk * (bf ? 64 * 2 : 2 * c->filter_u * 4)); c->act_in = p;
+  k.take(&c->partial, (size_t)c->filter_chunk * 16);
   k.take(&c->proj, N * 3);
   k.take(&c->bbox, 8);
   k.take(&c->grid, 1);

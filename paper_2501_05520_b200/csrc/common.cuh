@@ -15,7 +15,7 @@ namespace trk {
 constexpr int kMaxEmbDim = 16;      // d_e is padded to a multiple of 4, at most 16
 constexpr int kMaxEvents = 1024;    // event offsets travel as a kernel parameter
 constexpr int64_t kMaxCells = 1 << 21;  // FRNN grid cells summed over the events of a call
-constexpr int kFilterChunkRows = 128 * 148;  // S3 rows per pass: one 128-row tile per SM and N-tile column
+constexpr int kFilterChunkRows = 128 * 148 * 16;  // S3 rows per pass (upper bound; ctx->filter_chunk is the per-context value)
 
 // One Linear layer resident on the device.
 struct DevLinear {
@@ -87,6 +87,7 @@ struct trk_ctx {
   void* act_in = nullptr;           // S3 gathered input rows
   float* partial = nullptr;         // [chunk][4] fused last-layer partial dots
   int64_t act_rows = 0;
+  int64_t filter_chunk = 0;         // S3 rows per pass: min(kFilterChunkRows, max_cand_edges rounded up to 128)
   // S2
   float* proj = nullptr;            // [max_hits][3]
   int32_t* bbox = nullptr;          // [6] ordered-int min/max

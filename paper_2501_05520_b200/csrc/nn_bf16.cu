@@ -246,12 +246,12 @@ trk_status filter_forward_bf16(trk_ctx* ctx, const float* feat, const int32_t* s
   const int u = ctx->filter_u;
   bf16* bufs[2] = {(bf16*)ctx->act0, (bf16*)ctx->act1};
   bf16* gin = (bf16*)ctx->act_in;
-  for (int64_t off = 0; off < n_edges_cap; off += kFilterChunkRows) {
-    const int64_t cap = std::min<int64_t>(kFilterChunkRows, n_edges_cap - off);
+  for (int64_t off = 0; off < n_edges_cap; off += ctx->filter_chunk) {
+    const int64_t cap = std::min<int64_t>(ctx->filter_chunk, n_edges_cap - off);
     tc::Rows rows{n_edges_dev, off, cap};
     TRK_LAUNCH(ctx, filter_gather_kernel, (unsigned)ceil_div(cap * 8, 256), 256, 0, st, feat, u, src, dst, n_edges_dev, off, cap, gin);
     const bf16* in = gin;
-    int64_t in_rows = kFilterChunkRows;
+    int64_t in_rows = ctx->filter_chunk;
     int cur = 0;
     int n_tiles = 1;
     for (int l = 0; l < nl - 1; ++l) {

@@ -197,8 +197,8 @@ trk_status filter_forward_fp32(trk_ctx* ctx, const float* feat, const int32_t* s
   const auto& L = ctx->filter.layers;
   const int u = ctx->filter_u;
   float* bufs[2] = {(float*)ctx->act0, (float*)ctx->act1};
-  for (int64_t off = 0; off < n_edges_cap; off += kFilterChunkRows) {
-    const int64_t cap = std::min<int64_t>(kFilterChunkRows, n_edges_cap - off);
+  for (int64_t off = 0; off < n_edges_cap; off += ctx->filter_chunk) {
+    const int64_t cap = std::min<int64_t>(ctx->filter_chunk, n_edges_cap - off);
     float* gin = (float*)ctx->act_in;
     TRK_LAUNCH(ctx, gather_pair_f32_kernel, (unsigned)ceil_div(cap * 2 * u, 256), 256, 0, st, feat, u, src, dst, n_edges_dev, off,
                cap, gin);
