@@ -77,6 +77,18 @@ __device__ __forceinline__ void tma_load_2d(void* smem_dst, const CUtensorMap* t
       : "memory");
 }
 
+// TMA store of a shared-memory box (bulk async group completion)
+__device__ __forceinline__ void tma_store_2d(const CUtensorMap* tmap, const void* smem_src, int c0, int c1) {
+  asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%2, %3}], [%1];" ::"l"(reinterpret_cast<uint64_t>(tmap)),
+               "r"(smem_u32(smem_src)), "r"(c0), "r"(c1)
+               : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory"); }
+__device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
 template <int NCOLS>
 __device__ __forceinline__ void tmem_alloc(uint32_t* smem_slot) {
   asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(smem_slot)), "n"(NCOLS) : "memory");
@@ -143,7 +155,17 @@ __host__ __device__ constexpr uint32_t make_idesc(int bn) {
 constexpr int tmem_cols_for(int bn) { return 2 * bn <= 32 ? 32 : (2 * bn <= 64 ? 64 : (2 * bn <= 128 ? 128 : (2 * bn <= 256 ? 256 : 512))); }
 constexpr int stage_bytes(int bn) { return (BM + bn) * BK * 2; }
 constexpr int num_stages(int bn) { return (196 * 1024) / stage_bytes(bn) > 8 ? 8 : (196 * 1024) / stage_bytes(bn); }
-constexpr int smem_bytes(int bn) { return num_stages(bn) * stage_bytes(bn) + 1024 /*alignment*/ + 256 /*barriers*/; }
+constexpr int kStoreStage = 2 * 32 * 128;   // per epilogue warp: two 32-row x 128-byte boxes (TMA-store staging)
+constexpr int smem_bytes(int bn, bool tma_store = false) {
+  return num_stages(bn) * stage_bytes(bn) + (tma_store ? kEpiWarps * kStoreStage : 0) + 1024 /*alignment*/ + 256 /*barriers*/;
+}
+
+// What an epilogue may use besides its own parameters: a per-warp staging area and the output tensor map.
+struct EpiShared {
+  uint8_t* stage;           // kStoreStage bytes, 1024-byte aligned (only when Epi::kTmaStore)
+  const CUtensorMap* tmC;
+  uint32_t chunk;           // running count of staged boxes of this warp (selects the half of `stage`)
+};
 
 // ------------------------------------------------------------------ the kernel
 // Epi::run(params, tmem_tile_addr (lane and column base of this warp's quadrant), row0 (first row of the
@@ -151,15 +173,16 @@ constexpr int smem_bytes(int bn) { return num_stages(bn) * stage_bytes(bn) + 102
 //          `release` exactly once after its last TMEM read.
 template <int BN, class Epi>
 __global__ void __launch_bounds__(kThreads, 1)
-gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, Rows rows, int n_tiles, int k_blocks,
-               typename Epi::Params ep) {
+gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, const __grid_constant__ CUtensorMap tmC,
+               Rows rows, int n_tiles, int k_blocks, typename Epi::Params ep) {
   constexpr int STAGES = num_stages(BN);
   constexpr int A_BYTES = BM * BK * 2;
   constexpr int STAGE = stage_bytes(BN);
   constexpr int TMEM_COLS = tmem_cols_for(BN);
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
-  uint64_t* full_bar = reinterpret_cast<uint64_t*>(smem + STAGES * STAGE);
+  uint8_t* store_stage = smem + STAGES * STAGE;
+  uint64_t* full_bar = reinterpret_cast<uint64_t*>(store_stage + (Epi::kTmaStore ? kEpiWarps * kStoreStage : 0));
   uint64_t* empty_bar = full_bar + STAGES;
   uint64_t* tfull_bar = empty_bar + STAGES;
   uint64_t* tempty_bar = tfull_bar + 2;
@@ -235,6 +258,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     const int quad = warp & 3;   // TMEM lane quadrant this warp may access
     int as = 0;
     uint32_t aphase = 0;
+    EpiShared es{store_stage + (warp - 2) * kStoreStage, &tmC, 0u};
     for (int64_t tile = blockIdx.x; tile < total; tile += gridDim.x) {
       const int m_blk = (int)(tile / n_tiles), n_blk = (int)(tile % n_tiles);
       mbar_wait(&tfull_bar[as], aphase);
@@ -246,9 +270,10 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
         __syncwarp();
         if (lane == 0) mbar_arrive(rel);
       };
-      Epi::template run<BN>(ep, taddr, (int64_t)m_blk * BM + quad * 32 + lane, n_blk * BN, n_blk, M, release);
+      Epi::template run<BN>(ep, taddr, (int64_t)m_blk * BM + quad * 32 + lane, n_blk * BN, n_blk, M, release, es);
       if (++as == 2) { as = 0; aphase ^= 1; }
     }
+    if (Epi::kTmaStore && lane == 0) bulk_wait_all();   // staged boxes must be read before the CTA's shared memory goes away
   }
   tc_fence_before();
   __syncthreads();
@@ -265,43 +290,59 @@ __device__ __forceinline__ uint32_t pack_bf16(float a, float b) {
 }
 __device__ __forceinline__ float fast_sigmoid(float x) { return 1.f / (1.f + __expf(-x)); }
 
-// out[m][n] = act(acc + bias[n]) as bf16.
+// out[m][n] = act(acc + bias[n]) as bf16.  Each warp stages 32 rows x 64 columns (one 128-byte swizzled
+// box) in shared memory and hands it to the TMA (cp.async.bulk.tensor store): full 128-byte lines leave the
+// SM instead of 16-byte pieces of 32 different rows per store instruction.  Rows beyond M inside the last
+// tile are written too (finite values computed from zero padded inputs); rows beyond the tensor are clipped.
 struct EpiBiasActBf16 {
+  static constexpr bool kTmaStore = true;
   struct Params {
     const float* bias;
-    __nv_bfloat16* out;
-    int ldo;
     int relu;
   };
   template <int BN, class F>
-  __device__ static void run(const Params& p, uint32_t taddr, int64_t row, int col0, int n_blk, int64_t M, F release) {
+  __device__ static void run(const Params& p, uint32_t taddr, int64_t row, int col0, int n_blk, int64_t M, F release, EpiShared& es) {
+    const int lane = threadIdx.x & 31;
 #pragma unroll 1
-    for (int c = 0; c < BN; c += 32) {
-      uint32_t r[32];
-      tmem_ld32(taddr + c, r);
-      tmem_ld_wait();
-      if (c + 32 >= BN) release();
-      if (row < M) {
-        uint4* dst = reinterpret_cast<uint4*>(p.out + row * p.ldo + col0 + c);
-        const float4* b4 = reinterpret_cast<const float4*>(p.bias + col0 + c);
-#pragma unroll
-        for (int q = 0; q < 4; ++q) {
-          float v[8];
-#pragma unroll
-          for (int h = 0; h < 2; ++h) {
-            const float4 b = __ldg(b4 + q * 2 + h);
-            v[h * 4 + 0] = __uint_as_float(r[q * 8 + h * 4 + 0]) + b.x;
-            v[h * 4 + 1] = __uint_as_float(r[q * 8 + h * 4 + 1]) + b.y;
-            v[h * 4 + 2] = __uint_as_float(r[q * 8 + h * 4 + 2]) + b.z;
-            v[h * 4 + 3] = __uint_as_float(r[q * 8 + h * 4 + 3]) + b.w;
-          }
-          if (p.relu) {
-#pragma unroll
-            for (int i = 0; i < 8; ++i) v[i] = fmaxf(v[i], 0.f);
-          }
-          dst[q] = make_uint4(pack_bf16(v[0], v[1]), pack_bf16(v[2], v[3]), pack_bf16(v[4], v[5]), pack_bf16(v[6], v[7]));
-        }
+    for (int c = 0; c < BN; c += 64) {
+      uint32_t ra[32], rb[32];
+      tmem_ld32(taddr + c, ra);
+      tmem_ld32(taddr + c + 32, rb);
+      uint8_t* buf = es.stage + (es.chunk & 1u) * (kStoreStage / 2);
+      if (es.chunk >= 2) {          // the box staged two chunks ago must have left shared memory
+        if (lane == 0) bulk_wait_read<1>();
+        __syncwarp();
       }
+      tmem_ld_wait();
+      if (c + 64 >= BN) release();
+      const float4* b4 = reinterpret_cast<const float4*>(p.bias + col0 + c);
+#pragma unroll
+      for (int q = 0; q < 8; ++q) {
+        float v[8];
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+          const float4 b = __ldg(b4 + q * 2 + h);
+          const uint32_t* r = (q < 4 ? ra : rb) + (q & 3) * 8 + h * 4;
+          v[h * 4 + 0] = __uint_as_float(r[0]) + b.x;
+          v[h * 4 + 1] = __uint_as_float(r[1]) + b.y;
+          v[h * 4 + 2] = __uint_as_float(r[2]) + b.z;
+          v[h * 4 + 3] = __uint_as_float(r[3]) + b.w;
+        }
+        if (p.relu) {
+#pragma unroll
+          for (int i = 0; i < 8; ++i) v[i] = fmaxf(v[i], 0.f);
+        }
+        // 128-byte swizzle: 16-byte chunk q of row `lane` lives at chunk position q ^ (lane & 7)
+        *reinterpret_cast<uint4*>(buf + lane * 128 + ((q ^ (lane & 7)) << 4)) =
+            make_uint4(pack_bf16(v[0], v[1]), pack_bf16(v[2], v[3]), pack_bf16(v[4], v[5]), pack_bf16(v[6], v[7]));
+      }
+      fence_proxy_async();
+      __syncwarp();
+      if (lane == 0) {
+        tma_store_2d(es.tmC, buf, col0 + c, (int)(row - lane));
+        bulk_commit();
+      }
+      ++es.chunk;
     }
   }
 };
@@ -310,6 +351,7 @@ struct EpiBiasActBf16 {
 // The last Linear(N -> 1) of S3 folded into the epilogue of the layer before it; a tiny kernel adds
 // the n_tiles partials in fixed order, so the result is deterministic.
 struct EpiReluDot {
+  static constexpr bool kTmaStore = false;
   struct Params {
     const float* bias;
     const float* w_last;
@@ -317,7 +359,7 @@ struct EpiReluDot {
     int n_tiles;
   };
   template <int BN, class F>
-  __device__ static void run(const Params& p, uint32_t taddr, int64_t row, int col0, int n_blk, int64_t M, F release) {
+  __device__ static void run(const Params& p, uint32_t taddr, int64_t row, int col0, int n_blk, int64_t M, F release, EpiShared&) {
     float s = 0.f;
 #pragma unroll 1
     for (int c = 0; c < BN; c += 32) {
@@ -342,6 +384,7 @@ struct EpiReluDot {
 
 // out[m][0..n_valid) = acc + bias as fp32 (narrow output layer, BN = 16).
 struct EpiBiasF32Narrow {
+  static constexpr bool kTmaStore = false;
   struct Params {
     const float* bias;
     float* out;
@@ -349,7 +392,7 @@ struct EpiBiasF32Narrow {
     int n_valid;
   };
   template <int BN, class F>
-  __device__ static void run(const Params& p, uint32_t taddr, int64_t row, int col0, int n_blk, int64_t M, F release) {
+  __device__ static void run(const Params& p, uint32_t taddr, int64_t row, int col0, int n_blk, int64_t M, F release, EpiShared&) {
     static_assert(BN == 16, "narrow epilogue is for BN = 16");
     uint32_t r[16];
     tmem_ld16(taddr, r);
@@ -365,12 +408,13 @@ struct EpiBiasF32Narrow {
 
 // out[m][n] = acc as fp32 (the per-node halves of a split first layer, no bias).
 struct EpiStoreF32 {
+  static constexpr bool kTmaStore = false;
   struct Params {
     float* out;
     int ldo;
   };
   template <int BN, class F>
-  __device__ static void run(const Params& p, uint32_t taddr, int64_t row, int col0, int n_blk, int64_t M, F release) {
+  __device__ static void run(const Params& p, uint32_t taddr, int64_t row, int col0, int n_blk, int64_t M, F release, EpiShared&) {
 #pragma unroll 1
     for (int c = 0; c < BN; c += 32) {
       uint32_t r[32];
@@ -391,6 +435,7 @@ struct EpiStoreF32 {
 //   score mode:  score[m] = sigmoid(dot(v, w_out) + b_out)
 //   else:        out[m] = (res ? res[m] : 0) + v   as bf16   (out may alias res)
 struct EpiRowLn {
+  static constexpr bool kTmaStore = false;
   struct Params {
     const float* bias;
     const float* pab;        // fp32 [nodes][2*BN]: columns [0,BN) belong to src, [BN,2BN) to dst; may be null
@@ -406,7 +451,7 @@ struct EpiRowLn {
     float* score;
   };
   template <int BN, class F>
-  __device__ static void run(const Params& p, uint32_t taddr, int64_t row, int col0, int n_blk, int64_t M, F release) {
+  __device__ static void run(const Params& p, uint32_t taddr, int64_t row, int col0, int n_blk, int64_t M, F release, EpiShared&) {
     float v[BN];
 #pragma unroll
     for (int c = 0; c < BN; c += 32) {

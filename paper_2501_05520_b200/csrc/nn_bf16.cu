@@ -55,37 +55,52 @@ trk_status make_tmap(trk_ctx* ctx, CUtensorMap* m, const void* base, int64_t row
   return TRK_OK;
 }
 
+// Output of a TMA-store epilogue: bf16 [rows][n] with row stride ld (elements).
+struct OutBf16 {
+  bf16* ptr = nullptr;
+  int64_t rows = 0;
+  int64_t ld = 0;
+};
+
 // A [a_rows][K] bf16 (row stride lda), W [n_pad][K] bf16 K-major; rows of the product resolved on the device.
 template <int BN, class Epi>
 trk_status launch_gemm(trk_ctx* ctx, const bf16* A, int64_t a_rows, int64_t lda, int K, const bf16* W, int n_pad, tc::Rows rows,
-                       const typename Epi::Params& ep, cudaStream_t st) {
+                       const typename Epi::Params& ep, cudaStream_t st, OutBf16 out = OutBf16()) {
   if (rows.m_cap <= 0) return TRK_OK;
   if (K % tc::BK != 0 || n_pad % BN != 0) return fail(ctx, TRK_ERR_SHAPE, "gemm: K must be a multiple of 64 and N of the tile");
   static bool attr_set = false;
   auto kern = tc::gemm_tc_kernel<BN, Epi>;
   if (!attr_set) {
-    TRK_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::smem_bytes(BN)));
+    TRK_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::smem_bytes(BN, Epi::kTmaStore)));
     attr_set = true;
   }
-  CUtensorMap ta, tb;
+  CUtensorMap ta, tb, tc_out;
   TRK_TRY(make_tmap(ctx, &ta, A, a_rows, K, lda, tc::BM));
   TRK_TRY(make_tmap(ctx, &tb, W, n_pad, K, K, BN));
+  if (Epi::kTmaStore) {
+    if (!out.ptr || out.ld % 8 != 0) return fail(ctx, TRK_ERR_SHAPE, "gemm: the bf16 output needs a row stride that is a multiple of 8");
+    TRK_TRY(make_tmap(ctx, &tc_out, out.ptr, out.rows, n_pad, out.ld, 32));
+  } else {
+    tc_out = ta;
+  }
   const int n_tiles = n_pad / BN;
   const int64_t tiles = ceil_div(rows.m_cap, tc::BM) * n_tiles;
   const unsigned grid = (unsigned)std::min<int64_t>(tiles, ctx->sm_count);
-  TRK_LAUNCH(ctx, kern, grid, tc::kThreads, tc::smem_bytes(BN), st, ta, tb, rows, n_tiles, K / tc::BK, ep);
+  TRK_LAUNCH(ctx, kern, grid, tc::kThreads, tc::smem_bytes(BN, Epi::kTmaStore), st, ta, tb, tc_out, rows, n_tiles, K / tc::BK, ep);
   return TRK_OK;
 }
 
 int pick_bn(int n_pad) { return n_pad % 256 == 0 ? 256 : (n_pad % 128 == 0 ? 128 : 64); }
 
-trk_status gemm_bias_act(trk_ctx* ctx, const bf16* A, int64_t a_rows, int64_t lda, const DevLinear& L, bf16* out, int ldo, int relu,
-                         tc::Rows rows, cudaStream_t st) {
-  tc::EpiBiasActBf16::Params ep{L.b_f32, out, ldo, relu};
+// out: bf16 [out_rows][ldo]; every 128-row tile that holds a valid row is written in full (rows beyond out_rows are clipped).
+trk_status gemm_bias_act(trk_ctx* ctx, const bf16* A, int64_t a_rows, int64_t lda, const DevLinear& L, bf16* out, int64_t out_rows,
+                         int ldo, int relu, tc::Rows rows, cudaStream_t st) {
+  tc::EpiBiasActBf16::Params ep{L.b_f32, relu};
+  const OutBf16 o{out, out_rows, ldo};
   switch (pick_bn(L.out_pad)) {
-    case 256: return launch_gemm<256, tc::EpiBiasActBf16>(ctx, A, a_rows, lda, L.in_pad, L.w_bf16, L.out_pad, rows, ep, st);
-    case 128: return launch_gemm<128, tc::EpiBiasActBf16>(ctx, A, a_rows, lda, L.in_pad, L.w_bf16, L.out_pad, rows, ep, st);
-    default: return launch_gemm<64, tc::EpiBiasActBf16>(ctx, A, a_rows, lda, L.in_pad, L.w_bf16, L.out_pad, rows, ep, st);
+    case 256: return launch_gemm<256, tc::EpiBiasActBf16>(ctx, A, a_rows, lda, L.in_pad, L.w_bf16, L.out_pad, rows, ep, st, o);
+    case 128: return launch_gemm<128, tc::EpiBiasActBf16>(ctx, A, a_rows, lda, L.in_pad, L.w_bf16, L.out_pad, rows, ep, st, o);
+    default: return launch_gemm<64, tc::EpiBiasActBf16>(ctx, A, a_rows, lda, L.in_pad, L.w_bf16, L.out_pad, rows, ep, st, o);
   }
 }
 
@@ -230,7 +245,7 @@ trk_status embed_forward_bf16(trk_ctx* ctx, const float* hits, int64_t n, float*
   int cur = 0;
   tc::Rows rows{nullptr, 0, n};
   for (int l = 1; l < nl - 1; ++l) {
-    TRK_TRY(gemm_bias_act(ctx, bufs[cur], ctx->act_rows, L[l].in_pad, L[l], bufs[cur ^ 1], L[l].out_pad, 1, rows, st));
+    TRK_TRY(gemm_bias_act(ctx, bufs[cur], ctx->act_rows, L[l].in_pad, L[l], bufs[cur ^ 1], ctx->act_rows, L[l].out_pad, 1, rows, st));
     cur ^= 1;
   }
   const DevLinear& last = L[nl - 1];
@@ -262,7 +277,7 @@ trk_status filter_forward_bf16(trk_ctx* ctx, const float* feat, const int32_t* s
       if (l == nl - 2) {
         TRK_TRY(gemm_relu_dot(ctx, in, in_rows, lda, Ll, L[nl - 1].w_f32, ctx->partial, &n_tiles, rows, st));
       } else {
-        TRK_TRY(gemm_bias_act(ctx, in, in_rows, lda, Ll, bufs[cur], Ll.out_pad, 1, rows, st));
+        TRK_TRY(gemm_bias_act(ctx, in, in_rows, lda, Ll, bufs[cur], ctx->act_rows, Ll.out_pad, 1, rows, st));
         in = bufs[cur];
         in_rows = ctx->act_rows;
         cur ^= 1;
@@ -335,7 +350,7 @@ trk_status gemm_bf16_hook(trk_ctx* ctx, const void* a, const void* w, const floa
   L.out = L.out_pad = n;
   L.w_bf16 = (bf16*)w;
   L.b_f32 = const_cast<float*>(bias);
-  return gemm_bias_act(ctx, (const bf16*)a, m, k, L, (bf16*)out, n, relu, tc::Rows{nullptr, 0, m}, st);
+  return gemm_bias_act(ctx, (const bf16*)a, m, k, L, (bf16*)out, m, n, relu, tc::Rows{nullptr, 0, m}, st);
 }
 
 }  // namespace trk
