@@ -173,6 +173,12 @@ trk_status trk_stage_cc(trk_ctx* ctx, int64_t n, const int32_t* src, const int32
 trk_status trk_gemm_bf16(const void* a, const void* w, const float* bias, void* out, int64_t m, int32_t n,
                          int32_t k, int32_t relu, void* cuda_stream);
 
+/* Tuning / test knob, process wide: selects between kernel variants that compute the same result.
+ *   "gemm_pair"  1 (default): dense layers with >= 128 output columns run on CTA pairs (tcgen05.mma.cta_group::2,
+ *                256-row tiles); 0: single-CTA 128-row tiles.
+ * Returns TRK_ERR_INVALID_ARG for an unknown key.  Not thread safe against running trk_* calls. */
+trk_status trk_debug_set(const char* key, int64_t value);
+
 #ifdef __cplusplus
 }
 #endif

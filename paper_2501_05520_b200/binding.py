@@ -20,6 +20,7 @@ EXPORTS = [
     "trk_create", "trk_infer", "trk_destroy", "trk_infer_host", "trk_status_string", "trk_last_error",
     "trk_workspace_bytes", "trk_last_launch_count", "trk_stage_embed", "trk_stage_frnn", "trk_stage_filter",
     "trk_stage_compact", "trk_stage_gnn", "trk_stage_cc", "trk_gemm_bf16", "trk_profile_enable", "trk_profile_stage_ms",
+    "trk_debug_set",
 ]
 
 _f32p = C.POINTER(C.c_float)
@@ -89,6 +90,7 @@ def lib():
     L.trk_stage_cc.argtypes = [vp, i64, vp, vp, vp, i64, C.c_float, vp, vp]
     L.trk_gemm_bf16.argtypes = [vp, vp, vp, vp, i64, i32, i32, i32, vp]
     L.trk_profile_enable.argtypes = [vp, i32]
+    L.trk_debug_set.argtypes = [C.c_char_p, i64]
     L.trk_profile_stage_ms.argtypes = [vp, _f32p]
     for name in EXPORTS:
         if getattr(L, name).restype is C.c_int:
@@ -300,6 +302,13 @@ class Trk:
         self._check(lib().trk_stage_cc(self._h, n, _ptr(src), _ptr(dst), _ptr(score), src.numel(), float(cut), _ptr(labels),
                                        _stream_ptr(stream)))
         return labels
+
+
+def debug_set(key: str, value: int) -> None:
+    """Process-wide kernel-variant knob (include/trk.h trk_debug_set)."""
+    st = lib().trk_debug_set(key.encode(), int(value))
+    if st != 0:
+        raise TrkError(st, lib().trk_last_error(None).decode())
 
 
 def gemm_bf16(a, w, bias, relu=True, stream=None):

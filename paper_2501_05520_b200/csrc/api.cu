@@ -24,6 +24,9 @@ trk_status fail(trk_ctx* ctx, trk_status s, const std::string& msg) {
   return s;
 }
 
+static int64_t g_knobs[kKnobCount] = {1, 0, 0, 0, 0, 0, 0, 0};
+int64_t debug_knob(int which) { return g_knobs[which]; }
+
 trk_status gemm_bf16_hook(trk_ctx* ctx, const void* a, const void* w, const float* bias, void* out, int64_t m, int n, int k, int relu,
                           cudaStream_t st);
 
@@ -547,6 +550,12 @@ trk_status trk_stage_cc(trk_ctx* ctx, int64_t n, const int32_t* src, const int32
     return fail(ctx, TRK_ERR_INVALID_ARG, "stage_cc: bad arguments");
   if (n > ctx->cfg.max_hits) return fail(ctx, TRK_ERR_CAPACITY, "stage_cc: n exceeds max_hits");
   return cc_labels(ctx, n, src, dst, score, nullptr, n_edges, cut, labels, nullptr, (cudaStream_t)cuda_stream);
+}
+
+trk_status trk_debug_set(const char* key, int64_t value) {
+  if (!key) return TRK_ERR_INVALID_ARG;
+  if (std::strcmp(key, "gemm_pair") == 0) { g_knobs[kKnobGemmPair] = value; return TRK_OK; }
+  return fail(nullptr, TRK_ERR_INVALID_ARG, std::string("trk_debug_set: unknown key ") + key);
 }
 
 trk_status trk_gemm_bf16(const void* a, const void* w, const float* bias, void* out, int64_t m, int32_t n, int32_t k, int32_t relu,

@@ -158,6 +158,10 @@ trk_status fail(trk_ctx* ctx, trk_status s, const std::string& msg);
 
 inline int64_t ceil_div(int64_t a, int64_t b) { return (a + b - 1) / b; }
 
+// ---- tuning / test knobs (trk_debug_set) ----
+enum { kKnobGemmPair = 0, kKnobCount = 8 };
+int64_t debug_knob(int which);
+
 // ---- util_kernels.cu ----
 trk_status exclusive_scan_i32(trk_ctx* ctx, const int32_t* in, int32_t* out, int64_t n, int32_t* tmp, cudaStream_t st);
 trk_status fill_i32(trk_ctx* ctx, int32_t* p, int32_t v, int64_t n, cudaStream_t st);

@@ -14,6 +14,7 @@
 
 #include "common.cuh"
 #include "gemm_tc.cuh"
+#include "gemm_tc2.cuh"
 #include "graph.cuh"
 #include "nn.cuh"
 
@@ -74,9 +75,12 @@ trk_status launch_gemm(trk_ctx* ctx, const bf16* A, int64_t a_rows, int64_t lda,
     TRK_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::smem_bytes(BN, Epi::kTmaStore)));
     attr_set = true;
   }
+  // tcgen05.mma.cta_group::2 on 256 x BN tiles when the K loop is long enough to matter (measured: with one K block the
+  // epilogue paces the tile and coupling two CTAs only adds waiting)
+  const bool pair = BN >= 128 && K >= 4 * tc::BK && debug_knob(kKnobGemmPair) != 0;
   CUtensorMap ta, tb, tc_out;
   TRK_TRY(make_tmap(ctx, &ta, A, a_rows, K, lda, tc::BM));
-  TRK_TRY(make_tmap(ctx, &tb, W, n_pad, K, K, BN));
+  TRK_TRY(make_tmap(ctx, &tb, W, n_pad, K, K, pair ? BN / 2 : BN));
   if (Epi::kTmaStore) {
     if (!out.ptr || out.ld % 8 != 0) return fail(ctx, TRK_ERR_SHAPE, "gemm: the bf16 output needs a row stride that is a multiple of 8");
     TRK_TRY(make_tmap(ctx, &tc_out, out.ptr, out.rows, n_pad, out.ld, 32));
@@ -84,6 +88,20 @@ trk_status launch_gemm(trk_ctx* ctx, const bf16* A, int64_t a_rows, int64_t lda,
     tc_out = ta;
   }
   const int n_tiles = n_pad / BN;
+  if constexpr (BN >= 128) {
+    if (pair) {
+      static bool attr2_set = false;
+      auto kern2 = tc::gemm_tc2_kernel<BN, Epi>;
+      if (!attr2_set) {
+        TRK_CUDA(ctx, cudaFuncSetAttribute(kern2, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::smem_bytes_pair(BN, Epi::kTmaStore)));
+        attr2_set = true;
+      }
+      const int64_t ptiles = ceil_div(rows.m_cap, tc::kPairBM) * n_tiles;
+      const unsigned grid2 = 2u * (unsigned)std::min<int64_t>(ptiles, ctx->sm_count / 2);
+      TRK_LAUNCH(ctx, kern2, grid2, tc::kThreads, tc::smem_bytes_pair(BN, Epi::kTmaStore), st, ta, tb, tc_out, rows, n_tiles, K / tc::BK, ep);
+      return TRK_OK;
+    }
+  }
   const int64_t tiles = ceil_div(rows.m_cap, tc::BM) * n_tiles;
   const unsigned grid = (unsigned)std::min<int64_t>(tiles, ctx->sm_count);
   TRK_LAUNCH(ctx, kern, grid, tc::kThreads, tc::smem_bytes(BN, Epi::kTmaStore), st, ta, tb, tc_out, rows, n_tiles, K / tc::BK, ep);

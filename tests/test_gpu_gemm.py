@@ -5,12 +5,14 @@ import pytest
 pytestmark = pytest.mark.gpu
 
 
-@pytest.mark.parametrize("m,n,k", [(128, 64, 64), (1000, 256, 128), (4096, 1024, 1024), (18944 + 77, 1024, 64), (300, 128, 384),
+@pytest.mark.parametrize("m,n,k", [(128, 64, 64), (1000, 256, 128), (4096, 1024, 1024), (18944 + 77, 1024, 64), (300, 128, 384), (257, 256, 64), (129, 128, 128), (5000, 1024, 1024),
                                    (1, 64, 64)])
 @pytest.mark.parametrize("relu", [True, False])
-def test_gemm_bias_act_matches_fp32_reference(m, n, k, relu):
+@pytest.mark.parametrize("pair", [1, 0], ids=["cta_pair", "single_cta"])
+def test_gemm_bias_act_matches_fp32_reference(m, n, k, relu, pair):
     import torch
-    from paper_2501_05520_b200 import gemm_bf16
+    from paper_2501_05520_b200 import debug_set, gemm_bf16
+    debug_set("gemm_pair", pair)
     g = torch.Generator(device="cuda").manual_seed(m * 7 + n * 3 + k)
     a = (torch.randn(m, k, device="cuda", generator=g)).to(torch.bfloat16)
     w = (torch.randn(n, k, device="cuda", generator=g) / np.sqrt(k)).to(torch.bfloat16)
@@ -28,4 +30,5 @@ def test_gemm_bias_act_matches_fp32_reference(m, n, k, relu):
     wi = torch.randint(-2, 3, (n, k), device="cuda", generator=g).to(torch.bfloat16)
     outi = gemm_bf16(ai, wi, torch.zeros(n, device="cuda"), relu=False)
     refi = (ai.float() @ wi.float().t()).to(torch.bfloat16)
+    debug_set("gemm_pair", 1)
     assert torch.equal(outi, refi)
