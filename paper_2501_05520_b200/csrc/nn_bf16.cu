@@ -15,6 +15,7 @@
 #include "common.cuh"
 #include "gemm_tc.cuh"
 #include "gemm_tc2.cuh"
+#include "gnn_fused.cuh"
 #include "graph.cuh"
 #include "nn.cuh"
 
@@ -145,6 +146,31 @@ trk_status gemm_row_ln(trk_ctx* ctx, const bf16* A, int64_t a_rows, int64_t lda,
                        tc::Rows rows, cudaStream_t st) {
   if (ctx->H == 128) return launch_gemm<128, tc::EpiRowLn>(ctx, A, a_rows, lda, K, W, 128, rows, ep, st);
   return launch_gemm<64, tc::EpiRowLn>(ctx, A, a_rows, lda, K, W, 64, rows, ep, st);
+}
+
+// Fused edge update / decoder of S4 (gnn_fused.cuh), H = 128: E <- E + LNR(W2 LNR(W1 [h_s ; h_d ; e] + b1) + b2) in place,
+// or score = sigmoid(w_out . LNR(W1 [h_s ; h_d ; e] + b1) + b_out).
+template <int MODE>
+trk_status launch_edge_fused(trk_ctx* ctx, const bf16* X, int64_t ldx, bf16* E, int64_t e_rows, const int32_t* src, const int32_t* dst,
+                             const DevLinear& L1, const DevLinear& L2, const float* w_out, float b_out, float* score, tc::Rows rows,
+                             cudaStream_t st) {
+  if (rows.m_cap <= 0) return TRK_OK;
+  static bool attr_set = false;
+  auto kern = gf::gnn_edge_fused_kernel<MODE>;
+  if (!attr_set) {
+    TRK_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, gf::kSmemFused));
+    attr_set = true;
+  }
+  CUtensorMap tw1, tw2, te, test;
+  TRK_TRY(make_tmap(ctx, &tw1, L1.w_bf16, gf::kH, 3 * gf::kH, 3 * gf::kH, 64));
+  TRK_TRY(make_tmap(ctx, &tw2, L2.w_bf16, gf::kH, gf::kH, gf::kH, 64));
+  TRK_TRY(make_tmap(ctx, &te, E, e_rows, gf::kH, gf::kH, 128));
+  TRK_TRY(make_tmap(ctx, &test, E, e_rows, gf::kH, gf::kH, 32));
+  gf::FusedParams p{X, ldx, src, dst, L1.b_f32, L2.b_f32, ctx->cfg.gnn_layernorm, w_out, b_out, score};
+  const int64_t ptiles = ceil_div(rows.m_cap, 2 * gf::kTileRows);
+  const unsigned grid = 2u * (unsigned)std::min<int64_t>(ptiles, ctx->sm_count / 2);
+  TRK_LAUNCH(ctx, kern, grid, gf::kThreadsFused, gf::kSmemFused, st, tw1, tw2, te, test, rows, p);
+  return TRK_OK;
 }
 
 // ---------------------------------------------------------------- small SIMT kernels
@@ -335,8 +361,12 @@ trk_status gnn_forward_bf16(trk_ctx* ctx, const float* hits, int64_t n, const in
     tc::EpiRowLn::Params ep{ctx->edge_enc.layers[1].b_f32, nullptr, nullptr, nullptr, ln, nullptr, 0, E, H, nullptr, 0.f, nullptr};
     TRK_TRY(gemm_row_ln(ctx, T1, t_rows, H, H, ctx->edge_enc.layers[1].w_bf16, ep, erows, st));
   }
+  const bool fused = H == gf::kH && debug_knob(kKnobGnnFused) != 0;
   for (int t = 0; t < ctx->cfg.gnn_iters; ++t) {
-    if (n_edges_cap > 0) {
+    if (n_edges_cap > 0 && fused) {
+      TRK_TRY(launch_edge_fused<gf::kUpdate>(ctx, X, 3 * H, E, e_rows, src, dst, ctx->edge_net.layers[0], ctx->edge_net.layers[1], nullptr,
+                                             0.f, nullptr, erows, st));
+    } else if (n_edges_cap > 0) {
       // PA|PB = h [Wa ; Wb]^T per node, then e <- e + LNR(W2 LNR(Wc e + PA[src] + PB[dst] + b1) + b2)
       TRK_TRY(gemm_store_f32(ctx, X, x_rows, 3 * H, H, ctx->edge_net_wab, 2 * H, PAB, nrows, st));
       tc::EpiRowLn::Params e1{ctx->edge_net.layers[0].b_f32, PAB, src, dst, ln, nullptr, 0, T1, H, nullptr, 0.f, nullptr};
@@ -351,7 +381,11 @@ trk_status gnn_forward_bf16(trk_ctx* ctx, const float* hits, int64_t n, const in
     tc::EpiRowLn::Params n2{ctx->node_net.layers[1].b_f32, nullptr, nullptr, nullptr, ln, X, 3 * H, X, 3 * H, nullptr, 0.f, nullptr};
     TRK_TRY(gemm_row_ln(ctx, T1, t_rows, H, H, ctx->node_net.layers[1].w_bf16, n2, nrows, st));
   }
-  if (n_edges_cap > 0) {
+  if (n_edges_cap > 0 && fused) {
+    // the decoder's second layer is Linear(H -> 1): its fp32 weights are w_out; the W2 operand of the kernel is unused in this mode
+    TRK_TRY(launch_edge_fused<gf::kDecode>(ctx, X, 3 * H, E, e_rows, src, dst, ctx->edge_dec.layers[0], ctx->edge_net.layers[1],
+                                           ctx->edge_dec.layers[1].w_f32, ctx->edge_dec_b_last, score, erows, st));
+  } else if (n_edges_cap > 0) {
     TRK_TRY(gemm_store_f32(ctx, X, x_rows, 3 * H, H, ctx->edge_dec_wab, 2 * H, PAB, nrows, st));
     tc::EpiRowLn::Params d1{ctx->edge_dec.layers[0].b_f32, PAB, src, dst, ln, nullptr, 0, nullptr, 0,
                             ctx->edge_dec.layers[1].w_f32, ctx->edge_dec_b_last, score};
