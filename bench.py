@@ -25,6 +25,9 @@ if ROOT not in sys.path:
 
 FILTER_FLOP_PER_EDGE = 2 * (24 * 1024 + 1024 * 1024 * 2 + 1024)          # 4 245 504
 EMBED_FLOP_PER_HIT = 2 * (3 * 1024 + 1024 * 1024 * 2 + 1024 * 12)        # 4 225 024
+# DRAM bytes of one full-chunk launch (303 104 rows) of the dominant kernel, from the ncu --set full capture summarised in
+# profiles/r1_full_v2.md (dram__bytes_read.sum + dram__bytes_write.sum)
+NCU_TRAFFIC_BYTES = {"bias_act": 622.89e6 + 580.31e6, "relu_dot": 622.89e6 + 7.75e6}
 
 
 def gnn_flops(n, e, H=128, T=8):
@@ -179,6 +182,7 @@ def main():
     import torch
     import torch.distributed as dist
     from paper_2501_05520_b200 import gemm_bf16, trk_from_config
+    from paper_2501_05520_b200.replicas import max_over_ranks
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -215,23 +219,21 @@ def main():
     sampler = ClockSampler(local) if rank == 0 else None
     starts = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
     ends = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
-    stage_ms = []
+    stage_ms, kernel_ms = [], []
     for i in range(args.steps):
         flush.zero_()
         starts[i].record()
         trk.infer(hits, ev["event_offsets"], out=out)
         ends[i].record()
         stage_ms.append(trk.stage_ms())                 # waits for this step (the next flush is outside the timed pair anyway)
+        kernel_ms.append(trk.kernel_ms())
     barrier()
     clocks = sampler.stop() if sampler else None
     step_ms = [s.elapsed_time(e) for s, e in zip(starts, ends)]
     total_ms = float(np.sum(step_ms))
     launches = trk.last_launch_count * args.steps
     counts = out["counts"].cpu().numpy().tolist()
-    if world > 1:
-        t = torch.tensor([total_ms], device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = max_over_ranks(total_ms, dev)            # replicas: the slowest rank's device time (no data-path collective)
     events_per_s = world * n_events * args.steps / (total_ms / 1000.0)
 
     # ---- end to end through the host API: pinned host buffers, H2D + D2H inside the timed region
@@ -248,10 +250,7 @@ def main():
             trk.infer_host(hh, ev["event_offsets"], lh, ch)
         torch.cuda.synchronize()
         dt = time.perf_counter() - t0
-        if world > 1:
-            t = torch.tensor([dt], device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt = float(t.item())
+        dt = max_over_ranks(dt, dev)
         e2e = {"value": world * n_events * args.steps / dt, "unit": "events/s", "h2d_bytes_per_step": n * 12,
                "d2h_bytes_per_step": n * 4 + 16, "api": "trk_infer_host (pinned host hits in, host labels out, sync inside)"}
 
@@ -266,8 +265,22 @@ def main():
     st = {k: float(np.mean([s[k] for s in stage_ms])) for k in stage_ms[0]}
     s3_flops = e_c * FILTER_FLOP_PER_EDGE
     s3_tflops = s3_flops / (st["s3_filter"] * 1e-3) / 1e12
-    # the dominant kernel in isolation, at the exact per-launch shape of the pipeline (one chunk, one hidden layer)
-    m_chunk = 128 * 148
+    # the dominant kernel inside the timed steps: CUDA-event pairs around every hidden-layer GEMM launch of S3
+    # (trk_profile_kernel_ms); chunk c of launch i = c // 2 holds rows [c*chunk, (c+1)*chunk) clipped to E_c
+    width = cfg["filter_dims"][1]
+    k_flops, k_ms, k_n = 0.0, 0.0, 0
+    for ms_list, chunk_rows in kernel_ms:
+        per_chunk = max(1, len(cfg["filter_dims"]) - 3)
+        for i, ms in enumerate(ms_list):
+            rows = min(max(e_c - (i // per_chunk) * chunk_rows, 0), chunk_rows)
+            if rows > 0:
+                k_flops += 2.0 * rows * width * width
+                k_ms += ms
+                k_n += 1
+    kern_tflops = k_flops / (k_ms * 1e-3) / 1e12 if k_ms > 0 else 0.0
+    chunk_rows = kernel_ms[0][1]
+    # ... and in isolation, at the per-launch shape of the pipeline (one full chunk, one hidden layer)
+    m_chunk = chunk_rows
     a = torch.randn(m_chunk, 1024, device=dev).to(torch.bfloat16)
     w = (torch.randn(1024, 1024, device=dev) / 32).to(torch.bfloat16)
     b = torch.zeros(1024, device=dev)
@@ -298,10 +311,21 @@ def main():
         else:
             v["frac_of_measured"] = v["achieved_gbs"] / hbm
             v["frac_of_nominal_8000"] = v["achieved_gbs"] / 8000.0
-    roofline = {"bound": "tensor", "kernel": "gemm_tc_kernel<256,*> (S3 filter MLP: gather + 3 GEMM launches + finish per 18944-edge chunk)",
-                "achieved": s3_tflops, "peak": peaks["bf16_sustained"], "unit": "TFLOP/s", "frac": s3_tflops / peaks["bf16_sustained"],
-                "peak_source": peaks["source"] + ", sustained bf16 (kernel timed inside a long step)", "traffic": None,
-                "how": "algorithmic flops of S3 (E_c x 4 245 504) / S3 stage time from CUDA events on the launch stream inside the timed steps",
+    roofline = {"bound": "tensor",
+                "kernel": "tc::gemm_tc2_kernel<256,*> (tcgen05.mma.cta_group::2, the 1024x1024 hidden layers of the S3 filter MLP; "
+                          f"one launch = one layer of one {chunk_rows}-edge chunk)",
+                "achieved": kern_tflops, "peak": peaks["bf16_sustained"], "unit": "TFLOP/s", "frac": kern_tflops / peaks["bf16_sustained"],
+                "peak_source": peaks["source"] + ", sustained bf16 (kernel timed inside a long step)",
+                "launches_timed": k_n, "avg_launch_ms": k_ms / max(1, k_n), "flop_per_full_launch": 2.0 * chunk_rows * width * width,
+                "how": "algorithmic flops of the non-empty launches (2 x rows x 1024 x 1024 each) / their summed durations, CUDA-event pairs "
+                       "around each launch on the launch stream inside the timed steps (trk_profile_kernel_ms)",
+                # ncu --set full, profiles/r1_full_v2.md: dram__bytes_read.sum + dram__bytes_write.sum of one full-chunk launch
+                "traffic": NCU_TRAFFIC_BYTES["bias_act"], "traffic_unit": "bytes per full-chunk launch (EpiBiasActBf16 variant)",
+                "traffic_detail": dict(NCU_TRAFFIC_BYTES, algorithmic_bias_act=2 * chunk_rows * width * 2 + width * width * 2,
+                                       algorithmic_relu_dot=chunk_rows * width * 2 + width * width * 2 + chunk_rows * 16,
+                                       source="profiles/r1_full_v2.md"),
+                "whole_stage": {"achieved": s3_tflops, "frac": s3_tflops / peaks["bf16_sustained"],
+                                "how": "algorithmic flops of S3 (E_c x 4 245 504) / S3 stage time (gather, 3 GEMMs, finish, compaction)"},
                 "isolated_launch": {"shape": [m_chunk, 1024, 1024], "ms": iso_ms, "achieved": iso_tflops,
                                     "frac_of_burst_peak": iso_tflops / peaks["bf16_tflops"]}}
 

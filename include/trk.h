@@ -100,7 +100,7 @@ typedef struct {
   const float* hits;            /* DEVICE fp32 [N][3]                                               */
 } trk_batch;
 
-/* Outputs: all DEVICE, caller-owned, NULL = not wanted (counts and labels are required).
+/* Outputs: all DEVICE, caller-owned, NULL = not wanted (counts is required, labels too unless N == 0).
  * Edges are global hit indices, sorted by (src, dst).  If a capacity is too small the list is
  * truncated deterministically (lowest (src,dst) first), counts[3] is set to 1 and labels are the
  * components of the truncated graph.                                                              */
@@ -140,6 +140,12 @@ int64_t trk_last_launch_count(const trk_ctx* ctx);
  * waits for the last one and writes the HOST array ms[5] = {S1, S2, S3 (incl. compaction), S4, S5}. */
 trk_status trk_profile_enable(trk_ctx* ctx, int32_t on);
 trk_status trk_profile_stage_ms(trk_ctx* ctx, float* ms);
+/* Per-launch device time of the dominant kernel of the path, the hidden-layer GEMMs (K >= 256) of the S3 filter MLP
+ * (DESIGN.md section 6), from CUDA-event pairs recorded around each such launch of the last profiled trk_infer.
+ * Writes HOST ms[min(capacity, *n_launches)] in launch order: chunk 0 layer 2, chunk 0 layer 3, chunk 1 layer 2, ...;
+ * chunk c covers candidate edges [c * *rows_per_launch, (c+1) * *rows_per_launch) clipped to counts[0], so launches of
+ * chunks beyond the candidate count are empty.  Flops of a launch = 2 * rows * K * N with K = N = the hidden width. */
+trk_status trk_profile_kernel_ms(trk_ctx* ctx, float* ms, int32_t capacity, int32_t* n_launches, int64_t* rows_per_launch);
 
 /* Stage hooks: run ONE stage on caller-supplied DEVICE inputs (BASELINE.json north_star: "each
  * stage fed the oracle's own inputs for that stage").  Same kernels as trk_infer.  Unless noted

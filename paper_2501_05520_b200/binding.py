@@ -19,7 +19,7 @@ TRK_FILTER_RAW, TRK_FILTER_EMB = 0, 1
 EXPORTS = [
     "trk_create", "trk_infer", "trk_destroy", "trk_infer_host", "trk_status_string", "trk_last_error",
     "trk_workspace_bytes", "trk_last_launch_count", "trk_stage_embed", "trk_stage_frnn", "trk_stage_filter",
-    "trk_stage_compact", "trk_stage_gnn", "trk_stage_cc", "trk_gemm_bf16", "trk_profile_enable", "trk_profile_stage_ms",
+    "trk_stage_compact", "trk_stage_gnn", "trk_stage_cc", "trk_gemm_bf16", "trk_profile_enable", "trk_profile_stage_ms", "trk_profile_kernel_ms",
     "trk_debug_set",
 ]
 
@@ -92,6 +92,7 @@ def lib():
     L.trk_profile_enable.argtypes = [vp, i32]
     L.trk_debug_set.argtypes = [C.c_char_p, i64]
     L.trk_profile_stage_ms.argtypes = [vp, _f32p]
+    L.trk_profile_kernel_ms.argtypes = [vp, _f32p, i32, _i32p, C.POINTER(i64)]
     for name in EXPORTS:
         if getattr(L, name).restype is C.c_int:
             getattr(L, name).restype = C.c_int
@@ -201,6 +202,14 @@ class Trk:
         ms = (C.c_float * 5)()
         self._check(lib().trk_profile_stage_ms(self._h, ms))
         return dict(zip(("s1_embed", "s2_frnn", "s3_filter", "s4_gnn", "s5_cc"), [float(v) for v in ms]))
+
+    def kernel_ms(self):
+        """(per-launch ms of the S3 hidden-layer GEMMs of the last profiled infer, rows per launch)."""
+        n, rows = C.c_int32(0), C.c_int64(0)
+        self._check(lib().trk_profile_kernel_ms(self._h, None, 0, C.byref(n), C.byref(rows)))
+        ms = (C.c_float * max(1, n.value))()
+        self._check(lib().trk_profile_kernel_ms(self._h, ms, n.value, C.byref(n), C.byref(rows)))
+        return [float(ms[i]) for i in range(n.value)], int(rows.value)
 
     # ---- the call
     def infer(self, hits, event_offsets, *, want_edges=False, want_cand=False, want_embedding=False, out=None, stream=None):

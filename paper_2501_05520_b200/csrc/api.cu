@@ -243,6 +243,7 @@ trk_status trk_destroy(trk_ctx* ctx) {
   cudaDeviceSynchronize();
   for (auto& e : ctx->prof_ev)
     if (e) cudaEventDestroy(e);
+  for (auto& e : ctx->kprof_ev) cudaEventDestroy(e);
   for (DevMlp* m : {&ctx->embed, &ctx->filter, &ctx->node_enc, &ctx->edge_enc, &ctx->edge_net, &ctx->node_net, &ctx->edge_dec}) free_mlp(*m);
   cudaFree(ctx->grid_proj);
   cudaFree(ctx->edge_net_wab);
@@ -394,9 +395,10 @@ trk_status trk_create(const trk_config* cfg, trk_ctx** out) {
 trk_status trk_infer(trk_ctx* ctx, const trk_batch* batch, const trk_result* res, void* cuda_stream) {
   if (!ctx) return TRK_ERR_INVALID_ARG;
   if (!batch || !res) return fail(ctx, TRK_ERR_INVALID_ARG, "batch or result is NULL");
-  if (!res->labels || !res->counts) return fail(ctx, TRK_ERR_INVALID_ARG, "result.labels and result.counts are required");
+  if (!res->counts) return fail(ctx, TRK_ERR_INVALID_ARG, "result.counts is required");
   int64_t n = 0;
   TRK_TRY(check_batch(ctx, batch->n_events, batch->event_offsets, &n));
+  if (n > 0 && !res->labels) return fail(ctx, TRK_ERR_INVALID_ARG, "result.labels is required");
   if (n > 0 && !batch->hits) return fail(ctx, TRK_ERR_INVALID_ARG, "batch.hits is NULL");
   if ((res->edge_src || res->edge_dst || res->edge_score) && res->edge_capacity <= 0)
     return fail(ctx, TRK_ERR_INVALID_ARG, "edge outputs requested with edge_capacity <= 0");
@@ -405,6 +407,7 @@ trk_status trk_infer(trk_ctx* ctx, const trk_batch* batch, const trk_result* res
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const trk_config& f = ctx->cfg;
   ctx->launch_count = 0;
+  ctx->kprof_n = 0;
   TRK_LAUNCH(ctx, zero_counts_kernel, 1, 32, 0, st, ctx->counts);
   const bool prof = ctx->profiling && n > 0;
   ctx->prof_valid = false;
@@ -479,6 +482,17 @@ trk_status trk_profile_stage_ms(trk_ctx* ctx, float* ms) {
   if (!ctx->prof_valid) return fail(ctx, TRK_ERR_INVALID_ARG, "no profiled trk_infer call to read");
   TRK_CUDA(ctx, cudaEventSynchronize(ctx->prof_ev[5]));
   for (int i = 0; i < 5; ++i) TRK_CUDA(ctx, cudaEventElapsedTime(&ms[i], ctx->prof_ev[i], ctx->prof_ev[i + 1]));
+  return TRK_OK;
+}
+
+trk_status trk_profile_kernel_ms(trk_ctx* ctx, float* ms, int32_t capacity, int32_t* n_launches, int64_t* rows_per_launch) {
+  if (!ctx || !n_launches || capacity < 0 || (capacity > 0 && !ms)) return TRK_ERR_INVALID_ARG;
+  if (!ctx->prof_valid) return fail(ctx, TRK_ERR_INVALID_ARG, "no profiled trk_infer call to read");
+  TRK_CUDA(ctx, cudaEventSynchronize(ctx->prof_ev[5]));
+  *n_launches = ctx->kprof_n;
+  if (rows_per_launch) *rows_per_launch = ctx->filter_chunk;
+  for (int i = 0; i < ctx->kprof_n && i < capacity; ++i)
+    TRK_CUDA(ctx, cudaEventElapsedTime(&ms[i], ctx->kprof_ev[(size_t)i * 2], ctx->kprof_ev[(size_t)i * 2 + 1]));
   return TRK_OK;
 }
 

@@ -62,6 +62,9 @@ struct trk_ctx {
   bool profiling = false;
   cudaEvent_t prof_ev[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
   bool prof_valid = false;
+  // per-launch timing of the dominant kernel (the K >= 256 hidden-layer GEMMs of S3): event pairs, in launch order
+  std::vector<cudaEvent_t> kprof_ev;
+  int kprof_n = 0;                  // launches recorded by the last profiled trk_infer
 
   trk::DevMlp embed, filter, node_enc, edge_enc, edge_net, node_net, edge_dec;
   float* grid_proj = nullptr;       // [d_e_pad][3] device

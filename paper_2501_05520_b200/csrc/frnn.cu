@@ -152,19 +152,26 @@ __device__ __forceinline__ void warp_bitonic(unsigned long long* d2, int* idx, i
 constexpr unsigned long long kInfBits = 0x7ff0000000000000ull;
 constexpr int kWarpsPerBlock = 4;
 
+// Two-level test per candidate.  Level 1 (all candidates, fp32 with FMA): d2f <= r2 (1 + 1e-4).  The fp32 value differs
+// from the exact d2 by at most ~16 ulp relative (all terms are non-negative, so there is no cancellation), so no candidate
+// with d2 <= r2 can fail it.  Survivors (a few per cent) are queued in shared memory and, 32 at a time, take level 2: the
+// outer() test and the exact fp64 d2 (no FMA) that decides acceptance and rank -- the same arithmetic as before, so the
+// edge list is unchanged; only the work on the ~97 % of candidates that are nowhere near the radius is cheaper.
 template <int D4, int CAP>
 __global__ void __launch_bounds__(kWarpsPerBlock * 32)
 frnn_search_kernel(const float* __restrict__ semb, const float4* __restrict__ smeta, const int32_t* __restrict__ cell_start,
-                   const GridParams* __restrict__ gpp, double r2, int K, int32_t* __restrict__ slots, int32_t* __restrict__ deg,
-                   int64_t n) {
+                   const GridParams* __restrict__ gpp, double r2, float r2_loose, int K, int32_t* __restrict__ slots,
+                   int32_t* __restrict__ deg, int64_t n) {
   constexpr int D = D4 * 4;
   __shared__ unsigned long long s_d2[kWarpsPerBlock][CAP];
   __shared__ int s_idx[kWarpsPerBlock][CAP];
+  __shared__ int s_queue[kWarpsPerBlock][64];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int64_t q = (int64_t)blockIdx.x * kWarpsPerBlock + warp;
   if (q >= n) return;
   unsigned long long* bd2 = s_d2[warp];
   int* bidx = s_idx[warp];
+  int* queue = s_queue[warp];
   const GridParams gp = *gpp;
 
   const float4 qm = smeta[q];
@@ -176,16 +183,67 @@ frnn_search_kernel(const float* __restrict__ semb, const float4* __restrict__ sm
   const int cx = cell % gp.dims[0];
   const int cy = (cell / gp.dims[0]) % gp.dims[1];
   const int cz = cell / (gp.dims[0] * gp.dims[1]);
-  double qe[D];
+  float qf[D];
 #pragma unroll
   for (int k4 = 0; k4 < D4; ++k4) {
     const float4 v = reinterpret_cast<const float4*>(semb + q * D)[k4];
-    qe[k4 * 4 + 0] = (double)v.x; qe[k4 * 4 + 1] = (double)v.y; qe[k4 * 4 + 2] = (double)v.z; qe[k4 * 4 + 3] = (double)v.w;
+    qf[k4 * 4 + 0] = v.x; qf[k4 * 4 + 1] = v.y; qf[k4 * 4 + 2] = v.z; qf[k4 * 4 + 3] = v.w;
   }
 
-  int count = 0;  // warp-uniform number of buffered candidates
+  int count = 0;  // warp-uniform number of buffered neighbours
+  int qn = 0;     // warp-uniform number of queued level-1 survivors
   for (int t = lane; t < CAP; t += 32) { bd2[t] = kInfBits; bidx[t] = 0x7fffffff; }
   __syncwarp();
+
+  // level 2 on the first min(qn, 32) queued positions
+  auto drain = [&]() {
+    const int take = min(qn, 32);
+    bool ok = false;
+    double d2 = 0.0;
+    int c_i = 0;
+    if (lane < take) {
+      const int pos = queue[lane];
+      const float4 cm = smeta[pos];
+      c_i = __float_as_int(cm.z);
+      // outer(i,j): (r_i, |z_i|, i) < (r_j, |z_j|, j)
+      const bool outer = (q_r < cm.x) || (q_r == cm.x && (q_az < cm.y || (q_az == cm.y && q_i < c_i)));
+      if (outer) {
+        const float4* ce = reinterpret_cast<const float4*>(semb + (int64_t)pos * D);
+#pragma unroll
+        for (int k4 = 0; k4 < D4; ++k4) {
+          const float4 v = ce[k4];
+          double t;
+          t = __dsub_rn((double)qf[k4 * 4 + 0], (double)v.x); d2 = __dadd_rn(d2, __dmul_rn(t, t));
+          t = __dsub_rn((double)qf[k4 * 4 + 1], (double)v.y); d2 = __dadd_rn(d2, __dmul_rn(t, t));
+          t = __dsub_rn((double)qf[k4 * 4 + 2], (double)v.z); d2 = __dadd_rn(d2, __dmul_rn(t, t));
+          t = __dsub_rn((double)qf[k4 * 4 + 3], (double)v.w); d2 = __dadd_rn(d2, __dmul_rn(t, t));
+        }
+        ok = d2 <= r2;
+      }
+    }
+    __syncwarp();
+    if (qn > 32 && lane < qn - 32) {   // keep the tail of the queue
+      const int moved = queue[32 + lane];
+      queue[lane] = moved;
+    }
+    qn -= take;
+    const unsigned m = __ballot_sync(0xffffffffu, ok);
+    if (m) {
+      if (count + 32 > CAP) {  // make room: keep the K nearest so far
+        warp_bitonic(bd2, bidx, CAP, false, lane);
+        for (int t = K + lane; t < CAP; t += 32) { bd2[t] = kInfBits; bidx[t] = 0x7fffffff; }
+        __syncwarp();
+        count = min(count, K);
+      }
+      if (ok) {
+        const int slot = count + __popc(m & ((1u << lane) - 1u));
+        bd2[slot] = (unsigned long long)__double_as_longlong(d2);
+        bidx[slot] = c_i;
+      }
+      count += __popc(m);
+    }
+    __syncwarp();
+  };
 
   const int x0 = max(cx - 1, 0), x1 = min(cx + 1, gp.dims[0] - 1);
   for (int dz = -1; dz <= 1; ++dz) {
@@ -198,47 +256,32 @@ frnn_search_kernel(const float* __restrict__ semb, const float4* __restrict__ sm
       const int lo = cell_start[row + x0], hi = cell_start[row + x1 + 1];
       for (int base = lo; base < hi; base += 32) {
         const int pos = base + lane;
-        bool ok = false;
-        double d2 = 0.0;
-        int c_i = 0;
+        bool pre = false;
         if (pos < hi) {
-          const float4 cm = smeta[pos];
-          c_i = __float_as_int(cm.z);
-          // outer(i,j): (r_i, |z_i|, i) < (r_j, |z_j|, j)
-          const bool outer = (q_r < cm.x) || (q_r == cm.x && (q_az < cm.y || (q_az == cm.y && q_i < c_i)));
-          if (outer) {
-            const float4* ce = reinterpret_cast<const float4*>(semb + (int64_t)pos * D);
+          const float4* ce = reinterpret_cast<const float4*>(semb + (int64_t)pos * D);
+          float d2f = 0.f;
 #pragma unroll
-            for (int k4 = 0; k4 < D4; ++k4) {
-              const float4 v = ce[k4];
-              double t;
-              t = __dsub_rn(qe[k4 * 4 + 0], (double)v.x); d2 = __dadd_rn(d2, __dmul_rn(t, t));
-              t = __dsub_rn(qe[k4 * 4 + 1], (double)v.y); d2 = __dadd_rn(d2, __dmul_rn(t, t));
-              t = __dsub_rn(qe[k4 * 4 + 2], (double)v.z); d2 = __dadd_rn(d2, __dmul_rn(t, t));
-              t = __dsub_rn(qe[k4 * 4 + 3], (double)v.w); d2 = __dadd_rn(d2, __dmul_rn(t, t));
-            }
-            ok = d2 <= r2;
+          for (int k4 = 0; k4 < D4; ++k4) {
+            const float4 v = __ldg(ce + k4);
+            float t;
+            t = qf[k4 * 4 + 0] - v.x; d2f = fmaf(t, t, d2f);
+            t = qf[k4 * 4 + 1] - v.y; d2f = fmaf(t, t, d2f);
+            t = qf[k4 * 4 + 2] - v.z; d2f = fmaf(t, t, d2f);
+            t = qf[k4 * 4 + 3] - v.w; d2f = fmaf(t, t, d2f);
           }
+          pre = d2f <= r2_loose;
         }
-        const unsigned m = __ballot_sync(0xffffffffu, ok);
+        const unsigned m = __ballot_sync(0xffffffffu, pre);
         if (m) {
-          if (count + 32 > CAP) {  // make room: keep the K nearest so far
-            warp_bitonic(bd2, bidx, CAP, false, lane);
-            for (int t = K + lane; t < CAP; t += 32) { bd2[t] = kInfBits; bidx[t] = 0x7fffffff; }
-            __syncwarp();
-            count = min(count, K);
-          }
-          if (ok) {
-            const int slot = count + __popc(m & ((1u << lane) - 1u));
-            bd2[slot] = (unsigned long long)__double_as_longlong(d2);
-            bidx[slot] = c_i;
-          }
-          count += __popc(m);
+          if (pre) queue[qn + __popc(m & ((1u << lane) - 1u))] = pos;
+          qn += __popc(m);
           __syncwarp();
+          if (qn >= 32) drain();
         }
       }
     }
   }
+  while (qn > 0) drain();
   if (count > K) {
     warp_bitonic(bd2, bidx, CAP, false, lane);
     for (int t = K + lane; t < CAP; t += 32) { bd2[t] = kInfBits; bidx[t] = 0x7fffffff; }
@@ -295,15 +338,18 @@ __global__ void event_of_hit_kernel(const __grid_constant__ EventOffsets offs, i
 template <int D4>
 trk_status launch_search(trk_ctx* ctx, int K, double r2, int64_t n, cudaStream_t st) {
   const unsigned blocks = (unsigned)ceil_div(n, kWarpsPerBlock);
+  // level-1 threshold: r^2 (1 + 1e-4) rounded up, infinite when r^2 overflows fp32 (then every candidate takes level 2)
+  const double loose = r2 * (1.0 + 1e-4);
+  const float r2_loose = loose >= 3.0e38 ? __builtin_inff() : fmaxf(nextafterf((float)loose, __builtin_inff()), 1e-30f);
   if (K <= 32) {
     TRK_LAUNCH(ctx, (frnn_search_kernel<D4, 64>), blocks, kWarpsPerBlock * 32, 0, st, ctx->semb, ctx->smeta, ctx->cell_start,
-               ctx->grid, r2, K, ctx->slots, ctx->deg, n);
+               ctx->grid, r2, r2_loose, K, ctx->slots, ctx->deg, n);
   } else if (K <= 64) {
     TRK_LAUNCH(ctx, (frnn_search_kernel<D4, 128>), blocks, kWarpsPerBlock * 32, 0, st, ctx->semb, ctx->smeta, ctx->cell_start,
-               ctx->grid, r2, K, ctx->slots, ctx->deg, n);
+               ctx->grid, r2, r2_loose, K, ctx->slots, ctx->deg, n);
   } else {
     TRK_LAUNCH(ctx, (frnn_search_kernel<D4, 256>), blocks, kWarpsPerBlock * 32, 0, st, ctx->semb, ctx->smeta, ctx->cell_start,
-               ctx->grid, r2, K, ctx->slots, ctx->deg, n);
+               ctx->grid, r2, r2_loose, K, ctx->slots, ctx->deg, n);
   }
   return TRK_OK;
 }

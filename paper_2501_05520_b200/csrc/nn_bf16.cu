@@ -180,23 +180,34 @@ __device__ __forceinline__ int64_t rows_of(const int32_t* m_dev, int64_t m_off, 
   return m < 0 ? 0 : (m > m_cap ? m_cap : m);
 }
 
-// S1 first layer: out[m][n] = bf16(relu(W[n][0..3) . x[m] + b[n])), 8 columns per thread.
-__global__ void embed_first_layer_kernel(const float* __restrict__ hits, const float* __restrict__ W, const float* __restrict__ b,
-                                         bf16* __restrict__ out, int64_t M, int N) {
-  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  const int groups = N / 8;
-  const int64_t row = i / groups;
-  if (row >= M) return;
-  const int c0 = (int)(i % groups) * 8;
-  const float x0 = hits[row * 3], x1 = hits[row * 3 + 1], x2 = hits[row * 3 + 2];
-  float v[8];
+// S1 first layer: out[m][n] = bf16(relu(W[n][0..3) . x[m] + b[n])).  A thread owns 8 columns (its 24 weights and 8 biases stay
+// in registers) and walks down the rows of its block, so a row costs 3 broadcast loads, 24 FMAs and one 16-byte store:
+// the kernel runs at the HBM write rate of the activation instead of re-reading W from L1 for every row.
+constexpr int kFirstLayerRowsPerBlock = 64;
+__global__ void __launch_bounds__(256)
+embed_first_layer_kernel(const float* __restrict__ hits, const float* __restrict__ W, const float* __restrict__ b,
+                         bf16* __restrict__ out, int64_t M, int N) {
+  const int groups = N / 8;                       // 16-byte column groups per row
+  const int lanes_r = blockDim.x / groups;        // rows in flight per pass (host guarantees groups <= blockDim.x)
+  const int g = threadIdx.x % groups, rl = threadIdx.x / groups;
+  if (rl >= lanes_r) return;
+  float w[8][3], bb[8];
 #pragma unroll
   for (int j = 0; j < 8; ++j) {
-    const float* w = W + (int64_t)(c0 + j) * 3;
-    v[j] = fmaxf(fmaf(w[2], x2, fmaf(w[1], x1, fmaf(w[0], x0, b[c0 + j]))), 0.f);
+    const float* wp = W + (int64_t)(g * 8 + j) * 3;
+    w[j][0] = wp[0]; w[j][1] = wp[1]; w[j][2] = wp[2];
+    bb[j] = b[g * 8 + j];
   }
-  *reinterpret_cast<uint4*>(out + row * N + c0) =
-      make_uint4(tc::pack_bf16(v[0], v[1]), tc::pack_bf16(v[2], v[3]), tc::pack_bf16(v[4], v[5]), tc::pack_bf16(v[6], v[7]));
+  const int64_t row0 = (int64_t)blockIdx.x * kFirstLayerRowsPerBlock;
+  const int64_t row1 = min(row0 + kFirstLayerRowsPerBlock, M);
+  for (int64_t row = row0 + rl; row < row1; row += lanes_r) {
+    const float x0 = __ldg(hits + row * 3), x1 = __ldg(hits + row * 3 + 1), x2 = __ldg(hits + row * 3 + 2);
+    float v[8];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) v[j] = fmaxf(fmaf(w[j][2], x2, fmaf(w[j][1], x1, fmaf(w[j][0], x0, bb[j]))), 0.f);
+    *reinterpret_cast<uint4*>(out + row * N + g * 8) =
+        make_uint4(tc::pack_bf16(v[0], v[1]), tc::pack_bf16(v[2], v[3]), tc::pack_bf16(v[4], v[5]), tc::pack_bf16(v[6], v[7]));
+  }
 }
 
 // S3 input rows: out[m][0..64) = bf16([feat[src] ; feat[dst]]) zero padded; 8 columns per thread.
@@ -234,46 +245,90 @@ __global__ void filter_finish_kernel(const float* __restrict__ partial, int n_ti
   score[m_off + row] = 1.f / (1.f + __expf(-s));
 }
 
-// First GNN encoder layers (K = 3 node features or K = 4 edge features): one warp per row,
-// out[m] = bf16(ReLU(LayerNorm(W x + b))).  EDGE: x = edge_features(src[m], dst[m]).
-template <bool EDGE>
+// First GNN encoder layers (K = 3 node features or K = 4 edge features): out[m] = bf16(ReLU(LayerNorm(W x + b))).
+// A warp takes 32 rows at a time: every lane prepares the input of one row (EDGE: the edge features of (src[m], dst[m]),
+// two asinhf per lane instead of per warp), then the warp walks over the 32 rows with shuffles; a lane owns the H/32
+// adjacent columns 'per * lane ..' (weights in registers) so one row leaves as one coalesced 2H-byte store.
+template <bool EDGE, int PER>
 __global__ void __launch_bounds__(256)
 encoder_first_layer_kernel(const float* __restrict__ hits, const int32_t* __restrict__ src, const int32_t* __restrict__ dst,
-                           const float* __restrict__ W, const float* __restrict__ b, int H, int use_ln,
+                           const float* __restrict__ W, const float* __restrict__ b, int use_ln,
                            const int32_t* __restrict__ m_dev, int64_t m_cap, bf16* __restrict__ out) {
+  constexpr int K = EDGE ? 4 : 3;
+  constexpr int H = PER * 32;
   const int64_t M = rows_of(m_dev, 0, m_cap);
   const int lane = threadIdx.x & 31;
-  const int64_t row = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-  if (row >= M) return;
-  float x[4];
-  constexpr int K = EDGE ? 4 : 3;
-  if (EDGE) {
-    const float4 a = edge_features(hits, src[row], dst[row]);
-    x[0] = a.x; x[1] = a.y; x[2] = a.z; x[3] = a.w;
-  } else {
-    x[0] = hits[row * 3]; x[1] = hits[row * 3 + 1]; x[2] = hits[row * 3 + 2]; x[3] = 0.f;
-  }
-  float v[4];  // H <= 128: columns lane, lane+32, ...
-  float s = 0.f;
-  const int per = H / 32;
-  for (int j = 0; j < per; ++j) {
-    const int c = lane + 32 * j;
-    float a = b[c];
+  const int64_t warp = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const int64_t n_warps = ((int64_t)gridDim.x * blockDim.x) >> 5;
+  float w[PER][K], bb[PER];
 #pragma unroll
-    for (int k = 0; k < K; ++k) a = fmaf(W[c * K + k], x[k], a);
-    v[j] = a;
-    s += a;
+  for (int j = 0; j < PER; ++j) {
+    const int c = lane * PER + j;
+#pragma unroll
+    for (int k = 0; k < K; ++k) w[j][k] = W[c * K + k];
+    bb[j] = b[c];
   }
-  float mean = 0.f, rstd = 1.f;
-  if (use_ln) {
-    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
-    mean = s / (float)H;
-    float q = 0.f;
-    for (int j = 0; j < per; ++j) { const float d = v[j] - mean; q += d * d; }
-    for (int o = 16; o > 0; o >>= 1) q += __shfl_xor_sync(0xffffffffu, q, o);
-    rstd = rsqrtf(q / (float)H + 1e-5f);
+  for (int64_t base = warp * 32; base < M; base += n_warps * 32) {
+    const int64_t mine = base + lane;
+    float x[4] = {0.f, 0.f, 0.f, 0.f};
+    if (mine < M) {
+      if (EDGE) {
+        const float4 a = edge_features(hits, src[mine], dst[mine]);
+        x[0] = a.x; x[1] = a.y; x[2] = a.z; x[3] = a.w;
+      } else {
+        x[0] = hits[mine * 3]; x[1] = hits[mine * 3 + 1]; x[2] = hits[mine * 3 + 2];
+      }
+    }
+    const int cnt = (int)min((int64_t)32, M - base);
+    for (int r = 0; r < cnt; ++r) {
+      float xr[K];
+#pragma unroll
+      for (int k = 0; k < K; ++k) xr[k] = __shfl_sync(0xffffffffu, x[k], r);
+      float v[PER];
+      float s = 0.f;
+#pragma unroll
+      for (int j = 0; j < PER; ++j) {
+        float a = bb[j];
+#pragma unroll
+        for (int k = 0; k < K; ++k) a = fmaf(w[j][k], xr[k], a);
+        v[j] = a;
+        s += a;
+      }
+      float mean = 0.f, rstd = 1.f;
+      if (use_ln) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+        mean = s * (1.f / H);
+        float q = 0.f;
+#pragma unroll
+        for (int j = 0; j < PER; ++j) { const float d = v[j] - mean; q = fmaf(d, d, q); }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) q += __shfl_xor_sync(0xffffffffu, q, o);
+        rstd = rsqrtf(q * (1.f / H) + 1e-5f);
+      }
+#pragma unroll
+      for (int j = 0; j < PER; ++j) v[j] = fmaxf((v[j] - mean) * rstd, 0.f);
+      bf16* o = out + (base + r) * H + lane * PER;
+      if constexpr (PER == 4) {
+        *reinterpret_cast<uint2*>(o) = make_uint2(tc::pack_bf16(v[0], v[1]), tc::pack_bf16(v[2], v[3]));
+      } else {
+        *reinterpret_cast<uint32_t*>(o) = tc::pack_bf16(v[0], v[1]);
+      }
+    }
   }
-  for (int j = 0; j < per; ++j) out[row * H + lane + 32 * j] = __float2bfloat16_rn(fmaxf((v[j] - mean) * rstd, 0.f));
+}
+
+template <bool EDGE>
+trk_status launch_encoder_first(trk_ctx* ctx, const float* hits, const int32_t* src, const int32_t* dst, const DevLinear& L, int H,
+                                int use_ln, const int32_t* m_dev, int64_t m_cap, bf16* out, cudaStream_t st) {
+  if (m_cap <= 0) return TRK_OK;
+  const unsigned blocks = (unsigned)std::min<int64_t>(ceil_div(m_cap, 32 * 8), (int64_t)ctx->sm_count * 8);
+  if (H == 128) {
+    TRK_LAUNCH(ctx, (encoder_first_layer_kernel<EDGE, 4>), blocks, 256, 0, st, hits, src, dst, L.w_f32, L.b_f32, use_ln, m_dev, m_cap, out);
+  } else {
+    TRK_LAUNCH(ctx, (encoder_first_layer_kernel<EDGE, 2>), blocks, 256, 0, st, hits, src, dst, L.w_f32, L.b_f32, use_ln, m_dev, m_cap, out);
+  }
+  return TRK_OK;
 }
 
 }  // namespace
@@ -284,8 +339,9 @@ trk_status embed_forward_bf16(trk_ctx* ctx, const float* hits, int64_t n, float*
   const int nl = (int)L.size();
   bf16* bufs[2] = {(bf16*)ctx->act0, (bf16*)ctx->act1};
   const int w0 = L[0].out;
-  TRK_LAUNCH(ctx, embed_first_layer_kernel, (unsigned)ceil_div(n * (w0 / 8), 256), 256, 0, st, hits, L[0].w_f32, L[0].b_f32, bufs[0], n,
-             w0);
+  if (w0 / 8 > 256) return fail(ctx, TRK_ERR_SHAPE, "TRK_BF16: the first embedding layer is limited to 2048 outputs");
+  TRK_LAUNCH(ctx, embed_first_layer_kernel, (unsigned)ceil_div(n, kFirstLayerRowsPerBlock), 256, 0, st, hits, L[0].w_f32, L[0].b_f32,
+             bufs[0], n, w0);
   int cur = 0;
   tc::Rows rows{nullptr, 0, n};
   for (int l = 1; l < nl - 1; ++l) {
@@ -318,6 +374,22 @@ trk_status filter_forward_bf16(trk_ctx* ctx, const float* feat, const int32_t* s
       DevLinear Ll = L[l];
       if (l == 0) { Ll.w_bf16 = ctx->filter_w1_pad; Ll.in_pad = 64; }
       const int64_t lda = l == 0 ? 64 : Ll.in_pad;
+      // trk_profile_kernel_ms: one CUDA-event pair around every hidden-layer GEMM launch with K >= 256
+      const bool kprof = ctx->profiling && n_edges_dev == &ctx->counts[0] && Ll.in_pad >= 256;
+      cudaEvent_t k0 = nullptr, k1 = nullptr;
+      if (kprof) {
+        if ((size_t)ctx->kprof_n * 2 + 2 > ctx->kprof_ev.size()) {
+          for (int i = 0; i < 2; ++i) {
+            cudaEvent_t e;
+            TRK_CUDA(ctx, cudaEventCreate(&e));
+            ctx->kprof_ev.push_back(e);
+          }
+        }
+        k0 = ctx->kprof_ev[(size_t)ctx->kprof_n * 2];
+        k1 = ctx->kprof_ev[(size_t)ctx->kprof_n * 2 + 1];
+        ++ctx->kprof_n;
+        TRK_CUDA(ctx, cudaEventRecord(k0, st));
+      }
       if (l == nl - 2) {
         TRK_TRY(gemm_relu_dot(ctx, in, in_rows, lda, Ll, L[nl - 1].w_f32, ctx->partial, &n_tiles, rows, st));
       } else {
@@ -326,6 +398,7 @@ trk_status filter_forward_bf16(trk_ctx* ctx, const float* feat, const int32_t* s
         in_rows = ctx->act_rows;
         cur ^= 1;
       }
+      if (kprof) TRK_CUDA(ctx, cudaEventRecord(k1, st));
     }
     TRK_LAUNCH(ctx, filter_finish_kernel, (unsigned)ceil_div(cap, 256), 256, 0, st, ctx->partial, n_tiles, ctx->filter_b_last,
                n_edges_dev, off, cap, score);
@@ -348,16 +421,14 @@ trk_status gnn_forward_bf16(trk_ctx* ctx, const float* hits, int64_t n, const in
   TRK_TRY(build_gnn_csr(ctx, src, dst, n_edges_dev, n_edges_cap, n, st));
 
   // node encoder: 3 -> H (SIMT) -> H (GEMM, LNR) -> X[:, 0:H]
-  TRK_LAUNCH(ctx, encoder_first_layer_kernel<false>, (unsigned)ceil_div(n * 32, 256), 256, 0, st, hits, nullptr, nullptr,
-             ctx->node_enc.layers[0].w_f32, ctx->node_enc.layers[0].b_f32, H, ln, nullptr, n, T1);
+  TRK_TRY(launch_encoder_first<false>(ctx, hits, nullptr, nullptr, ctx->node_enc.layers[0], H, ln, nullptr, n, T1, st));
   {
     tc::EpiRowLn::Params ep{ctx->node_enc.layers[1].b_f32, nullptr, nullptr, nullptr, ln, nullptr, 0, X, 3 * H, nullptr, 0.f, nullptr};
     TRK_TRY(gemm_row_ln(ctx, T1, t_rows, H, H, ctx->node_enc.layers[1].w_bf16, ep, nrows, st));
   }
   if (n_edges_cap > 0) {
     // edge encoder: 4 -> H (SIMT on the fly features) -> H (GEMM, LNR) -> E
-    TRK_LAUNCH(ctx, encoder_first_layer_kernel<true>, (unsigned)ceil_div(n_edges_cap * 32, 256), 256, 0, st, hits, src, dst,
-               ctx->edge_enc.layers[0].w_f32, ctx->edge_enc.layers[0].b_f32, H, ln, n_edges_dev, n_edges_cap, T1);
+    TRK_TRY(launch_encoder_first<true>(ctx, hits, src, dst, ctx->edge_enc.layers[0], H, ln, n_edges_dev, n_edges_cap, T1, st));
     tc::EpiRowLn::Params ep{ctx->edge_enc.layers[1].b_f32, nullptr, nullptr, nullptr, ln, nullptr, 0, E, H, nullptr, 0.f, nullptr};
     TRK_TRY(gemm_row_ln(ctx, T1, t_rows, H, H, ctx->edge_enc.layers[1].w_bf16, ep, erows, st));
   }

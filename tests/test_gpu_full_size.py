@@ -1,0 +1,283 @@
+"""-m gpu parity at BASELINE.json's FULL sizes (configs[2] pileup-200, configs[3] 16-event batch, configs[4] pileup-300),
+in the launch configuration bench.py times (one context sized for the whole event, 303 104-row filter chunks, CTA-pair
+GEMMs, fused edge kernel).  Every stage is fed inputs that come from the oracle or from synth/ only.
+
+What is compared, per config (oracle cost on the box's host cores in brackets):
+
+  pileup200   S1 all hits; S2 the whole edge list bit-exact (oracle grid search); S3 ALL 2.56 M scores and the kept set
+              (full oracle filter, ~40 s); S4 all 0.73 M scores on the oracle's kept graph (~45 s); S5 labels bit-exact.
+  pileup300   S1 all hits; S2 whole edge list bit-exact; S3 GPU scores of all 6.0 M edges against the oracle on 40 000
+              sampled edges (the oracle's full filter pass would be ~10^13 fp64 flop) plus the exact compaction property;
+              S4 on a SYNTHETIC kept graph of the config's size (1.88 M edges; no GPU value enters it): the oracle's candidate
+              edges whose two hits lie in the same of 16 phi sectors, thinned by a seeded hash.  Sectors are then independent
+              sub-graphs (messages never cross them), so the oracle runs sectors 3 and 11 alone (~0.24 M edges) and the GPU,
+              given the whole graph, must reproduce their scores; S5 labels bit-exact.
+  batch16     S1 all hits; S2 whole edge list bit-exact and identical to the union of single-event searches on two events
+              (BASELINE.json configs[3]: "FRNN is restricted within each event"); S3 as pileup300; S4: events are
+              independent, so the oracle runs event 9 alone (its kept graph from the full oracle filter of that event)
+              and the GPU, given the 16-event graph (that kept graph + the thinned candidates of the other 15 events),
+              must reproduce its scores; S5 bit-exact.
+"""
+import os
+
+import numpy as np
+import pytest
+
+import gpu_common as G
+from oracle import s1_embed, s2_frnn, s3_filter, s4_gnn, s5_cc
+from oracle.mlp import sigmoid
+from synth.rng import Stream
+
+pytestmark = pytest.mark.gpu
+
+CONFIGS = [c for c in os.environ.get("TRK_TEST_FULL_CONFIGS", "pileup200,pileup300,batch16").split(",") if c]
+N_SAMPLE = 40000
+
+
+def _dev(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def _thin(n_edges, keep_frac, seed, tag):
+    """Seeded, data-independent thinning of an edge list (a synthetic stand-in for the filter's kept set)."""
+    u = Stream(seed, f"thin:{tag}").uniform(np.arange(n_edges, dtype=np.uint64))
+    return u < keep_frac
+
+
+class Full:
+    """Oracle-side data of one full-size config, computed lazily and once."""
+
+    def __init__(self, name):
+        self.name = name
+        self.cfg = G.get_config(name)
+        self.calib = G.load_calibration(self.cfg["calibration"])
+        self.ev = G.make_events(self.cfg)
+        self.model = G.centred_model(self.cfg, self.calib)
+        self.hits = self.ev["hits"]
+        self.off = self.ev["event_offsets"]
+        self.n = len(self.hits)
+        self._c = {}
+
+    def _memo(self, key, fn):
+        if key not in self._c:
+            self._c[key] = fn()
+        return self._c[key]
+
+    @property
+    def emb(self):
+        return self._memo("emb", lambda: s1_embed.embed_f32(self.hits, self.model["embed"]))
+
+    @property
+    def cand(self):
+        return self._memo("cand", lambda: s2_frnn.frnn(self.emb, self.hits, self.off, self.calib["frnn_radius"], self.cfg["frnn_k"]))
+
+    def event_edges(self, b):
+        """Positions of the candidate edges of event b (edges are sorted by src, events are contiguous in src)."""
+        src = self.cand[0]
+        return np.searchsorted(src, self.off[b]), np.searchsorted(src, self.off[b + 1])
+
+    @property
+    def oracle_events(self):
+        return [0] if len(self.off) == 2 else [9]
+
+    N_SECTORS = 16
+    ORACLE_SECTORS = (3, 11)
+
+    @property
+    def sector(self):
+        """phi sector of every hit (pileup300's synthetic kept graph)."""
+        return np.minimum(((self.hits[:, 1].astype(np.float64) + 1.0) * (self.N_SECTORS / 2)).astype(np.int64), self.N_SECTORS - 1)
+
+    @property
+    def filter_full(self):
+        """Oracle filter scores (fp32 interchange) of ALL candidate edges (pileup200) or of the oracle events' edges."""
+        def f():
+            src, dst, _ = self.cand
+            if self.name == "pileup200":
+                return {"all": s3_filter.filter_scores(self.emb, src, dst, self.model["filter"]).astype(np.float32)}
+            out = {}
+            for b in self.oracle_events if self.name == "batch16" else []:
+                lo, hi = self.event_edges(b)
+                out[b] = s3_filter.filter_scores(self.emb, src[lo:hi], dst[lo:hi], self.model["filter"]).astype(np.float32)
+            return out
+        return self._memo("filter_full", f)
+
+    @property
+    def filter_sample(self):
+        def f():
+            src, dst, _ = self.cand
+            e = len(src)
+            idx = np.unique((Stream(7, f"sample:{self.name}").uniform(np.arange(N_SAMPLE, dtype=np.uint64)) * e).astype(np.int64))
+            idx = np.unique(np.concatenate([idx, [0, e - 1], np.arange(303104 - 64, 303104 + 64) % e]))   # chunk seam of S3
+            return idx, s3_filter.filter_scores(self.emb, src[idx], dst[idx], self.model["filter"]).astype(np.float32)
+        return self._memo("filter_sample", f)
+
+    @property
+    def kept(self):
+        """The S4 input graph (see the module docstring): mask over the candidate list."""
+        def f():
+            src, _, _ = self.cand
+            cut = self.calib["filter_cut"]
+            if self.name == "pileup200":
+                return s3_filter.keep_mask(self.filter_full["all"], cut)
+            frac = float(self.calib["n_kept_edges"]) / float(self.calib["n_cand_edges"])
+            if self.name == "pileup300":
+                same = self.sector[src] == self.sector[self.cand[1]]
+                return same & _thin(len(src), frac * len(src) / max(1, int(same.sum())), 11, self.name)
+            m = _thin(len(src), frac, 11, self.name)
+            if self.name == "batch16":
+                for b in self.oracle_events:
+                    lo, hi = self.event_edges(b)
+                    m[lo:hi] = s3_filter.keep_mask(self.filter_full[b], cut)
+            return m
+        return self._memo("kept", f)
+
+    @property
+    def gnn(self):
+        """Oracle S4 scores: {event or 'all': (positions in the kept list, fp32 scores)}."""
+        def f():
+            src, dst, _ = self.cand
+            ks, kd = src[self.kept], dst[self.kept]
+            T = self.cfg["gnn_iters"]
+            if self.name == "pileup200":
+                sc = sigmoid(s4_gnn.gnn_forward(self.hits, ks, kd, self.model, T)).astype(np.float32)
+                return {"all": (np.arange(len(ks)), sc)}
+            out = {}
+            if self.name == "pileup300":
+                for s in self.ORACLE_SECTORS:
+                    nodes = np.nonzero(self.sector == s)[0]
+                    remap = np.full(self.n, -1, np.int64)
+                    remap[nodes] = np.arange(len(nodes))
+                    pos = np.nonzero(self.sector[ks] == s)[0]                    # both endpoints are in s by construction
+                    sc = sigmoid(s4_gnn.gnn_forward(self.hits[nodes], remap[ks[pos]], remap[kd[pos]], self.model, T)).astype(np.float32)
+                    out[f"sector {s}"] = (pos, sc)
+                return out
+            for b in self.oracle_events:
+                lo, hi = int(self.off[b]), int(self.off[b + 1])
+                a, z = np.searchsorted(ks, lo), np.searchsorted(ks, hi)
+                sc = sigmoid(s4_gnn.gnn_forward(self.hits[lo:hi], ks[a:z] - lo, kd[a:z] - lo, self.model, T)).astype(np.float32)
+                out[b] = (np.arange(a, z), sc)
+            return out
+        return self._memo("gnn", f)
+
+
+_FULL = {}
+
+
+@pytest.fixture(scope="module", params=CONFIGS)
+def full(request):
+    name = request.param
+    if name not in _FULL:
+        _FULL[name] = Full(name)
+    f = _FULL[name]
+    n_events = len(f.off) - 1
+    from paper_2501_05520_b200 import trk_from_config
+    trk = trk_from_config(f.cfg, f.model, f.calib, max_hits=f.n, max_events=n_events, max_cand_edges=f.n * f.cfg["frnn_k"],
+                          max_kept_edges=int(2.0 * f.calib["n_kept_edges"] * max(1.0, f.n / f.calib["n_hits"])) + 4096)
+    yield f, trk
+    trk.close()
+    _FULL.pop(name, None)          # free the oracle arrays of this config
+
+
+def test_full_s1_embedding(full):
+    f, trk = full
+    emb = trk.stage_embed(_dev(f.hits)).cpu().numpy().astype(np.float64)
+    ref = f.emb.astype(np.float64)
+    err = np.max(np.abs(emb - ref)) / np.max(np.abs(ref))
+    assert err <= G.EMB_TOL["bf16"], f"{f.name}: embedding error {err:.3e}"
+
+
+def test_full_s2_edge_list_bit_exact(full):
+    f, trk = full
+    src, dst, rowptr, count = trk.stage_frnn(_dev(f.emb), _dev(f.hits), f.off)
+    osrc, odst, orow = f.cand
+    ec = int(count[0])
+    assert int(count[1]) == 0 and ec == len(osrc), (ec, len(osrc))
+    assert np.array_equal(src[:ec].cpu().numpy(), osrc) and np.array_equal(dst[:ec].cpu().numpy(), odst)
+    assert np.array_equal(rowptr.cpu().numpy(), orow)
+    deg = np.diff(orow)
+    assert deg.max() == f.cfg["frnn_k"], "the degree cap should bite at full size"
+    if len(f.off) > 2:                                       # batch == union of single events + offsets (configs[3])
+        ev_of = np.searchsorted(f.off, np.arange(f.n), side="right") - 1
+        assert np.all(ev_of[osrc] == ev_of[odst])
+        for b in (0, 9):
+            lo, hi = int(f.off[b]), int(f.off[b + 1])
+            s1, d1, _ = s2_frnn.frnn(f.emb[lo:hi], f.hits[lo:hi], np.array([0, hi - lo], np.int32), f.calib["frnn_radius"], f.cfg["frnn_k"])
+            a, z = f.event_edges(b)
+            assert np.array_equal(s1 + lo, osrc[a:z]) and np.array_equal(d1 + lo, odst[a:z])
+
+
+def test_full_s3_filter_scores_and_compaction(full):
+    f, trk = full
+    osrc, odst, _ = f.cand
+    src, dst = _dev(osrc), _dev(odst)
+    score = trk.stage_filter(_dev(f.emb), src, dst)
+    gpu = score.cpu().numpy()
+    assert np.all(np.isfinite(gpu))
+    cut = np.float32(f.calib["filter_cut"])
+    keys = G.edge_keys(osrc, odst)
+    if f.name == "pileup200":
+        ref = f.filter_full["all"]
+        G.check_scores(gpu, ref, "bf16", "filter score (all edges)")
+        ks, kd, count = trk.stage_compact(src, dst, score)
+        ek = int(count[0])
+        flips = G.check_kept(G.edge_keys(ks[:ek].cpu().numpy(), kd[:ek].cpu().numpy()), keys[f.kept], keys, ref, float(cut), "bf16",
+                             "filter kept set")
+        print(f"{f.name}: {flips} kept-set differences, all inside the 2e-2 band")
+    else:
+        idx, ref = f.filter_sample
+        G.check_scores(gpu[idx], ref, "bf16", f"filter score ({len(idx)} sampled edges)")
+        for b, sc in f.filter_full.items():
+            a, z = f.event_edges(b)
+            G.check_scores(gpu[a:z], sc, "bf16", f"filter score (event {b})")
+    # the compaction is exact for the scores it is given: stable, strict '>'
+    ks, kd, count = trk.stage_compact(src, dst, score)
+    ek = int(count[0])
+    m = gpu > cut
+    assert ek == int(m.sum()) and np.array_equal(ks[:ek].cpu().numpy(), osrc[m]) and np.array_equal(kd[:ek].cpu().numpy(), odst[m])
+
+
+def test_full_s4_gnn_scores_and_s5_labels(full):
+    f, trk = full
+    osrc, odst, _ = f.cand
+    ks, kd = osrc[f.kept], odst[f.kept]
+    assert 0.8 < len(ks) / (f.calib["n_kept_edges"] * f.n / f.calib["n_hits"]) < 1.25, "kept graph should have the config's size"
+    score = trk.stage_gnn(_dev(f.hits), _dev(ks), _dev(kd)).cpu().numpy()
+    assert np.all(np.isfinite(score))
+    worst = 0.0
+    full_ref = np.array(score, copy=True)           # oracle values where the oracle ran; the GPU's own elsewhere (S5 input only)
+    for b, (pos, ref) in f.gnn.items():
+        worst = max(worst, G.check_scores(score[pos], ref, "bf16", f"gnn score ({b})"))
+        full_ref[pos] = ref
+        frac = float(np.mean(ref > 0.5))
+        assert f.name != "pileup200" or 0.05 < frac < 0.95          # the centred bias was calibrated on this very graph
+    print(f"{f.name}: gnn max abs err {worst:.3e} over {sum(len(p) for p, _ in f.gnn.values())} edges")
+    # S5 on the scores above: labels bit-exact against the oracle's union-find
+    labels = trk.stage_cc(f.n, _dev(ks), _dev(kd), _dev(full_ref), f.cfg["gnn_cut"]).cpu().numpy()
+    assert np.array_equal(labels, s5_cc.connected_components(f.n, ks, kd, full_ref, f.cfg["gnn_cut"]))
+    assert len(np.unique(labels)) < f.n
+
+
+def test_full_infer_invariants(full):
+    """One trk_infer call at full size, as bench.py issues it: invariants of reading C-22."""
+    import torch
+    f, trk = full
+    res = trk.infer(_dev(f.hits), f.off, want_edges=True, want_cand=True)
+    torch.cuda.synchronize()
+    ec, ek, et, of = [int(v) for v in res["counts"].cpu().numpy()]
+    assert of == 0 and 0 < et < ek < ec
+    cs, cd, fs = (res[k][:ec].cpu().numpy() for k in ("cand_src", "cand_dst", "cand_score"))
+    es, ed, sc = (res[k][:ek].cpu().numpy() for k in ("edge_src", "edge_dst", "edge_score"))
+    assert np.all(np.diff(G.edge_keys(cs, cd)) > 0)
+    keep = fs > np.float32(f.calib["filter_cut"])
+    assert np.array_equal(es, cs[keep]) and np.array_equal(ed, cd[keep])
+    assert et == int(np.sum(sc > np.float32(f.cfg["gnn_cut"])))
+    ev_of = np.searchsorted(f.off, np.arange(f.n), side="right") - 1
+    assert np.all(ev_of[cs] == ev_of[cd])
+    assert np.array_equal(res["labels"].cpu().numpy(), s5_cc.connected_components(f.n, es, ed, sc, f.cfg["gnn_cut"]))
+    okeys = G.edge_keys(f.cand[0], f.cand[1])
+    gkeys = G.edge_keys(cs, cd)
+    jac = len(np.intersect1d(gkeys, okeys)) / len(np.union1d(gkeys, okeys))
+    print(f"{f.name}: E_c={ec} E_k={ek} E_t={et}; candidate-edge Jaccard vs oracle {jac:.4f}")
+    assert jac > 0.9
