@@ -16,6 +16,7 @@
 #include "gemm_tc.cuh"
 #include "gemm_tc2.cuh"
 #include "gnn_fused.cuh"
+#include "gnn_fused2.cuh"
 #include "graph.cuh"
 #include "nn.cuh"
 
@@ -157,8 +158,10 @@ trk_status launch_edge_fused(trk_ctx* ctx, const bf16* X, int64_t ldx, bf16* E, 
   if (rows.m_cap <= 0) return TRK_OK;
   static bool attr_set = false;
   auto kern = gf::gnn_edge_fused_kernel<MODE>;
+  auto kern2 = gf2::gnn_edge_fused2_kernel<MODE>;
   if (!attr_set) {
     TRK_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, gf::kSmemFused));
+    TRK_CUDA(ctx, cudaFuncSetAttribute(kern2, cudaFuncAttributeMaxDynamicSharedMemorySize, gf2::kSmemFused2));
     attr_set = true;
   }
   CUtensorMap tw1, tw2, te, test;
@@ -169,7 +172,11 @@ trk_status launch_edge_fused(trk_ctx* ctx, const bf16* X, int64_t ldx, bf16* E, 
   gf::FusedParams p{X, ldx, src, dst, L1.b_f32, L2.b_f32, ctx->cfg.gnn_layernorm, w_out, b_out, score};
   const int64_t ptiles = ceil_div(rows.m_cap, 2 * gf::kTileRows);
   const unsigned grid = 2u * (unsigned)std::min<int64_t>(ptiles, ctx->sm_count / 2);
-  TRK_LAUNCH(ctx, kern, grid, gf::kThreadsFused, gf::kSmemFused, st, tw1, tw2, te, test, rows, p);
+  if (debug_knob(kKnobGnnFused) >= 2) {
+    TRK_LAUNCH(ctx, kern2, grid, gf2::kThreads2, gf2::kSmemFused2, st, tw1, tw2, te, test, rows, p);
+  } else {
+    TRK_LAUNCH(ctx, kern, grid, gf::kThreadsFused, gf::kSmemFused, st, tw1, tw2, te, test, rows, p);
+  }
   return TRK_OK;
 }
 

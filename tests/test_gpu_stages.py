@@ -126,3 +126,19 @@ def test_end_to_end_invariants(case):
     res2 = trk.infer(_dev(ev["hits"]), ev["event_offsets"], want_edges=True)
     torch.cuda.synchronize()
     assert torch.equal(res2["labels"], res["labels"]) and torch.equal(res2["edge_score"][:ek], res["edge_score"][:ek])
+
+
+@pytest.mark.parametrize("variant", [0, 1, 2], ids=["layerwise", "fused_v1", "fused_v2"])
+def test_s4_kernel_variants_agree_with_the_oracle(variant):
+    """The three implementations of the S4 edge update (trk_debug_set 'gnn_fused') against the same oracle scores."""
+    from paper_2501_05520_b200 import debug_set
+    run = G.oracle_run("pileup50", "bf16", True, 600)
+    o = run["out"]
+    trk = G.make_trk(run)
+    try:
+        debug_set("gnn_fused", variant)
+        score = trk.stage_gnn(_dev(run["ev"]["hits"]), _dev(o["src"]), _dev(o["dst"])).cpu().numpy()
+        G.check_scores(score, o["gnn_score"], "bf16", f"gnn score (variant {variant})")
+    finally:
+        debug_set("gnn_fused", 2)
+        trk.close()
