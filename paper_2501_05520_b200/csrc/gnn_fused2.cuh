@@ -77,6 +77,15 @@ __device__ __forceinline__ bool mbar_test(uint64_t* bar, uint32_t parity) {
   return ok != 0;
 }
 
+// Arrive on an mbarrier of the pair's leader CTA with CTA-scope release (the form CUTLASS uses for its 2-SM pipelines).
+// What the leader's MMA issuer must see before it continues is either a finished TMEM read (ordered by
+// tcgen05.fence::before_thread_sync) or shared memory of the ARRIVING CTA that its own tensor core / TMA will read
+// (ordered by fence.proxy.async); neither needs the cluster-wide memory barrier of .release.cluster, which cost the
+// epilogue warps of version 1 several hundred cycles per arrive (stall_membar in profiles/r1_full_v2.md).
+__device__ __forceinline__ void mbar_arrive_remote(uint32_t cluster_addr) {
+  asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
+}
+
 __device__ __forceinline__ void tma_prefetch_l2_2d(const CUtensorMap* tmap, int c0, int c1) {
   asm volatile("cp.async.bulk.prefetch.tensor.2d.L2.global.tile [%0, {%1, %2}];" ::"l"(reinterpret_cast<uint64_t>(tmap)), "r"(c0), "r"(c1)
                : "memory");
@@ -125,6 +134,13 @@ __device__ __forceinline__ void row_stats(const float (&x)[kH], int use_ln, floa
   rstd = rsqrtf(((q0 + q1) + (q2 + q3)) * (1.f / kH) + 1e-5f);
 }
 
+#ifdef TRK_FUSED_PROF
+__device__ unsigned long long g_fused_prof[4][16][8];
+#define FPW(slot, stmt) do { long long _t0 = clock64(); stmt; pw[slot] += clock64() - _t0; } while (0)
+#else
+#define FPW(slot, stmt) stmt
+#endif
+
 template <int MODE>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads2, 1)
 gnn_edge_fused2_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constant__ CUtensorMap tmW2,
@@ -142,6 +158,10 @@ gnn_edge_fused2_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_co
   const int64_t M = resolve_rows(rows);
   const int64_t total = (M + 2 * kTileRows - 1) / (2 * kTileRows);
   const int n_my = total > pair ? (int)((total - pair + n_pairs - 1) / n_pairs) : 0;
+#ifdef TRK_FUSED_PROF
+  long long pw[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+  const long long t_begin = clock64();
+#endif
 
   if (warp == 0 && lane == 0) {
     prefetch_tmap(&tmW1); prefetch_tmap(&tmW2); prefetch_tmap(&tmE); prefetch_tmap(&tmEst);
@@ -195,7 +215,7 @@ gnn_edge_fused2_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_co
         const int64_t tile = pair + (int64_t)tl * n_pairs;
         const int b = tl & 1;
         const uint32_t ph = (tl >> 1) & 1;
-        mbar_wait(&bar->eempty[b], ph ^ 1);
+        FPW(0, mbar_wait(&bar->eempty[b], ph ^ 1));
         if (leader) mbar_arrive_expect_tx(&bar->efull[b], 2 * 2 * kKB);
         const uint32_t full_leader = mapa_u32(smem_u32(&bar->efull[b]), 0);
         const int row0 = (int)(tile * 2 * kTileRows + rank * kTileRows);
@@ -271,7 +291,7 @@ gnn_edge_fused2_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_co
       const int s_hi = row + 32 < M ? p.src[row + 32] : -1, d_hi = row + 32 < M ? p.dst[row + 32] : -1;
 #pragma unroll 1
       for (int h = 0; h < 2; ++h) {
-        mbar_wait(&bar->gempty[h], (uint32_t)(tl & 1) ^ 1);
+        FPW(h, mbar_wait(&bar->gempty[h], (uint32_t)(tl & 1) ^ 1));
         const int lo = h == 0 ? s_lo : d_lo, hi = h == 0 ? s_hi : d_hi;
 #pragma unroll 8
         for (int i = 0; i < 32; ++i) {
@@ -284,14 +304,14 @@ gnn_edge_fused2_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_co
         }
         cp_async_commit();
       }
-      cp_async_wait<1>();
+      FPW(2, cp_async_wait<1>());
       fence_proxy_async();
       __syncwarp();
-      if (lane == 0) mbar_arrive_cluster(gfull0);
-      cp_async_wait<0>();
+      if (lane == 0) mbar_arrive_remote(gfull0);
+      FPW(3, cp_async_wait<0>());
       fence_proxy_async();
       __syncwarp();
-      if (lane == 0) mbar_arrive_cluster(gfull1);
+      if (lane == 0) mbar_arrive_remote(gfull1);
     }
   } else if (warp < 8) {
     // ---------------------------------------------------------------- epilogue 1: acc1 -> LNR -> T (or score)
@@ -303,13 +323,13 @@ gnn_edge_fused2_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_co
       const int64_t tile = pair + (int64_t)tl * n_pairs;
       const int b = tl & 1;
       const uint32_t ph = (tl >> 1) & 1;
-      mbar_wait(&bar->a1full[b], ph);
+      FPW(0, mbar_wait(&bar->a1full[b], ph));
       tc_fence_after();
       float x[kH];
-      load_row(tmem_base + ((uint32_t)(quad * 32) << 16) + (uint32_t)(b * kH), sb1, x);
+      FPW(2, load_row(tmem_base + ((uint32_t)(quad * 32) << 16) + (uint32_t)(b * kH), sb1, x));
       tc_fence_before();
       __syncwarp();
-      if (lane == 0) mbar_arrive_cluster(b == 0 ? a1empty0 : a1empty1);     // the accumulator is in registers now
+      if (lane == 0) mbar_arrive_remote(b == 0 ? a1empty0 : a1empty1);     // the accumulator is in registers now
       float mean, rstd;
       row_stats(x, p.use_ln, mean, rstd);
       const float shift = -mean * rstd;
@@ -328,7 +348,7 @@ gnn_edge_fused2_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_co
         __syncwarp();
         if (lane == 0) mbar_arrive(&bar->eempty[b]);   // a1full: the layer-1 MMAs that read the e tile are complete
       } else {
-        mbar_wait(&bar->tempty, (uint32_t)(tl & 1) ^ 1);   // the layer-2 MMA of the previous tile has read T
+        FPW(1, mbar_wait(&bar->tempty, (uint32_t)(tl & 1) ^ 1));   // the layer-2 MMA of the previous tile has read T
 #pragma unroll
         for (int c = 0; c < kH; c += 8) {                  // 8 columns = one 16-byte chunk of the swizzled K block
           float f[8];
@@ -340,7 +360,7 @@ gnn_edge_fused2_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_co
         }
         fence_proxy_async();
         __syncwarp();
-        if (lane == 0) mbar_arrive_cluster(tfull_l);
+        if (lane == 0) mbar_arrive_remote(tfull_l);
       }
     }
   } else {
@@ -353,13 +373,13 @@ gnn_edge_fused2_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_co
         const int64_t tile = pair + (int64_t)tl * n_pairs;
         const int b = tl & 1;
         const uint32_t ph = (tl >> 1) & 1;
-        mbar_wait(&bar->a2full[b], ph);
+        FPW(0, mbar_wait(&bar->a2full[b], ph));
         tc_fence_after();
         float x[kH];
-        load_row(tmem_base + ((uint32_t)(quad * 32) << 16) + (uint32_t)(2 * kH + b * kH), sb2, x);
+        FPW(2, load_row(tmem_base + ((uint32_t)(quad * 32) << 16) + (uint32_t)(2 * kH + b * kH), sb2, x));
         tc_fence_before();
         __syncwarp();
-        if (lane == 0) mbar_arrive_cluster(b == 0 ? a2empty0 : a2empty1);
+        if (lane == 0) mbar_arrive_remote(b == 0 ? a2empty0 : a2empty1);
         float mean, rstd;
         row_stats(x, p.use_ln, mean, rstd);
         const float shift = -mean * rstd;
@@ -384,13 +404,19 @@ gnn_edge_fused2_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_co
           const int row0 = (int)(tile * 2 * kTileRows + rank * kTileRows + quad * 32);
           for (int kb = 0; kb < 2; ++kb) tma_store_2d(&tmEst, eh + kb * kKB + quad * 32 * 128, kb * 64, row0);
           bulk_commit();
-          bulk_wait_read<0>();          // the tile's rows have left shared memory: the buffer may be refilled
+          FPW(1, bulk_wait_read<0>());          // the tile's rows have left shared memory: the buffer may be refilled
           mbar_arrive(&bar->eempty[b]);
         }
       }
       if (lane == 0) bulk_wait_all();
     }
   }
+#ifdef TRK_FUSED_PROF
+  if (MODE == gf::kUpdate && blockIdx.x < 4 && lane == 0) {
+    for (int i = 0; i < 7; ++i) g_fused_prof[blockIdx.x][warp][i] = (unsigned long long)pw[i];
+    g_fused_prof[blockIdx.x][warp][7] = (unsigned long long)(clock64() - t_begin);
+  }
+#endif
   tc_fence_before();
   cluster_sync_all();
   if (warp == 1) {

@@ -472,6 +472,13 @@ trk_status gnn_forward_bf16(trk_ctx* ctx, const float* hits, int64_t n, const in
   return TRK_OK;
 }
 
+#ifdef TRK_FUSED_PROF
+// per-role wait cycles of the fused edge kernel (profiling builds only: TRK_NVCC_EXTRA=-DTRK_FUSED_PROF)
+extern "C" int trk_debug_fused_prof(unsigned long long* host) {
+  return (int)cudaMemcpyFromSymbol(host, gf2::g_fused_prof, sizeof(gf2::g_fused_prof));
+}
+#endif
+
 // ---------------------------------------------------------------- test hook
 trk_status gemm_bf16_hook(trk_ctx* ctx, const void* a, const void* w, const float* bias, void* out, int64_t m, int n, int k, int relu,
                           cudaStream_t st) {
