@@ -20,5 +20,5 @@ parity unpinned: the end-to-end physics quality of the whole pipeline (trained w
 and the paper's events are not available).  Every stage function
 is pinned on its own.
 """
-from . import s1_embed, s2_frnn, s3_filter, s4_gnn, s5_cc  # noqa: F401
+from . import s1_embed, s2_frnn, s3_filter, s4_gnn, s5_cc, s6_tracks  # noqa: F401
 from .mlp import layernorm, linear, mlp_forward, sigmoid  # noqa: F401
