@@ -2,7 +2,9 @@
  *
  * One call runs the five stages of PAPER.md line 85 (section 2.2.2) on the device:
  *   S1 embedding MLP -> S2 fixed-radius graph in the latent space -> S3 filter MLP + cut ->
- *   S4 interaction-network GNN edge scores -> S5 weakly-connected components (track labels).
+ *   S4 interaction-network GNN edge scores -> S5 weakly-connected components (track labels),
+ * and, when asked for, S6: the track candidates as lists of hits (line 85: "Each track candidate is
+ * a list of spacepoints").
  * The lifecycle mirrors the paper's backend: "loading the full
  * pipeline, performing inference, and setting the GPU device ID" == trk_create / trk_infer /
  * trk_destroy, with constants preloaded once and intermediates kept on the device (lines 77, 115).
@@ -92,6 +94,9 @@ typedef struct {
   int64_t max_events;
   int64_t max_cand_edges;       /* S2 output capacity; max_hits*frnn_k can never overflow           */
   int64_t max_kept_edges;       /* S3 output capacity (data dependent)                              */
+  /* S6: a track candidate is a component with at least min_track_hits hits (values < 1 mean 1;
+   * the paper states no minimum, reading C-23).  Used only when track outputs are wanted. */
+  int32_t min_track_hits;
 } trk_config;
 
 typedef struct {
@@ -116,6 +121,13 @@ typedef struct {
   float* cand_score;            /* [cand_capacity] S3 sigmoid scores                                */
   int64_t cand_capacity;
   float* embedding;             /* [N][d_e] S1 output                                               */
+  /* S6 (all three or none): tracks ordered by label (= their smallest hit index), the hits of a track
+   * in ascending hit index.  If there are more than track_capacity tracks the first track_capacity
+   * are written and counts[3] is set.                                                              */
+  int32_t* track_offsets;       /* [track_capacity+1]; track t = track_hits[offsets[t] .. offsets[t+1]) */
+  int32_t* track_hits;          /* [N]; entries beyond the last track are -1                         */
+  int32_t* track_counts;        /* [2] = {number of tracks T, hits in tracks = track_offsets[T]}      */
+  int64_t track_capacity;
 } trk_result;
 
 trk_status trk_create(const trk_config* cfg, trk_ctx** out);
@@ -127,6 +139,13 @@ trk_status trk_destroy(trk_ctx* ctx);
  * pointers are non-NULL, counts[4]) D2H and synchronises.  hits_host/labels_host should be pinned. */
 trk_status trk_infer_host(trk_ctx* ctx, int32_t n_events, const int32_t* event_offsets,
                           const float* hits_host, int32_t* labels_host, int32_t* counts_host);
+
+/* The same request returning the track candidates themselves: additionally copies
+ * track_offsets_host[T+1] and track_hits_host[track_offsets[T]] D2H; both must hold N+1 / N entries.
+ * counts_host is [6] = counts[4] followed by {T, hits in tracks}.  labels_host may be NULL.          */
+trk_status trk_infer_host_tracks(trk_ctx* ctx, int32_t n_events, const int32_t* event_offsets, const float* hits_host,
+                                 int32_t* labels_host, int32_t* track_offsets_host, int32_t* track_hits_host,
+                                 int32_t* counts_host);
 
 const char* trk_status_string(trk_status s);
 const char* trk_last_error(const trk_ctx* ctx); /* ctx may be NULL: error of the last failed trk_create */
@@ -172,6 +191,11 @@ trk_status trk_stage_gnn(trk_ctx* ctx, const float* hits, int64_t n, const int32
 /* S5: labels int32 [n]; edges with score > cut are kept. */
 trk_status trk_stage_cc(trk_ctx* ctx, int64_t n, const int32_t* src, const int32_t* dst, const float* score,
                         int64_t n_edges, float cut, int32_t* labels, void* cuda_stream);
+
+/* S6: track lists from labels [n] (as S5 writes them: label = smallest hit index of the component).
+ * track_offsets [capacity+1], track_hits [n], track_counts [3] = {T, hits in tracks, overflow}.    */
+trk_status trk_stage_tracks(trk_ctx* ctx, const int32_t* labels, int64_t n, int32_t min_hits, int32_t* track_offsets,
+                            int64_t capacity, int32_t* track_hits, int32_t* track_counts, void* cuda_stream);
 
 /* Kernel hook for tests/bench: out = act(A W^T + bias) through the ctx-independent tcgen05 GEMM.
  * A DEVICE bf16 [m][k] (k % 64 == 0), W DEVICE bf16 [n][k] (n % 16 == 0, n <= 1024 ... see DESIGN.md),

@@ -20,7 +20,7 @@ EXPORTS = [
     "trk_create", "trk_infer", "trk_destroy", "trk_infer_host", "trk_status_string", "trk_last_error",
     "trk_workspace_bytes", "trk_last_launch_count", "trk_stage_embed", "trk_stage_frnn", "trk_stage_filter",
     "trk_stage_compact", "trk_stage_gnn", "trk_stage_cc", "trk_gemm_bf16", "trk_profile_enable", "trk_profile_stage_ms", "trk_profile_kernel_ms",
-    "trk_debug_set",
+    "trk_debug_set", "trk_stage_tracks", "trk_infer_host_tracks",
 ]
 
 _f32p = C.POINTER(C.c_float)
@@ -41,6 +41,7 @@ class TrkConfig(C.Structure):
         ("node_enc", TrkMlp), ("edge_enc", TrkMlp), ("edge_net", TrkMlp), ("node_net", TrkMlp), ("edge_dec", TrkMlp),
         ("gnn_cut", C.c_float),
         ("max_hits", C.c_int64), ("max_events", C.c_int64), ("max_cand_edges", C.c_int64), ("max_kept_edges", C.c_int64),
+        ("min_track_hits", C.c_int32),
     ]
 
 
@@ -54,6 +55,7 @@ class TrkResult(C.Structure):
         ("edge_src", C.c_void_p), ("edge_dst", C.c_void_p), ("edge_score", C.c_void_p), ("edge_capacity", C.c_int64),
         ("cand_src", C.c_void_p), ("cand_dst", C.c_void_p), ("cand_score", C.c_void_p), ("cand_capacity", C.c_int64),
         ("embedding", C.c_void_p),
+        ("track_offsets", C.c_void_p), ("track_hits", C.c_void_p), ("track_counts", C.c_void_p), ("track_capacity", C.c_int64),
     ]
 
 
@@ -93,6 +95,8 @@ def lib():
     L.trk_debug_set.argtypes = [C.c_char_p, i64]
     L.trk_profile_stage_ms.argtypes = [vp, _f32p]
     L.trk_profile_kernel_ms.argtypes = [vp, _f32p, i32, _i32p, C.POINTER(i64)]
+    L.trk_stage_tracks.argtypes = [vp, vp, i64, i32, vp, i64, vp, vp, vp]
+    L.trk_infer_host_tracks.argtypes = [vp, i32, _i32p, vp, vp, vp, vp, vp]
     for name in EXPORTS:
         if getattr(L, name).restype is C.c_int:
             getattr(L, name).restype = C.c_int
@@ -132,7 +136,7 @@ class Trk:
 
     def __init__(self, *, model, precision, frnn_radius, frnn_k, filter_input, filter_cut, gnn_hidden, gnn_iters, gnn_cut,
                  max_hits, max_events=1, max_cand_edges=None, max_kept_edges=None, gnn_layernorm=True, grid_proj=None,
-                 grid_dims=None, device=0):
+                 grid_dims=None, device=0, min_track_hits=3):
         L = lib()
         keep = []
         cfg = TrkConfig()
@@ -162,6 +166,7 @@ class Trk:
         cfg.max_events = int(max_events)
         cfg.max_cand_edges = int(max_cand_edges if max_cand_edges is not None else max_hits * frnn_k)
         cfg.max_kept_edges = int(max_kept_edges if max_kept_edges is not None else cfg.max_cand_edges)
+        cfg.min_track_hits = int(min_track_hits)
         self.cfg = cfg
         self.d_e = d_e
         self.device = device
@@ -212,7 +217,8 @@ class Trk:
         return [float(ms[i]) for i in range(n.value)], int(rows.value)
 
     # ---- the call
-    def infer(self, hits, event_offsets, *, want_edges=False, want_cand=False, want_embedding=False, out=None, stream=None):
+    def infer(self, hits, event_offsets, *, want_edges=False, want_cand=False, want_embedding=False, want_tracks=False, out=None,
+              stream=None):
         """hits: CUDA fp32 [N,3]; event_offsets: host int32 [B+1].  Returns dict of CUDA tensors (no sync)."""
         import torch
         off = np.ascontiguousarray(event_offsets, dtype=np.int32)
@@ -234,6 +240,10 @@ class Trk:
                 o["cand_score"] = torch.empty(cap, dtype=torch.float32, device=dev)
             if want_embedding:
                 o["embedding"] = torch.empty(n, self.d_e, dtype=torch.float32, device=dev)
+            if want_tracks:
+                o["track_offsets"] = torch.zeros(max(n, 1) + 1, dtype=torch.int32, device=dev)
+                o["track_hits"] = torch.empty(n, dtype=torch.int32, device=dev)
+                o["track_counts"] = torch.zeros(2, dtype=torch.int32, device=dev)
         b = TrkBatch(len(off) - 1, off.ctypes.data_as(_i32p), _ptr(hits))
         r = TrkResult()
         r.labels, r.counts = _ptr(o["labels"]), _ptr(o["counts"])
@@ -242,6 +252,8 @@ class Trk:
         r.cand_src, r.cand_dst, r.cand_score = _ptr(o.get("cand_src")), _ptr(o.get("cand_dst")), _ptr(o.get("cand_score"))
         r.cand_capacity = o["cand_src"].numel() if "cand_src" in o else 0
         r.embedding = _ptr(o.get("embedding"))
+        r.track_offsets, r.track_hits, r.track_counts = _ptr(o.get("track_offsets")), _ptr(o.get("track_hits")), _ptr(o.get("track_counts"))
+        r.track_capacity = o["track_offsets"].numel() - 1 if "track_offsets" in o else 0
         self._check(lib().trk_infer(self._h, C.byref(b), C.byref(r), _stream_ptr(stream)))
         return o
 
@@ -258,6 +270,22 @@ class Trk:
             return C.c_void_p(a.data_ptr() if hasattr(a, "data_ptr") else a.ctypes.data)
         self._check(lib().trk_infer_host(self._h, len(off) - 1, off.ctypes.data_as(_i32p), hp(hits_host), hp(labels_host), hp(counts_host)))
         return labels_host, counts_host
+
+    def infer_host_tracks(self, hits_host, event_offsets, labels_host=None):
+        """HOST hits in, HOST track candidates out: (track_offsets [T+1], track_hits, labels, counts [6])."""
+        off = np.ascontiguousarray(event_offsets, dtype=np.int32)
+        n = int(off[-1])
+        if labels_host is None:
+            labels_host = np.empty(n, dtype=np.int32)
+        toff = np.zeros(n + 1, dtype=np.int32)
+        thit = np.empty(n, dtype=np.int32)
+        counts = np.zeros(6, dtype=np.int32)
+
+        def hp(a):
+            return C.c_void_p(a.data_ptr() if hasattr(a, "data_ptr") else a.ctypes.data)
+        self._check(lib().trk_infer_host_tracks(self._h, len(off) - 1, off.ctypes.data_as(_i32p), hp(hits_host), hp(labels_host), hp(toff),
+                                                hp(thit), hp(counts)))
+        return toff[:counts[4] + 1], thit[:counts[5]], labels_host, counts
 
     # ---- stage hooks (device tensors in, device tensors out, enqueued on the current stream)
     def stage_embed(self, hits, stream=None):
@@ -311,6 +339,19 @@ class Trk:
         self._check(lib().trk_stage_cc(self._h, n, _ptr(src), _ptr(dst), _ptr(score), src.numel(), float(cut), _ptr(labels),
                                        _stream_ptr(stream)))
         return labels
+
+
+    def stage_tracks(self, labels, min_hits, capacity=None, stream=None):
+        """labels CUDA int32 [n] -> (track_offsets [capacity+1], track_hits [n], track_counts [3] = {T, hits, overflow})."""
+        import torch
+        n = labels.numel()
+        cap = int(capacity if capacity is not None else max(n, 1))
+        toff = torch.zeros(cap + 1, dtype=torch.int32, device=labels.device)
+        thit = torch.empty(n, dtype=torch.int32, device=labels.device)
+        cnt = torch.zeros(3, dtype=torch.int32, device=labels.device)
+        self._check(lib().trk_stage_tracks(self._h, _ptr(labels), n, int(min_hits), _ptr(toff), cap, _ptr(thit), _ptr(cnt),
+                                           _stream_ptr(stream)))
+        return toff, thit, cnt
 
 
 def debug_set(key: str, value: int) -> None:

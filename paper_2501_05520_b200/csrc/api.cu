@@ -140,7 +140,7 @@ void carve(trk_ctx* c, Carver& k) {
   k.take(&c->slots, N * f.frnn_k);
   k.take(&c->deg, N + 2);
   k.take(&c->rowptr, N + 2);
-  const size_t scan_n = std::max(std::max(EC, (size_t)c->max_cells + 1), std::max(N + 2, EK));
+  const size_t scan_n = std::max(std::max(EC, (size_t)c->max_cells + 1), std::max(N + 1024, EK));
   k.take(&c->scan_tmp, scan_n / 2048 + 4);
   k.take(&c->cand_src, EC);
   k.take(&c->cand_dst, EC);
@@ -160,9 +160,14 @@ void carve(trk_ctx* c, Carver& k) {
   k.take(&c->in_fill, N + 2);
   k.take(&c->out_rowptr, N + 2);
   k.take(&c->parent, N);
+  for (int32_t** t : {&c->tk_a, &c->tk_b, &c->tk_c, &c->tk_d, &c->tk_e, &c->tk_f, &c->tk_g}) k.take(t, N + 2);
+  k.take(&c->tk_hist, (N + 255) / 256 * 256 + 2);
+  k.take(&c->tk_hist_scan, (N + 255) / 256 * 256 + 2);
   k.take(&c->io_hits, N * 3);
   k.take(&c->io_labels, N);
-  k.take(&c->io_counts, 4);
+  k.take(&c->io_counts, 8);
+  k.take(&c->io_track_offsets, N + 1);
+  k.take(&c->io_track_hits, N);
 }
 
 __global__ void finalize_counts_kernel(const int32_t* __restrict__ counts, int64_t edge_cap, int64_t cand_cap, int32_t* __restrict__ out) {
@@ -404,6 +409,9 @@ trk_status trk_infer(trk_ctx* ctx, const trk_batch* batch, const trk_result* res
     return fail(ctx, TRK_ERR_INVALID_ARG, "edge outputs requested with edge_capacity <= 0");
   if ((res->cand_src || res->cand_dst || res->cand_score) && res->cand_capacity <= 0)
     return fail(ctx, TRK_ERR_INVALID_ARG, "candidate outputs requested with cand_capacity <= 0");
+  const bool want_t = res->track_offsets || res->track_hits || res->track_counts;
+  if (want_t && (!res->track_offsets || !res->track_hits || !res->track_counts || res->track_capacity <= 0))
+    return fail(ctx, TRK_ERR_INVALID_ARG, "track outputs need track_offsets, track_hits, track_counts and track_capacity > 0");
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const trk_config& f = ctx->cfg;
   ctx->launch_count = 0;
@@ -433,6 +441,9 @@ trk_status trk_infer(trk_ctx* ctx, const trk_batch* batch, const trk_result* res
                       &ctx->counts[2], st));
     TRK_MARK(5);
     ctx->prof_valid = prof;
+    if (want_t)
+      TRK_TRY(build_tracks(ctx, res->labels, n, f.min_track_hits, res->track_offsets, res->track_capacity, res->track_hits,
+                           res->track_counts, &ctx->counts[3], st));
     if (res->embedding) TRK_CUDA(ctx, cudaMemcpyAsync(res->embedding, ctx->emb, (size_t)n * ctx->d_e * 4, cudaMemcpyDeviceToDevice, st));
     const size_t ne = (size_t)std::min<int64_t>(res->edge_capacity, kept_cap), nc = (size_t)std::min<int64_t>(res->cand_capacity, cand_cap);
     if (res->edge_src) TRK_CUDA(ctx, cudaMemcpyAsync(res->edge_src, ctx->kept_src, ne * 4, cudaMemcpyDeviceToDevice, st));
@@ -442,6 +453,7 @@ trk_status trk_infer(trk_ctx* ctx, const trk_batch* batch, const trk_result* res
     if (res->cand_dst) TRK_CUDA(ctx, cudaMemcpyAsync(res->cand_dst, ctx->cand_dst, nc * 4, cudaMemcpyDeviceToDevice, st));
     if (res->cand_score) TRK_CUDA(ctx, cudaMemcpyAsync(res->cand_score, ctx->cand_score, nc * 4, cudaMemcpyDeviceToDevice, st));
   }
+  if (n <= 0 && want_t) TRK_TRY(build_tracks(ctx, nullptr, 0, 1, res->track_offsets, res->track_capacity, res->track_hits, res->track_counts, nullptr, st));
   const bool want_e = res->edge_src || res->edge_dst || res->edge_score, want_c = res->cand_src || res->cand_dst || res->cand_score;
   TRK_LAUNCH(ctx, finalize_counts_kernel, 1, 32, 0, st, ctx->counts, want_e ? res->edge_capacity : (int64_t)-1,
              want_c ? res->cand_capacity : (int64_t)-1, res->counts);
@@ -464,6 +476,36 @@ trk_status trk_infer_host(trk_ctx* ctx, int32_t n_events, const int32_t* event_o
   TRK_TRY(trk_infer(ctx, &b, &r, st));
   if (n > 0) TRK_CUDA(ctx, cudaMemcpyAsync(labels_host, ctx->io_labels, (size_t)n * 4, cudaMemcpyDeviceToHost, st));
   if (counts_host) TRK_CUDA(ctx, cudaMemcpyAsync(counts_host, ctx->io_counts, 16, cudaMemcpyDeviceToHost, st));
+  TRK_CUDA(ctx, cudaStreamSynchronize(st));
+  return TRK_OK;
+}
+
+trk_status trk_infer_host_tracks(trk_ctx* ctx, int32_t n_events, const int32_t* event_offsets, const float* hits_host,
+                                 int32_t* labels_host, int32_t* track_offsets_host, int32_t* track_hits_host, int32_t* counts_host) {
+  if (!ctx) return TRK_ERR_INVALID_ARG;
+  int64_t n = 0;
+  TRK_TRY(check_batch(ctx, n_events, event_offsets, &n));
+  if (!track_offsets_host || !counts_host || (n > 0 && (!hits_host || !track_hits_host)))
+    return fail(ctx, TRK_ERR_INVALID_ARG, "infer_host_tracks: a required host pointer is NULL");
+  cudaStream_t st = ctx->own_stream;
+  if (n > 0) TRK_CUDA(ctx, cudaMemcpyAsync(ctx->io_hits, hits_host, (size_t)n * 12, cudaMemcpyHostToDevice, st));
+  trk_batch b{n_events, event_offsets, ctx->io_hits};
+  trk_result r;
+  std::memset(&r, 0, sizeof(r));
+  r.labels = ctx->io_labels;
+  r.counts = ctx->io_counts;
+  r.track_offsets = ctx->io_track_offsets;
+  r.track_hits = ctx->io_track_hits;
+  r.track_counts = ctx->io_counts + 4;
+  r.track_capacity = std::max<int64_t>(n, 1);
+  TRK_TRY(trk_infer(ctx, &b, &r, st));
+  if (n > 0 && labels_host) TRK_CUDA(ctx, cudaMemcpyAsync(labels_host, ctx->io_labels, (size_t)n * 4, cudaMemcpyDeviceToHost, st));
+  TRK_CUDA(ctx, cudaMemcpyAsync(counts_host, ctx->io_counts, 24, cudaMemcpyDeviceToHost, st));
+  TRK_CUDA(ctx, cudaStreamSynchronize(st));
+  // the sizes are known now: copy exactly the T+1 offsets and the hits of the tracks
+  const int64_t T = counts_host[4], nh = counts_host[5];
+  TRK_CUDA(ctx, cudaMemcpyAsync(track_offsets_host, ctx->io_track_offsets, (size_t)(T + 1) * 4, cudaMemcpyDeviceToHost, st));
+  if (nh > 0) TRK_CUDA(ctx, cudaMemcpyAsync(track_hits_host, ctx->io_track_hits, (size_t)nh * 4, cudaMemcpyDeviceToHost, st));
   TRK_CUDA(ctx, cudaStreamSynchronize(st));
   return TRK_OK;
 }
@@ -564,6 +606,17 @@ trk_status trk_stage_cc(trk_ctx* ctx, int64_t n, const int32_t* src, const int32
     return fail(ctx, TRK_ERR_INVALID_ARG, "stage_cc: bad arguments");
   if (n > ctx->cfg.max_hits) return fail(ctx, TRK_ERR_CAPACITY, "stage_cc: n exceeds max_hits");
   return cc_labels(ctx, n, src, dst, score, nullptr, n_edges, cut, labels, nullptr, (cudaStream_t)cuda_stream);
+}
+
+trk_status trk_stage_tracks(trk_ctx* ctx, const int32_t* labels, int64_t n, int32_t min_hits, int32_t* track_offsets, int64_t capacity,
+                            int32_t* track_hits, int32_t* track_counts, void* cuda_stream) {
+  if (!ctx) return TRK_ERR_INVALID_ARG;
+  if (n < 0 || capacity <= 0 || !track_offsets || !track_counts || (n > 0 && (!labels || !track_hits)))
+    return fail(ctx, TRK_ERR_INVALID_ARG, "stage_tracks: bad arguments");
+  if (n > ctx->cfg.max_hits) return fail(ctx, TRK_ERR_CAPACITY, "stage_tracks: n exceeds max_hits");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  TRK_TRY(fill_i32(ctx, track_counts, 0, 3, st));
+  return build_tracks(ctx, labels, n, min_hits, track_offsets, capacity, track_hits, track_counts, track_counts + 2, st);
 }
 
 trk_status trk_debug_set(const char* key, int64_t value) {

@@ -127,10 +127,16 @@ struct trk_ctx {
   int32_t* out_rowptr = nullptr;    // [max_hits+1] CSR by src (edges are src-sorted)
   // S5
   int32_t* parent = nullptr;        // [max_hits]
+  // S6 (tracks.cu): sizes / flags / scans and the (key, value) ping-pong of the radix sort, [max_hits+2] each
+  int32_t *tk_a = nullptr, *tk_b = nullptr, *tk_c = nullptr, *tk_d = nullptr, *tk_e = nullptr, *tk_f = nullptr, *tk_g = nullptr;
+  int32_t* tk_hist = nullptr;       // [256 * ceil(max_hits/256) + 2] digit-major block histograms
+  int32_t* tk_hist_scan = nullptr;
   // trk_infer_host staging (device side)
   float* io_hits = nullptr;         // [max_hits][3]
   int32_t* io_labels = nullptr;     // [max_hits]
-  int32_t* io_counts = nullptr;     // [4]
+  int32_t* io_counts = nullptr;     // [8]: counts[4], then {n_tracks, n_track_hits}
+  int32_t* io_track_offsets = nullptr;  // [max_hits+1]
+  int32_t* io_track_hits = nullptr;     // [max_hits]
 };
 
 namespace trk {
@@ -184,5 +190,9 @@ trk_status cc_labels(trk_ctx* ctx, int64_t n, const int32_t* src, const int32_t*
                      const int32_t* n_edges_dev, int64_t n_edges_cap, float cut, int32_t* labels, int32_t* pass_count,
                      cudaStream_t st);
 
+// ---- tracks.cu ----
+// track_offsets [capacity+1], track_hits [n] (entries beyond the last track are -1), track_counts [2] = {T, hits in tracks}
+trk_status build_tracks(trk_ctx* ctx, const int32_t* labels, int64_t n, int min_hits, int32_t* track_offsets, int64_t capacity,
+                        int32_t* track_hits, int32_t* track_counts, int32_t* overflow_flag, cudaStream_t st);
 
 }  // namespace trk
