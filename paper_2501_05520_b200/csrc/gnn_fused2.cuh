@@ -6,7 +6,7 @@
 // Same data flow as gnn_fused.cuh (weights resident in shared memory and split by output row between the two CTAs of a
 // pair, e tile by TMA, endpoint h rows gathered by cp.async into the swizzled UMMA layout, layer-1 accumulator -> LayerNorm
 // -> bf16 tile T in shared memory -> layer-2 MMA -> LayerNorm + residual in place -> TMA store; nothing intermediate
-// touches HBM).  What changed, from the per-role wait profile of version 1 (profiles/r1_fused_v2_roles.md): the two
+// touches HBM).  What changed, from the per-role wait profile of version 1 (same method as profiles/r1_fused_roles_v3.md): the two
 // LayerNorm epilogues were latency-bound single warps (two TMEM passes, 128-long dependent FMA chains, ~7 k cycles per tile
 // each) and the e-tile loads came cold from HBM behind them.  Here
 //   * an epilogue thread reads its whole 128-column accumulator row from TMEM in one go (4 loads, one wait), releases the
