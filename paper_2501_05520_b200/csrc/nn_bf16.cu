@@ -17,6 +17,7 @@
 #include "gemm_tc2.cuh"
 #include "gnn_fused.cuh"
 #include "gnn_fused2.cuh"
+#include "gnn_fused3.cuh"
 #include "graph.cuh"
 #include "nn.cuh"
 
@@ -159,7 +160,9 @@ trk_status launch_edge_fused(trk_ctx* ctx, const bf16* X, int64_t ldx, bf16* E, 
   static bool attr_set = false;
   auto kern = gf::gnn_edge_fused_kernel<MODE>;
   auto kern2 = gf2::gnn_edge_fused2_kernel<MODE>;
+  auto kern3 = gf3::gnn_edge_fused3_kernel<MODE>;
   if (!attr_set) {
+    TRK_CUDA(ctx, cudaFuncSetAttribute(kern3, cudaFuncAttributeMaxDynamicSharedMemorySize, gf3::kSmemFused3));
     TRK_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, gf::kSmemFused));
     TRK_CUDA(ctx, cudaFuncSetAttribute(kern2, cudaFuncAttributeMaxDynamicSharedMemorySize, gf2::kSmemFused2));
     attr_set = true;
@@ -172,7 +175,9 @@ trk_status launch_edge_fused(trk_ctx* ctx, const bf16* X, int64_t ldx, bf16* E, 
   gf::FusedParams p{X, ldx, src, dst, L1.b_f32, L2.b_f32, ctx->cfg.gnn_layernorm, w_out, b_out, score};
   const int64_t ptiles = ceil_div(rows.m_cap, 2 * gf::kTileRows);
   const unsigned grid = 2u * (unsigned)std::min<int64_t>(ptiles, ctx->sm_count / 2);
-  if (debug_knob(kKnobGnnFused) >= 2) {
+  if (debug_knob(kKnobGnnFused) >= 3) {
+    TRK_LAUNCH(ctx, kern3, grid, gf3::kThreads3, gf3::kSmemFused3, st, tw1, tw2, te, test, rows, p);
+  } else if (debug_knob(kKnobGnnFused) >= 2) {
     TRK_LAUNCH(ctx, kern2, grid, gf2::kThreads2, gf2::kSmemFused2, st, tw1, tw2, te, test, rows, p);
   } else {
     TRK_LAUNCH(ctx, kern, grid, gf::kThreadsFused, gf::kSmemFused, st, tw1, tw2, te, test, rows, p);
