@@ -206,9 +206,12 @@ trk_status trk_gemm_bf16(const void* a, const void* w, const float* bias, void* 
 /* Tuning / test knob, process wide: selects between kernel variants that compute the same result.
  *   "gemm_pair"  1 (default): dense layers with >= 128 output columns run on CTA pairs (tcgen05.mma.cta_group::2,
  *                256-row tiles); 0: single-CTA 128-row tiles.
- *   "gnn_fused"  2 (default): with gnn_hidden == 128 the S4 edge update and the decoder run as one fused CTA-pair kernel
+ *   "gnn_fused"  2: with gnn_hidden == 128 the S4 edge update and the decoder run as one fused CTA-pair kernel
  *                per iteration (gathered endpoint rows, both layers, LayerNorm, residual; gnn_fused2.cuh); 1: the first
  *                version of that kernel (gnn_fused.cuh); 0: layer-by-layer GEMM launches.
+ *                3 (default): its third version (gnn_fused3.cuh) -- see that value's description in DESIGN.md section 6.
+ *   "epi_split"  1 (default): bf16-output layers with 256-column tiles and a single 64-wide K block (the first layer of the S3
+ *                filter MLP) run their epilogue on eight warps (two per TMEM lane quadrant); 0: four warps.
  * Returns TRK_ERR_INVALID_ARG for an unknown key.  Not thread safe against running trk_* calls. */
 trk_status trk_debug_set(const char* key, int64_t value);
 

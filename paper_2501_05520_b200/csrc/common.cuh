@@ -168,7 +168,7 @@ trk_status fail(trk_ctx* ctx, trk_status s, const std::string& msg);
 inline int64_t ceil_div(int64_t a, int64_t b) { return (a + b - 1) / b; }
 
 // ---- tuning / test knobs (trk_debug_set) ----
-enum { kKnobGemmPair = 0, kKnobGnnFused = 1, kKnobCount = 8 };
+enum { kKnobGemmPair = 0, kKnobGnnFused = 1, kKnobEpiSplit = 2, kKnobCount = 8 };
 int64_t debug_knob(int which);
 
 // ---- util_kernels.cu ----

@@ -154,11 +154,16 @@ __host__ __device__ constexpr uint32_t make_idesc(int bn) {
 
 constexpr int tmem_cols_for(int bn) { return 2 * bn <= 32 ? 32 : (2 * bn <= 64 ? 64 : (2 * bn <= 128 ? 128 : (2 * bn <= 256 ? 256 : 512))); }
 constexpr int stage_bytes(int bn) { return (BM + bn) * BK * 2; }
-constexpr int num_stages(int bn) { return (196 * 1024) / stage_bytes(bn) > 8 ? 8 : (196 * 1024) / stage_bytes(bn); }
 constexpr int kStoreStage = 2 * 32 * 128;   // per epilogue warp: two 32-row x 128-byte boxes (TMA-store staging)
-constexpr int smem_bytes(int bn, bool tma_store = false) {
-  return num_stages(bn) * stage_bytes(bn) + (tma_store ? kEpiWarps * kStoreStage : 0) + 1024 /*alignment*/ + 256 /*barriers*/;
+// SPLIT = 2 doubles the epilogue warps (two per TMEM lane quadrant, each taking half of the tile's columns): for layers whose
+// K loop is one block long the epilogue, not the tensor pipe, paces a tile.  Their staging takes the room of one ring stage.
+constexpr int num_stages(int bn, int split = 1) {
+  return ((196 - 32 * (split - 1)) * 1024) / stage_bytes(bn) > 8 ? 8 : ((196 - 32 * (split - 1)) * 1024) / stage_bytes(bn);
 }
+constexpr int smem_bytes(int bn, bool tma_store = false, int split = 1) {
+  return num_stages(bn, split) * stage_bytes(bn) + (tma_store ? split * kEpiWarps * kStoreStage : 0) + 1024 /*alignment*/ + 256 /*barriers*/;
+}
+constexpr int threads_for(int split) { return 64 + 32 * kEpiWarps * split; }
 
 // What an epilogue may use besides its own parameters: a per-warp staging area and the output tensor map.
 struct EpiShared {
@@ -171,18 +176,19 @@ struct EpiShared {
 // Epi::run(params, tmem_tile_addr (lane and column base of this warp's quadrant), row0 (first row of the
 //          tile), col0 (first column of the tile), n_blk, rows M, lane-row index r, release()) must call
 //          `release` exactly once after its last TMEM read.
-template <int BN, class Epi>
-__global__ void __launch_bounds__(kThreads, 1)
+template <int BN, class Epi, int SPLIT = 1>
+__global__ void __launch_bounds__(threads_for(SPLIT), 1)
 gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, const __grid_constant__ CUtensorMap tmC,
                Rows rows, int n_tiles, int k_blocks, typename Epi::Params ep) {
-  constexpr int STAGES = num_stages(BN);
+  constexpr int STAGES = num_stages(BN, SPLIT);
   constexpr int A_BYTES = BM * BK * 2;
   constexpr int STAGE = stage_bytes(BN);
   constexpr int TMEM_COLS = tmem_cols_for(BN);
+  static_assert(SPLIT == 1 || (SPLIT == 2 && BN % 128 == 0), "column split of the epilogue");
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
   uint8_t* store_stage = smem + STAGES * STAGE;
-  uint64_t* full_bar = reinterpret_cast<uint64_t*>(store_stage + (Epi::kTmaStore ? kEpiWarps * kStoreStage : 0));
+  uint64_t* full_bar = reinterpret_cast<uint64_t*>(store_stage + (Epi::kTmaStore ? SPLIT * kEpiWarps * kStoreStage : 0));
   uint64_t* empty_bar = full_bar + STAGES;
   uint64_t* tfull_bar = empty_bar + STAGES;
   uint64_t* tempty_bar = tfull_bar + 2;
@@ -201,7 +207,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     }
     for (int s = 0; s < 2; ++s) {
       mbar_init(&tfull_bar[s], 1);
-      mbar_init(&tempty_bar[s], kEpiWarps);
+      mbar_init(&tempty_bar[s], kEpiWarps * SPLIT);
     }
     fence_barrier_init();
   }
@@ -256,6 +262,8 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     }
   } else {
     const int quad = warp & 3;   // TMEM lane quadrant this warp may access
+    const int chalf = (warp - 2) >> 2;   // SPLIT == 2: which half of the tile's columns
+    constexpr int BNE = BN / SPLIT;
     int as = 0;
     uint32_t aphase = 0;
     EpiShared es{store_stage + (warp - 2) * kStoreStage, &tmC, 0u};
@@ -263,14 +271,14 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
       const int m_blk = (int)(tile / n_tiles), n_blk = (int)(tile % n_tiles);
       mbar_wait(&tfull_bar[as], aphase);
       tc_fence_after();
-      const uint32_t taddr = tmem_base + ((uint32_t)(quad * 32) << 16) + (uint32_t)(as * BN);
+      const uint32_t taddr = tmem_base + ((uint32_t)(quad * 32) << 16) + (uint32_t)(as * BN + chalf * BNE);
       uint64_t* rel = &tempty_bar[as];
       auto release = [&]() {
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(rel);
       };
-      Epi::template run<BN>(ep, taddr, (int64_t)m_blk * BM + quad * 32 + lane, n_blk * BN, n_blk, M, release, es);
+      Epi::template run<BNE>(ep, taddr, (int64_t)m_blk * BM + quad * 32 + lane, n_blk * BN + chalf * BNE, n_blk, M, release, es);
       if (++as == 2) { as = 0; aphase ^= 1; }
     }
     if (Epi::kTmaStore && lane == 0) bulk_wait_all();   // staged boxes must be read before the CTA's shared memory goes away

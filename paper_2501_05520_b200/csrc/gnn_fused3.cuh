@@ -132,6 +132,10 @@ gnn_edge_fused3_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_co
   const int64_t M = resolve_rows(rows);
   const int64_t total = (M + 2 * kTileRows - 1) / (2 * kTileRows);
   const int n_my = total > pair ? (int)((total - pair + n_pairs - 1) / n_pairs) : 0;
+#ifdef TRK_FUSED_PROF
+  long long pw[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+  const long long t_begin = clock64();
+#endif
 
   if (warp == 0 && lane == 0) {
     prefetch_tmap(&tmW1); prefetch_tmap(&tmW2); prefetch_tmap(&tmE); prefetch_tmap(&tmEst);
@@ -279,7 +283,7 @@ gnn_edge_fused3_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_co
       const int s_hi = row + 32 < M ? p.src[row + 32] : 0, d_hi = row + 32 < M ? p.dst[row + 32] : 0;
 #pragma unroll 1
       for (int h = 0; h < 2; ++h) {
-        mbar_wait(&bar->gempty[h], (uint32_t)(tl & 1) ^ 1);
+        FPW(h, mbar_wait(&bar->gempty[h], (uint32_t)(tl & 1) ^ 1));
         const int lo = h == 0 ? s_lo : d_lo, hi = h == 0 ? s_hi : d_hi;
         const uint32_t dsth = dst0 + h * 2 * kKB;
 #pragma unroll
@@ -289,11 +293,11 @@ gnn_edge_fused3_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_co
         }
         cp_async_commit();
       }
-      cp_async_wait<1>();
+      FPW(2, cp_async_wait<1>());
       fence_proxy_async();
       __syncwarp();
       if (lane == 0) mbar_arrive_remote(gfull0);
-      cp_async_wait<0>();
+      FPW(3, cp_async_wait<0>());
       fence_proxy_async();
       __syncwarp();
       if (lane == 0) mbar_arrive_remote(gfull1);
@@ -308,10 +312,10 @@ gnn_edge_fused3_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_co
       const int64_t tile = pair + (int64_t)tl * n_pairs;
       const int b = tl & 1;
       const uint32_t ph = (tl >> 1) & 1;
-      mbar_wait(&bar->a1full[b], ph);
+      FPW(0, mbar_wait(&bar->a1full[b], ph));
       tc_fence_after();
       float2 x[kH / 2];
-      load_row2(tmem_base + ((uint32_t)(quad * 32) << 16) + (uint32_t)(b * kH), sb1, x);
+      FPW(2, load_row2(tmem_base + ((uint32_t)(quad * 32) << 16) + (uint32_t)(b * kH), sb1, x));
       tc_fence_before();
       __syncwarp();
       if (lane == 0) mbar_arrive_remote(b == 0 ? a1empty0 : a1empty1);     // the accumulator is in registers now
@@ -331,7 +335,7 @@ gnn_edge_fused3_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_co
         const int64_t row = tile * 2 * kTileRows + rank * kTileRows + r;
         if (row < M) p.score[row] = fast_sigmoid((d0.x + d0.y) + (d1.x + d1.y));
       } else {
-        mbar_wait(&bar->tempty, (uint32_t)(tl & 1) ^ 1);   // the layer-2 MMA of the previous tile has read T
+        FPW(1, mbar_wait(&bar->tempty, (uint32_t)(tl & 1) ^ 1));   // the layer-2 MMA of the previous tile has read T
 #pragma unroll
         for (int c = 0; c < kH; c += 8) {                  // 8 columns = one 16-byte chunk of the swizzled K block
           uint32_t w[4];
@@ -359,17 +363,17 @@ gnn_edge_fused3_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_co
         const int64_t tile = pair + (int64_t)tl * n_pairs;
         const int b = tl & 1;
         const uint32_t ph = (tl >> 1) & 1;
-        mbar_wait(&bar->a2full[b], ph);
+        FPW(0, mbar_wait(&bar->a2full[b], ph));
         tc_fence_after();
         float2 x[kH / 2];
-        load_row2(tmem_base + ((uint32_t)(quad * 32) << 16) + (uint32_t)(2 * kH + b * kH), sb2, x);
+        FPW(2, load_row2(tmem_base + ((uint32_t)(quad * 32) << 16) + (uint32_t)(2 * kH + b * kH), sb2, x));
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive_remote(b == 0 ? a2empty0 : a2empty1);
         float mean, rstd;
         row_stats2(x, p.use_ln, mean, rstd);
         const float2 rs = f2(rstd, rstd), sh = f2(-mean * rstd, -mean * rstd);
-        mbar_wait(&bar->resfull, (uint32_t)(tl & 1));        // the residual copy of this tile has landed
+        FPW(3, mbar_wait(&bar->resfull, (uint32_t)(tl & 1)));      // the residual copy of this tile has landed
 #pragma unroll
         for (int c = 0; c < kH; c += 8) {
           const int kb = c >> 6, ch = (c & 63) >> 3;
@@ -393,13 +397,19 @@ gnn_edge_fused3_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_co
           const int row0 = (int)(tile * 2 * kTileRows + rank * kTileRows + quad * 32);
           for (int kb = 0; kb < 2; ++kb) tma_store_2d(&tmEst, res + kb * kKB + quad * 32 * 128, kb * 64, row0);
           bulk_commit();
-          bulk_wait_read<0>();          // the tile's rows have left shared memory: the buffer may be refilled
+          FPW(1, bulk_wait_read<0>());  // the tile's rows have left shared memory: the buffer may be refilled
           mbar_arrive(&bar->resempty);
         }
       }
       if (lane == 0) bulk_wait_all();
     }
   }
+#ifdef TRK_FUSED_PROF
+  if (MODE == gf::kUpdate && blockIdx.x < 4 && lane == 0) {
+    for (int i = 0; i < 7; ++i) gf2::g_fused_prof[blockIdx.x][warp][i] = (unsigned long long)pw[i];
+    gf2::g_fused_prof[blockIdx.x][warp][7] = (unsigned long long)(clock64() - t_begin);
+  }
+#endif
   tc_fence_before();
   cluster_sync_all();
   if (warp == 1) {

@@ -107,6 +107,19 @@ trk_status launch_gemm(trk_ctx* ctx, const bf16* A, int64_t a_rows, int64_t lda,
   }
   const int64_t tiles = ceil_div(rows.m_cap, tc::BM) * n_tiles;
   const unsigned grid = (unsigned)std::min<int64_t>(tiles, ctx->sm_count);
+  if constexpr (BN == 256 && Epi::kTmaStore) {
+    // a single K block per tile: the bf16-store epilogue paces the kernel, so it gets eight warps (column split)
+    if (K == tc::BK && debug_knob(kKnobEpiSplit) != 0) {
+      static bool attr3_set = false;
+      auto kern3 = tc::gemm_tc_kernel<BN, Epi, 2>;
+      if (!attr3_set) {
+        TRK_CUDA(ctx, cudaFuncSetAttribute(kern3, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::smem_bytes(BN, true, 2)));
+        attr3_set = true;
+      }
+      TRK_LAUNCH(ctx, kern3, grid, tc::threads_for(2), tc::smem_bytes(BN, true, 2), st, ta, tb, tc_out, rows, n_tiles, K / tc::BK, ep);
+      return TRK_OK;
+    }
+  }
   TRK_LAUNCH(ctx, kern, grid, tc::kThreads, tc::smem_bytes(BN, Epi::kTmaStore), st, ta, tb, tc_out, rows, n_tiles, K / tc::BK, ep);
   return TRK_OK;
 }
