@@ -137,6 +137,7 @@ void carve(trk_ctx* c, Carver& k) {
   k.take(&c->cell_fill, (size_t)c->max_cells + 1);
   k.take(&c->semb, N * c->d_e_pad);
   k.take(&c->smeta, N);
+  k.take(&c->sproj, N);
   k.take(&c->slots, N * f.frnn_k);
   k.take(&c->deg, N + 2);
   k.take(&c->rowptr, N + 2);
@@ -350,6 +351,18 @@ trk_status trk_create(const trk_config* cfg, trk_ctx** out) {
       const double sc = nn > 0 ? std::min(1.0, 1.0 / std::sqrt(nn)) * (1.0 - 1e-6) : 0.0;
       for (int k = 0; k < d_e; ++k) P[k * 3 + a] = (float)(P[k * 3 + a] * sc);
     }
+    // ||P^T v||^2 <= lambda ||v||^2 with lambda = largest eigenvalue of P^T P <= max absolute row sum (Gershgorin)
+    double gain = 0.0;
+    for (int a = 0; a < 3; ++a) {
+      double rowsum = 0.0;
+      for (int b = 0; b < 3; ++b) {
+        double g = 0.0;
+        for (int k = 0; k < d_e; ++k) g += (double)P[k * 3 + a] * P[k * 3 + b];
+        rowsum += std::fabs(g);
+      }
+      gain = std::max(gain, rowsum);
+    }
+    ctx->proj_gain = (float)std::max(gain * (1.0 + 1e-6), 1e-12);
     if (cudaMalloc(&ctx->grid_proj, P.size() * 4) != cudaSuccess ||
         cudaMemcpy(ctx->grid_proj, P.data(), P.size() * 4, cudaMemcpyHostToDevice) != cudaSuccess)
       return bail(fail(ctx, TRK_ERR_OOM, "grid_proj upload failed"));

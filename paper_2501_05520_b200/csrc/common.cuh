@@ -101,6 +101,8 @@ struct trk_ctx {
   int32_t* cell_fill = nullptr;     // [max_cells]
   float* semb = nullptr;            // [max_hits][d_e_pad] sorted by cell
   float4* smeta = nullptr;          // [max_hits] (r, |z|, idx bits, cell bits)
+  float4* sproj = nullptr;          // [max_hits] binning coordinates P^T e, sorted by cell
+  float proj_gain = 1.f;            // >= largest eigenvalue of P^T P (Gershgorin), 1 without a projection
   int32_t* slots = nullptr;         // [max_hits][K]
   int32_t* deg = nullptr;           // [max_hits+1]
   int32_t* rowptr = nullptr;        // [max_hits+1]

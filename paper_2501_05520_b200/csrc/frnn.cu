@@ -12,6 +12,8 @@
 // One warp serves one query: lanes stride over the candidates, accepted ones are appended to a
 // shared-memory buffer via ballot, and a warp bitonic sort on (d2, j) prunes to the K nearest
 // whenever the buffer fills; a final sort on j gives the (src, dst) output order.
+#include <cmath>
+
 #include "common.cuh"
 
 namespace trk {
@@ -117,13 +119,14 @@ __global__ void frnn_count_kernel(const float* __restrict__ proj, const int32_t*
 __global__ void frnn_scatter_kernel(const float* __restrict__ emb, const float* __restrict__ hits, int d_e, int d_pad,
                                     const int32_t* __restrict__ cell_of_hit, const int32_t* __restrict__ cell_start,
                                     int32_t* __restrict__ cell_fill, float* __restrict__ semb, float4* __restrict__ smeta,
-                                    int64_t n) {
+                                    const float* __restrict__ proj, float4* __restrict__ sproj, int64_t n) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   const int cell = cell_of_hit[i];
   const int pos = cell_start[cell] + atomicAdd(&cell_fill[cell], 1);
   for (int k = 0; k < d_pad; ++k) semb[(int64_t)pos * d_pad + k] = k < d_e ? emb[i * d_e + k] : 0.f;
   smeta[pos] = make_float4(hits[i * 3 + 0], fabsf(hits[i * 3 + 2]), __int_as_float((int)i), __int_as_float(cell));
+  sproj[pos] = make_float4(proj[i * 3 + 0], proj[i * 3 + 1], proj[i * 3 + 2], 0.f);
 }
 
 // ---- warp-level bitonic sort of n (power of two) entries held in shared memory ----
@@ -152,27 +155,33 @@ __device__ __forceinline__ void warp_bitonic(unsigned long long* d2, int* idx, i
 constexpr unsigned long long kInfBits = 0x7ff0000000000000ull;
 constexpr int kWarpsPerBlock = 4;
 
-// Two-level test per candidate.  Level 1 (all candidates, fp32 with FMA): d2f <= r2 (1 + 1e-4).  The fp32 value differs
+// Three-level test per candidate.  Level 0 (all candidates, 16 bytes and 6 flops each): the squared distance of the
+// binning coordinates P^T e (the same fp32 values the grid was built from) against lambda r^2 with slack, lambda >= the
+// largest eigenvalue of P^T P (1 for orthonormal P), so no pair with d2 <= r2 can fail it; a ball inside the 27 cells keeps
+// ~15 % of them.  Survivors are queued and, 32 at a time, take level 1 (fp32 with FMA, all d_e coordinates): d2f <= r2 (1 + 1e-4).  The fp32 value differs
 // from the exact d2 by at most ~16 ulp relative (all terms are non-negative, so there is no cancellation), so no candidate
 // with d2 <= r2 can fail it.  Survivors (a few per cent) are queued in shared memory and, 32 at a time, take level 2: the
 // outer() test and the exact fp64 d2 (no FMA) that decides acceptance and rank -- the same arithmetic as before, so the
 // edge list is unchanged; only the work on the ~97 % of candidates that are nowhere near the radius is cheaper.
 template <int D4, int CAP>
 __global__ void __launch_bounds__(kWarpsPerBlock * 32)
-frnn_search_kernel(const float* __restrict__ semb, const float4* __restrict__ smeta, const int32_t* __restrict__ cell_start,
-                   const GridParams* __restrict__ gpp, double r2, float r2_loose, int K, int32_t* __restrict__ slots,
-                   int32_t* __restrict__ deg, int64_t n) {
+frnn_search_kernel(const float* __restrict__ semb, const float4* __restrict__ smeta, const float4* __restrict__ sproj,
+                   const int32_t* __restrict__ cell_start, const GridParams* __restrict__ gpp, double r2, float r2_loose,
+                   float r2_proj, int K, int32_t* __restrict__ slots, int32_t* __restrict__ deg, int64_t n) {
   constexpr int D = D4 * 4;
   __shared__ unsigned long long s_d2[kWarpsPerBlock][CAP];
   __shared__ int s_idx[kWarpsPerBlock][CAP];
   __shared__ int s_queue[kWarpsPerBlock][64];
+  __shared__ int s_queue0[kWarpsPerBlock][64];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int64_t q = (int64_t)blockIdx.x * kWarpsPerBlock + warp;
   if (q >= n) return;
   unsigned long long* bd2 = s_d2[warp];
   int* bidx = s_idx[warp];
   int* queue = s_queue[warp];
+  int* queue0 = s_queue0[warp];
   const GridParams gp = *gpp;
+  const float4 qp = sproj[q];
 
   const float4 qm = smeta[q];
   const float q_r = qm.x, q_az = qm.y;
@@ -192,6 +201,7 @@ frnn_search_kernel(const float* __restrict__ semb, const float4* __restrict__ sm
 
   int count = 0;  // warp-uniform number of buffered neighbours
   int qn = 0;     // warp-uniform number of queued level-1 survivors
+  int qn0 = 0;    // warp-uniform number of queued level-0 survivors
   for (int t = lane; t < CAP; t += 32) { bd2[t] = kInfBits; bidx[t] = 0x7fffffff; }
   __syncwarp();
 
@@ -245,42 +255,74 @@ frnn_search_kernel(const float* __restrict__ semb, const float4* __restrict__ sm
     __syncwarp();
   };
 
-  const int x0 = max(cx - 1, 0), x1 = min(cx + 1, gp.dims[0] - 1);
-  for (int dz = -1; dz <= 1; ++dz) {
-    const int z = cz + dz;
-    if (z < 0 || z >= gp.dims[2]) continue;
-    for (int dy = -1; dy <= 1; ++dy) {
-      const int y = cy + dy;
-      if (y < 0 || y >= gp.dims[1]) continue;
-      const int row = ev * gp.cells_per_event + (z * gp.dims[1] + y) * gp.dims[0];
-      const int lo = cell_start[row + x0], hi = cell_start[row + x1 + 1];
-      for (int base = lo; base < hi; base += 32) {
-        const int pos = base + lane;
-        bool pre = false;
-        if (pos < hi) {
-          const float4* ce = reinterpret_cast<const float4*>(semb + (int64_t)pos * D);
-          float d2f = 0.f;
+  // level 1 on the first min(qn0, 32) queued level-0 survivors
+  auto drain0 = [&]() {
+    const int take = min(qn0, 32);
+    bool pre = false;
+    int pos = 0;
+    if (lane < take) {
+      pos = queue0[lane];
+      const float4* ce = reinterpret_cast<const float4*>(semb + (int64_t)pos * D);
+      float d2f = 0.f;
 #pragma unroll
-          for (int k4 = 0; k4 < D4; ++k4) {
-            const float4 v = __ldg(ce + k4);
-            float t;
-            t = qf[k4 * 4 + 0] - v.x; d2f = fmaf(t, t, d2f);
-            t = qf[k4 * 4 + 1] - v.y; d2f = fmaf(t, t, d2f);
-            t = qf[k4 * 4 + 2] - v.z; d2f = fmaf(t, t, d2f);
-            t = qf[k4 * 4 + 3] - v.w; d2f = fmaf(t, t, d2f);
-          }
-          pre = d2f <= r2_loose;
-        }
-        const unsigned m = __ballot_sync(0xffffffffu, pre);
-        if (m) {
-          if (pre) queue[qn + __popc(m & ((1u << lane) - 1u))] = pos;
-          qn += __popc(m);
-          __syncwarp();
-          if (qn >= 32) drain();
-        }
+      for (int k4 = 0; k4 < D4; ++k4) {
+        const float4 v = __ldg(ce + k4);
+        float t;
+        t = qf[k4 * 4 + 0] - v.x; d2f = fmaf(t, t, d2f);
+        t = qf[k4 * 4 + 1] - v.y; d2f = fmaf(t, t, d2f);
+        t = qf[k4 * 4 + 2] - v.z; d2f = fmaf(t, t, d2f);
+        t = qf[k4 * 4 + 3] - v.w; d2f = fmaf(t, t, d2f);
+      }
+      pre = d2f <= r2_loose;
+    }
+    __syncwarp();
+    if (qn0 > 32 && lane < qn0 - 32) {   // keep the tail of the queue
+      const int moved = queue0[32 + lane];
+      queue0[lane] = moved;
+    }
+    qn0 -= take;
+    const unsigned m = __ballot_sync(0xffffffffu, pre);
+    if (m) {
+      if (pre) queue[qn + __popc(m & ((1u << lane) - 1u))] = pos;
+      qn += __popc(m);
+      __syncwarp();
+      if (qn >= 32) drain();
+    }
+    __syncwarp();
+  };
+
+  // the (up to) nine rows of three x-adjacent cells: lane r < 9 fetches the candidate range of row r, so the nine dependent
+  // cell_start look-ups cost one memory latency instead of nine
+  const int x0 = max(cx - 1, 0), x1 = min(cx + 1, gp.dims[0] - 1);
+  int my_lo = 0, my_hi = 0;
+  if (lane < 9) {
+    const int z = cz + lane / 3 - 1, y = cy + lane % 3 - 1;
+    if (z >= 0 && z < gp.dims[2] && y >= 0 && y < gp.dims[1]) {
+      const int row = ev * gp.cells_per_event + (z * gp.dims[1] + y) * gp.dims[0];
+      my_lo = cell_start[row + x0];
+      my_hi = cell_start[row + x1 + 1];
+    }
+  }
+  for (int rr = 0; rr < 9; ++rr) {
+    const int lo = __shfl_sync(0xffffffffu, my_lo, rr), hi = __shfl_sync(0xffffffffu, my_hi, rr);
+    for (int base = lo; base < hi; base += 32) {
+      const int pos = base + lane;
+      bool pre = false;
+      if (pos < hi) {
+        const float4 cp = __ldg(sproj + pos);
+        const float tx = qp.x - cp.x, ty = qp.y - cp.y, tz = qp.z - cp.z;
+        pre = fmaf(tz, tz, fmaf(ty, ty, tx * tx)) <= r2_proj;
+      }
+      const unsigned m = __ballot_sync(0xffffffffu, pre);
+      if (m) {
+        if (pre) queue0[qn0 + __popc(m & ((1u << lane) - 1u))] = pos;
+        qn0 += __popc(m);
+        __syncwarp();
+        if (qn0 >= 32) drain0();
       }
     }
   }
+  while (qn0 > 0) drain0();
   while (qn > 0) drain();
   if (count > K) {
     warp_bitonic(bd2, bidx, CAP, false, lane);
@@ -337,19 +379,22 @@ __global__ void event_of_hit_kernel(const __grid_constant__ EventOffsets offs, i
 
 template <int D4>
 trk_status launch_search(trk_ctx* ctx, int K, double r2, int64_t n, cudaStream_t st) {
+  // level-0 threshold on the binning coordinates: (sqrt(lambda) r with the slack of the grid's cell edge)^2
+  const double r0 = std::sqrt((double)ctx->proj_gain) * (double)ctx->cfg.frnn_radius * 1.001 + 2e-5;
+  const float r2_proj = r0 * r0 >= 3.0e38 ? __builtin_inff() : nextafterf((float)(r0 * r0), __builtin_inff());
   const unsigned blocks = (unsigned)ceil_div(n, kWarpsPerBlock);
   // level-1 threshold: r^2 (1 + 1e-4) rounded up, infinite when r^2 overflows fp32 (then every candidate takes level 2)
   const double loose = r2 * (1.0 + 1e-4);
   const float r2_loose = loose >= 3.0e38 ? __builtin_inff() : fmaxf(nextafterf((float)loose, __builtin_inff()), 1e-30f);
   if (K <= 32) {
-    TRK_LAUNCH(ctx, (frnn_search_kernel<D4, 64>), blocks, kWarpsPerBlock * 32, 0, st, ctx->semb, ctx->smeta, ctx->cell_start,
-               ctx->grid, r2, r2_loose, K, ctx->slots, ctx->deg, n);
+    TRK_LAUNCH(ctx, (frnn_search_kernel<D4, 64>), blocks, kWarpsPerBlock * 32, 0, st, ctx->semb, ctx->smeta, ctx->sproj, ctx->cell_start,
+               ctx->grid, r2, r2_loose, r2_proj, K, ctx->slots, ctx->deg, n);
   } else if (K <= 64) {
-    TRK_LAUNCH(ctx, (frnn_search_kernel<D4, 128>), blocks, kWarpsPerBlock * 32, 0, st, ctx->semb, ctx->smeta, ctx->cell_start,
-               ctx->grid, r2, r2_loose, K, ctx->slots, ctx->deg, n);
+    TRK_LAUNCH(ctx, (frnn_search_kernel<D4, 128>), blocks, kWarpsPerBlock * 32, 0, st, ctx->semb, ctx->smeta, ctx->sproj, ctx->cell_start,
+               ctx->grid, r2, r2_loose, r2_proj, K, ctx->slots, ctx->deg, n);
   } else {
-    TRK_LAUNCH(ctx, (frnn_search_kernel<D4, 256>), blocks, kWarpsPerBlock * 32, 0, st, ctx->semb, ctx->smeta, ctx->cell_start,
-               ctx->grid, r2, r2_loose, K, ctx->slots, ctx->deg, n);
+    TRK_LAUNCH(ctx, (frnn_search_kernel<D4, 256>), blocks, kWarpsPerBlock * 32, 0, st, ctx->semb, ctx->smeta, ctx->sproj, ctx->cell_start,
+               ctx->grid, r2, r2_loose, r2_proj, K, ctx->slots, ctx->deg, n);
   }
   return TRK_OK;
 }
@@ -375,7 +420,7 @@ trk_status frnn_build(trk_ctx* ctx, const float* emb, const float* hits, int64_t
   TRK_TRY(exclusive_scan_i32(ctx, ctx->cell_count, ctx->cell_start, n_cells, ctx->scan_tmp, st));
   TRK_TRY(fill_i32(ctx, ctx->cell_fill, 0, n_cells, st));
   TRK_LAUNCH(ctx, frnn_scatter_kernel, nb, 256, 0, st, emb, hits, ctx->d_e, ctx->d_e_pad, ctx->cell_of_hit, ctx->cell_start,
-             ctx->cell_fill, ctx->semb, ctx->smeta, n);
+             ctx->cell_fill, ctx->semb, ctx->smeta, ctx->proj, ctx->sproj, n);
   const double r = (double)ctx->cfg.frnn_radius;
   const double r2 = r * r;
   switch (ctx->d_e_pad / 4) {
