@@ -324,7 +324,12 @@ trk_status trk_create(const trk_config* cfg, trk_ctx** out) {
   ctx->filter_u = u;
   ctx->H = H;
   ctx->grid_dims = cfg->grid_dims;
-  ctx->grid_max = cfg->max_events * 32768ll <= kMaxCells ? 32 : (cfg->max_events * 4096ll <= kMaxCells ? 16 : 8);
+  // cells per axis and event: the finest grid whose cell table fits (the cell edge never goes below r, so a finer bound only
+  // helps: candidates per query fall with the cell volume until the edge reaches r)
+  ctx->grid_max = 8;
+  for (int g : {128, 64, 32, 16})
+    if (cfg->max_events * (int64_t)g * g * g <= kMaxCells) { ctx->grid_max = g; break; }
+  if (const char* e = std::getenv("TRK_GRID_MAX")) ctx->grid_max = std::max(1, std::min(128, std::atoi(e)));   // tuning knob
   ctx->max_cells = (int64_t)cfg->max_events * ctx->grid_max * ctx->grid_max * ctx->grid_max;
 
   trk_status s = TRK_OK;

@@ -69,7 +69,7 @@ struct trk_ctx {
   trk::DevMlp embed, filter, node_enc, edge_enc, edge_net, node_net, edge_dec;
   float* grid_proj = nullptr;       // [d_e_pad][3] device
   int grid_dims = 3;
-  int grid_max = 32;                // cells per axis and event (32, 16 or 8 by max_events)
+  int grid_max = 32;                // upper bound of cells per axis and event (128 .. 8 by max_events)
 
   // stacked bf16 weights of the split first layers (bf16 mode): [2H][H] = [W1[:, :H] ; W1[:, H:2H]]
   __nv_bfloat16* edge_net_wab = nullptr;

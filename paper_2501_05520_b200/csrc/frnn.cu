@@ -166,8 +166,8 @@ constexpr int kWarpsPerBlock = 4;
 template <int D4, int CAP>
 __global__ void __launch_bounds__(kWarpsPerBlock * 32)
 frnn_search_kernel(const float* __restrict__ semb, const float4* __restrict__ smeta, const float4* __restrict__ sproj,
-                   const int32_t* __restrict__ cell_start, const GridParams* __restrict__ gpp, double r2, float r2_loose,
-                   float r2_proj, int K, int32_t* __restrict__ slots, int32_t* __restrict__ deg, int64_t n) {
+                   const int32_t* __restrict__ cell_start, const GridParams* __restrict__ gpp, double r2_in, float r2_loose_in,
+                   float r2_proj_in, float proj_scale, int K, int32_t* __restrict__ slots, int32_t* __restrict__ deg, int64_t n) {
   constexpr int D = D4 * 4;
   __shared__ unsigned long long s_d2[kWarpsPerBlock][CAP];
   __shared__ int s_idx[kWarpsPerBlock][CAP];
@@ -202,6 +202,19 @@ frnn_search_kernel(const float* __restrict__ semb, const float4* __restrict__ sm
   int count = 0;  // warp-uniform number of buffered neighbours
   int qn = 0;     // warp-uniform number of queued level-1 survivors
   int qn0 = 0;    // warp-uniform number of queued level-0 survivors
+  // Thresholds shrink once K neighbours are known: after a prune the K-th smallest d2 so far bounds every later accept
+  // (a candidate with a larger d2 can never enter the K nearest; equal d2 is kept and settled by the (d2, j) order).
+  double r2 = r2_in;
+  float r2_loose = r2_loose_in, r2_proj = r2_proj_in;
+  auto tighten = [&]() {
+    const double kth = __longlong_as_double((long long)bd2[K - 1]);
+    if (kth < r2) {
+      r2 = kth;
+      r2_loose = fminf(r2_loose, __double2float_ru(kth * (1.0 + 1e-4)));
+      const float r0 = proj_scale * __double2float_ru(sqrt(kth)) + 2e-5f;
+      r2_proj = fminf(r2_proj, __fmul_ru(r0, r0));
+    }
+  };
   for (int t = lane; t < CAP; t += 32) { bd2[t] = kInfBits; bidx[t] = 0x7fffffff; }
   __syncwarp();
 
@@ -241,6 +254,8 @@ frnn_search_kernel(const float* __restrict__ semb, const float4* __restrict__ sm
     if (m) {
       if (count + 32 > CAP) {  // make room: keep the K nearest so far
         warp_bitonic(bd2, bidx, CAP, false, lane);
+        if (count >= K) tighten();
+        __syncwarp();
         for (int t = K + lane; t < CAP; t += 32) { bd2[t] = kInfBits; bidx[t] = 0x7fffffff; }
         __syncwarp();
         count = min(count, K);
@@ -330,11 +345,13 @@ frnn_search_kernel(const float* __restrict__ semb, const float4* __restrict__ sm
     __syncwarp();
     count = K;
   }
-  // order the kept neighbours by index; unused entries hold INT_MAX and sort to the end
-  int nsort = 32;
-  while (nsort < count) nsort <<= 1;
-  warp_bitonic(bd2, bidx, nsort, true, lane);
-  for (int t = lane; t < count; t += 32) slots[(int64_t)q_i * K + t] = bidx[t];
+  // order the kept neighbours by index: the indices are distinct, so the rank of one is the number of smaller ones
+  for (int t = lane; t < count; t += 32) {
+    const int mine = bidx[t];
+    int rank = 0;
+    for (int u = 0; u < count; ++u) rank += bidx[u] < mine ? 1 : 0;
+    slots[(int64_t)q_i * K + rank] = mine;
+  }
   if (lane == 0) deg[q_i] = count;
 }
 
@@ -382,19 +399,20 @@ trk_status launch_search(trk_ctx* ctx, int K, double r2, int64_t n, cudaStream_t
   // level-0 threshold on the binning coordinates: (sqrt(lambda) r with the slack of the grid's cell edge)^2
   const double r0 = std::sqrt((double)ctx->proj_gain) * (double)ctx->cfg.frnn_radius * 1.001 + 2e-5;
   const float r2_proj = r0 * r0 >= 3.0e38 ? __builtin_inff() : nextafterf((float)(r0 * r0), __builtin_inff());
+  const float proj_scale = nextafterf((float)(std::sqrt((double)ctx->proj_gain) * 1.001), __builtin_inff());
   const unsigned blocks = (unsigned)ceil_div(n, kWarpsPerBlock);
   // level-1 threshold: r^2 (1 + 1e-4) rounded up, infinite when r^2 overflows fp32 (then every candidate takes level 2)
   const double loose = r2 * (1.0 + 1e-4);
   const float r2_loose = loose >= 3.0e38 ? __builtin_inff() : fmaxf(nextafterf((float)loose, __builtin_inff()), 1e-30f);
   if (K <= 32) {
     TRK_LAUNCH(ctx, (frnn_search_kernel<D4, 64>), blocks, kWarpsPerBlock * 32, 0, st, ctx->semb, ctx->smeta, ctx->sproj, ctx->cell_start,
-               ctx->grid, r2, r2_loose, r2_proj, K, ctx->slots, ctx->deg, n);
+               ctx->grid, r2, r2_loose, r2_proj, proj_scale, K, ctx->slots, ctx->deg, n);
   } else if (K <= 64) {
     TRK_LAUNCH(ctx, (frnn_search_kernel<D4, 128>), blocks, kWarpsPerBlock * 32, 0, st, ctx->semb, ctx->smeta, ctx->sproj, ctx->cell_start,
-               ctx->grid, r2, r2_loose, r2_proj, K, ctx->slots, ctx->deg, n);
+               ctx->grid, r2, r2_loose, r2_proj, proj_scale, K, ctx->slots, ctx->deg, n);
   } else {
     TRK_LAUNCH(ctx, (frnn_search_kernel<D4, 256>), blocks, kWarpsPerBlock * 32, 0, st, ctx->semb, ctx->smeta, ctx->sproj, ctx->cell_start,
-               ctx->grid, r2, r2_loose, r2_proj, K, ctx->slots, ctx->deg, n);
+               ctx->grid, r2, r2_loose, r2_proj, proj_scale, K, ctx->slots, ctx->deg, n);
   }
   return TRK_OK;
 }
