@@ -2,6 +2,11 @@
 //
 //   e_k <- e_k + LNR(W2 LNR(W1 [h_src(k) ; h_dst(k) ; e_k] + b1) + b2)           (kUpdate)
 //   score_k = sigmoid(w_out . LNR(W1 [h_src ; h_dst ; e_k] + b1) + b_out)        (kDecode)
+//   h_v <- h_v + LNR(W2 LNR(W1 [h_v ; m_in_v ; m_out_v] + b1) + b2)              (kNode: the node update, rows of X)
+//
+// kNode runs the same pipeline on the node table X [n][3H] = (h | m_in | m_out): all six K blocks of the operand come by
+// TMA (h takes the place of the e tile: operand copy + residual copy, new h stored in place; m_in | m_out take the place of
+// the gathered rows), the gather warps idle.
 //
 // Same arithmetic and data flow as gnn_fused2.cuh.  What changed, from the per-role wait profile of version 2
 // (profiles/r1_fused_roles_v3.md: no role busier than 65 %, the tile period set by the chain  e-tile load -> MMA 1 ->
@@ -37,6 +42,7 @@ using gf2::mbar_test;
 using gf2::tma_prefetch_l2_2d;
 
 constexpr int kThreads3 = 12 * 32;
+constexpr int kNode = 2;                        // third mode besides gf::kUpdate / gf::kDecode
 constexpr int kOffW1 = 0;                       // 6 K blocks of this CTA's 64 output rows of W1
 constexpr int kOffW2 = kOffW1 + 6 * kWKB;       // 2 K blocks of W2
 constexpr int kOffRing = kOffW2 + 2 * kWKB;     // 4 K blocks: h_src (2), h_dst (2)
@@ -132,6 +138,11 @@ gnn_edge_fused3_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_co
   const int64_t M = resolve_rows(rows);
   const int64_t total = (M + 2 * kTileRows - 1) / (2 * kTileRows);
   const int n_my = total > pair ? (int)((total - pair + n_pairs - 1) / n_pairs) : 0;
+  constexpr bool kTwoLayers = MODE != gf::kDecode;
+  // K blocks of W1 that go with the operand tile (e, or h in kNode) and with the two ring halves
+  constexpr int kbE = MODE == kNode ? 0 : 4;
+  constexpr int kbR = MODE == kNode ? 2 : 0;
+  constexpr int colE = 0;                        // first column of the operand / residual tile in its tensor
 #ifdef TRK_FUSED_PROF
   long long pw[8] = {0, 0, 0, 0, 0, 0, 0, 0};
   const long long t_begin = clock64();
@@ -145,7 +156,7 @@ gnn_edge_fused3_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_co
     mbar_init(&bar->resfull, 1);
     mbar_init(&bar->resempty, 4);
     for (int i = 0; i < 2; ++i) {
-      mbar_init(&bar->gfull[i], 4);
+      mbar_init(&bar->gfull[i], MODE == kNode ? 1 : 4);
       mbar_init(&bar->gempty[i], 1);
       mbar_init(&bar->a1full[i], 1);
       mbar_init(&bar->a1empty[i], 8);
@@ -164,7 +175,7 @@ gnn_edge_fused3_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_co
   if (threadIdx.x >= 128 && threadIdx.x < 128 + kH) {
     const int c = threadIdx.x - 128;
     sb1[c] = p.b1[c];
-    sb2[c] = MODE == gf::kUpdate ? p.b2[c] : 0.f;
+    sb2[c] = kTwoLayers ? p.b2[c] : 0.f;
     swo[c] = MODE == gf::kDecode ? p.w_out[c] : 0.f;
   }
   __syncthreads();
@@ -181,24 +192,35 @@ gnn_edge_fused3_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_co
       auto row0_of = [&](int tl) { return (int)((pair + (int64_t)tl * n_pairs) * 2 * kTileRows + rank * kTileRows); };
       auto prefetch = [&](int tl) {
         if (tl < n_my)
-          for (int kb = 0; kb < 2; ++kb) tma_prefetch_l2_2d(&tmE, kb * 64, row0_of(tl));
+          for (int kb = 0; kb < (MODE == kNode ? 6 : 2); ++kb) tma_prefetch_l2_2d(&tmE, kb * 64, row0_of(tl));
       };
       prefetch(1);
       prefetch(2);
       const uint32_t eopfull_leader = mapa_u32(smem_u32(&bar->eopfull), 0);
-      int n_op = 0, n_res = 0;
-      const int res_end = MODE == gf::kUpdate ? n_my : 0;
-      while (n_op < n_my || n_res < res_end) {
+      const uint32_t gfull_leader[2] = {mapa_u32(smem_u32(&bar->gfull[0]), 0), mapa_u32(smem_u32(&bar->gfull[1]), 0)};
+      int n_op = 0, n_res = 0, n_g[2] = {0, 0};
+      const int res_end = kTwoLayers ? n_my : 0;
+      const int g_end = MODE == kNode ? n_my : 0;
+      while (n_op < n_my || n_res < res_end || n_g[0] < g_end || n_g[1] < g_end) {
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {              // kNode: m_in | m_out blocks into the ring halves
+          if (n_g[h] < g_end && mbar_test(&bar->gempty[h], (uint32_t)(n_g[h] & 1) ^ 1)) {
+            if (leader) mbar_arrive_expect_tx(&bar->gfull[h], 2 * 2 * kKB);
+            for (int kb = 0; kb < 2; ++kb)
+              tma_load_2d_pair(smem + kOffRing + (h * 2 + kb) * kKB, &tmE, gfull_leader[h], kH + h * kH + kb * 64, row0_of(n_g[h]));
+            ++n_g[h];
+          }
+        }
         if (n_op < n_my && mbar_test(&bar->eopempty, (uint32_t)(n_op & 1) ^ 1)) {
           if (leader) mbar_arrive_expect_tx(&bar->eopfull, 2 * 2 * kKB);
-          for (int kb = 0; kb < 2; ++kb) tma_load_2d_pair(smem + kOffEOp + kb * kKB, &tmE, eopfull_leader, kb * 64, row0_of(n_op));
+          for (int kb = 0; kb < 2; ++kb) tma_load_2d_pair(smem + kOffEOp + kb * kKB, &tmE, eopfull_leader, colE + kb * 64, row0_of(n_op));
           prefetch(n_op + 3);
           ++n_op;
         }
         // the residual copy of tile t is asked for only after its operand copy, so it finds the rows in L2
         if (n_res < res_end && n_res < n_op && mbar_test(&bar->resempty, (uint32_t)(n_res & 1) ^ 1)) {
           mbar_arrive_expect_tx(&bar->resfull, 2 * kKB);
-          for (int kb = 0; kb < 2; ++kb) tma_load_2d(smem + kOffRes + kb * kKB, &tmE, &bar->resfull, kb * 64, row0_of(n_res));
+          for (int kb = 0; kb < 2; ++kb) tma_load_2d(smem + kOffRes + kb * kKB, &tmE, &bar->resfull, colE + kb * 64, row0_of(n_res));
           ++n_res;
         }
       }
@@ -215,7 +237,7 @@ gnn_edge_fused3_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_co
       };
       int n1 = 0, n2 = 0;      // next tile of layer 1 / layer 2
       int stage1 = 0;          // 0: waiting for the accumulator and h_src, 1: for h_dst, 2: for the e operand tile
-      const int n2_end = MODE == gf::kUpdate ? n_my : 0;
+      const int n2_end = kTwoLayers ? n_my : 0;
       while (n1 < n_my || n2 < n2_end) {
         if (n2 < n2_end && n2 < n1) {
           const int b = n2 & 1;
@@ -236,7 +258,7 @@ gnn_edge_fused3_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_co
           if (stage1 == 0) {
             if (mbar_test(&bar->a1empty[b], ph ^ 1) && mbar_test(&bar->gfull[0], (uint32_t)(n1 & 1))) {
               tc_fence_after();
-              for (int kb = 0; kb < 2; ++kb) kblock(d, sbase + kOffRing + kb * kKB, sbase + kOffW1 + kb * kWKB, kb == 0);
+              for (int kb = 0; kb < 2; ++kb) kblock(d, sbase + kOffRing + kb * kKB, sbase + kOffW1 + (kbR + kb) * kWKB, kb == 0);
               tc_commit_pair(&bar->gempty[0]);
               stage1 = 1;
             }
@@ -244,7 +266,7 @@ gnn_edge_fused3_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_co
           if (stage1 == 1) {
             if (mbar_test(&bar->gfull[1], (uint32_t)(n1 & 1))) {
               tc_fence_after();
-              for (int kb = 0; kb < 2; ++kb) kblock(d, sbase + kOffRing + (2 + kb) * kKB, sbase + kOffW1 + (2 + kb) * kWKB, false);
+              for (int kb = 0; kb < 2; ++kb) kblock(d, sbase + kOffRing + (2 + kb) * kKB, sbase + kOffW1 + (kbR + 2 + kb) * kWKB, false);
               tc_commit_pair(&bar->gempty[1]);
               stage1 = 2;
             }
@@ -252,7 +274,7 @@ gnn_edge_fused3_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_co
           if (stage1 == 2) {
             if (mbar_test(&bar->eopfull, (uint32_t)(n1 & 1))) {
               tc_fence_after();
-              for (int kb = 0; kb < 2; ++kb) kblock(d, sbase + kOffEOp + kb * kKB, sbase + kOffW1 + (4 + kb) * kWKB, false);
+              for (int kb = 0; kb < 2; ++kb) kblock(d, sbase + kOffEOp + kb * kKB, sbase + kOffW1 + (kbE + kb) * kWKB, false);
               tc_commit_pair(&bar->eopempty);
               tc_commit_pair(&bar->a1full[b]);
               stage1 = 0;
@@ -275,7 +297,7 @@ gnn_edge_fused3_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_co
     const uint32_t dst0 = sbase + kOffRing + kb * kKB + (gw * 64 + half) * 128;
     const char* xb = reinterpret_cast<const char*>(p.X) + chunk * 16;
     const int64_t ldb = p.ldx * 2;
-    for (int tl = 0; tl < n_my; ++tl) {
+    for (int tl = 0; tl < (MODE == kNode ? 0 : n_my); ++tl) {
       const int64_t tile = pair + (int64_t)tl * n_pairs;
       const int64_t row = tile * 2 * kTileRows + rank * kTileRows + gw * 64 + lane;
       // rows beyond M gather node 0: their results are computed but never read (segment sums and scores stop at M)
@@ -354,7 +376,7 @@ gnn_edge_fused3_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_co
     }
   } else {
     // ---------------------------------------------------------------- epilogue 2: acc2 -> LNR -> + e -> store
-    if (MODE == gf::kUpdate) {
+    if (kTwoLayers) {
       const int quad = warp & 3;
       const int r = quad * 32 + lane;
       const uint32_t a2empty0 = mapa_u32(smem_u32(&bar->a2empty[0]), 0), a2empty1 = mapa_u32(smem_u32(&bar->a2empty[1]), 0);
@@ -395,7 +417,7 @@ gnn_edge_fused3_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_co
         __syncwarp();
         if (lane == 0) {
           const int row0 = (int)(tile * 2 * kTileRows + rank * kTileRows + quad * 32);
-          for (int kb = 0; kb < 2; ++kb) tma_store_2d(&tmEst, res + kb * kKB + quad * 32 * 128, kb * 64, row0);
+          for (int kb = 0; kb < 2; ++kb) tma_store_2d(&tmEst, res + kb * kKB + quad * 32 * 128, colE + kb * 64, row0);
           bulk_commit();
           FPW(1, bulk_wait_read<0>());  // the tile's rows have left shared memory: the buffer may be refilled
           mbar_arrive(&bar->resempty);

@@ -198,6 +198,28 @@ trk_status launch_edge_fused(trk_ctx* ctx, const bf16* X, int64_t ldx, bf16* E, 
   return TRK_OK;
 }
 
+// Fused node update of S4 (gnn_fused3.cuh, kNode), H = 128: X[:, 0:H] <- X[:, 0:H] + LNR(W2 LNR(W1 X + b1) + b2) in place.
+trk_status launch_node_fused(trk_ctx* ctx, bf16* X, int64_t x_rows, const DevLinear& L1, const DevLinear& L2, tc::Rows rows,
+                             cudaStream_t st) {
+  if (rows.m_cap <= 0) return TRK_OK;
+  static bool attr_set = false;
+  auto kern = gf3::gnn_edge_fused3_kernel<gf3::kNode>;
+  if (!attr_set) {
+    TRK_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, gf3::kSmemFused3));
+    attr_set = true;
+  }
+  CUtensorMap tw1, tw2, tx, txst;
+  TRK_TRY(make_tmap(ctx, &tw1, L1.w_bf16, gf::kH, 3 * gf::kH, 3 * gf::kH, 64));
+  TRK_TRY(make_tmap(ctx, &tw2, L2.w_bf16, gf::kH, gf::kH, gf::kH, 64));
+  TRK_TRY(make_tmap(ctx, &tx, X, x_rows, 3 * gf::kH, 3 * gf::kH, 128));
+  TRK_TRY(make_tmap(ctx, &txst, X, x_rows, gf::kH, 3 * gf::kH, 32));
+  gf::FusedParams p{X, 3 * gf::kH, nullptr, nullptr, L1.b_f32, L2.b_f32, ctx->cfg.gnn_layernorm, nullptr, 0.f, nullptr};
+  const int64_t ptiles = ceil_div(rows.m_cap, 2 * gf::kTileRows);
+  const unsigned grid = 2u * (unsigned)std::min<int64_t>(ptiles, ctx->sm_count / 2);
+  TRK_LAUNCH(ctx, kern, grid, gf3::kThreads3, gf3::kSmemFused3, st, tw1, tw2, tx, txst, rows, p);
+  return TRK_OK;
+}
+
 // ---------------------------------------------------------------- small SIMT kernels
 __device__ __forceinline__ int64_t rows_of(const int32_t* m_dev, int64_t m_off, int64_t m_cap) {
   if (!m_dev) return m_cap;
@@ -472,6 +494,10 @@ trk_status gnn_forward_bf16(trk_ctx* ctx, const float* hits, int64_t n, const in
     }
     TRK_TRY(segment_sums(ctx, E, true, n, X, st));
     // h <- h + LNR(W2 LNR(W1 [h ; m_in ; m_out] + b1) + b2): X is the concatenation already
+    if (fused && debug_knob(kKnobGnnFused) >= 3) {
+      TRK_TRY(launch_node_fused(ctx, X, x_rows, ctx->node_net.layers[0], ctx->node_net.layers[1], nrows, st));
+      continue;
+    }
     tc::EpiRowLn::Params n1{ctx->node_net.layers[0].b_f32, nullptr, nullptr, nullptr, ln, nullptr, 0, T1, H, nullptr, 0.f, nullptr};
     TRK_TRY(gemm_row_ln(ctx, X, x_rows, 3 * H, 3 * H, ctx->node_net.layers[0].w_bf16, n1, nrows, st));
     tc::EpiRowLn::Params n2{ctx->node_net.layers[1].b_f32, nullptr, nullptr, nullptr, ln, X, 3 * H, X, 3 * H, nullptr, 0.f, nullptr};
