@@ -92,13 +92,27 @@ segment_sum_kernel(const T* __restrict__ E, int H, const int32_t* __restrict__ i
   const int lane = threadIdx.x & 31;
   const int64_t w = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   if (w >= 2 * n_nodes) return;
-  const int64_t v = w >> 1;
+  // nodes from the back: the edge kernel has just written E front to back, so its last rows (the out-edges of the
+  // highest nodes) are still in L2
+  const int64_t v = n_nodes - 1 - (w >> 1);
   const int dir = (int)(w & 1);  // 0: in (dst == v, via perm), 1: out (src == v, contiguous)
   const int32_t* rp = dir == 0 ? in_rowptr : out_rowptr;
   const int b = rp[v], e = rp[v + 1];
   for (int c = lane * 4; c < H; c += 128) {
     float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-    for (int k = b; k < e; ++k) {
+    int k = b;
+    for (; k + 4 <= e; k += 4) {               // four independent row loads in flight; the sum keeps its fixed order
+      int64_t r0, r1, r2, r3;
+      if (dir == 0) { r0 = in_perm[k]; r1 = in_perm[k + 1]; r2 = in_perm[k + 2]; r3 = in_perm[k + 3]; }
+      else { r0 = k; r1 = k + 1; r2 = k + 2; r3 = k + 3; }
+      const float4 x0 = load4<T>(E + r0 * H + c), x1 = load4<T>(E + r1 * H + c), x2 = load4<T>(E + r2 * H + c),
+                   x3 = load4<T>(E + r3 * H + c);
+      acc.x += x0.x; acc.y += x0.y; acc.z += x0.z; acc.w += x0.w;
+      acc.x += x1.x; acc.y += x1.y; acc.z += x1.z; acc.w += x1.w;
+      acc.x += x2.x; acc.y += x2.y; acc.z += x2.z; acc.w += x2.w;
+      acc.x += x3.x; acc.y += x3.y; acc.z += x3.z; acc.w += x3.w;
+    }
+    for (; k < e; ++k) {
       const int64_t row = dir == 0 ? in_perm[k] : k;
       const float4 x = load4<T>(E + row * H + c);
       acc.x += x.x; acc.y += x.y; acc.z += x.z; acc.w += x.w;
