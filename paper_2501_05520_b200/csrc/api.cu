@@ -24,7 +24,7 @@ trk_status fail(trk_ctx* ctx, trk_status s, const std::string& msg) {
   return s;
 }
 
-static int64_t g_knobs[kKnobCount] = {1, 3, 1, 0, 0, 0, 0, 0};
+static int64_t g_knobs[kKnobCount] = {1, 4, 1, 0, 0, 0, 0, 0};
 int64_t debug_knob(int which) { return g_knobs[which]; }
 
 trk_status gemm_bf16_hook(trk_ctx* ctx, const void* a, const void* w, const float* bias, void* out, int64_t m, int n, int k, int relu,

@@ -135,7 +135,7 @@ __device__ __forceinline__ void row_stats(const float (&x)[kH], int use_ln, floa
 }
 
 #ifdef TRK_FUSED_PROF
-__device__ unsigned long long g_fused_prof[4][16][8];
+__device__ unsigned long long g_fused_prof[4][24][8];
 #define FPW(slot, stmt) do { long long _t0 = clock64(); stmt; pw[slot] += clock64() - _t0; } while (0)
 #else
 #define FPW(slot, stmt) stmt

@@ -1,0 +1,451 @@
+// Fused interaction-network edge / node update of S4 for H = 128 on CTA pairs, fourth version (reading C-12).
+// Modes, arithmetic, TMA / MMA / gather warps and buffer lifetimes are those of gnn_fused3.cuh.  What changed, from its
+// per-role wait profile (epilogue 2 was the busiest role: 5.5 k cycles per tile, 7 % of it waiting for input): both LayerNorm
+// epilogues run on EIGHT warps, two per TMEM lane quadrant, each taking one 64-column K block of the row:
+//   * a thread reads 64 accumulator columns, adds the bias, forms the partial (sum, sum of squares) of its half row and
+//     exchanges it with the thread that holds the other half through shared memory (named barriers of 64 threads);
+//     variance = E[x^2] - mean^2 in fp32 (the values are LayerNorm-scale, no cancellation problem);
+//   * no extra shared memory: epilogue 1 exchanges inside its own rows of the T buffer before it writes them, epilogue 2
+//     inside the first 16-byte cell of its row of the residual tile (the cell's residual values wait in registers);
+//   * 22 warps (704 threads, 88 registers): 0 TMA, 1 MMA issuer, 2-5 gather (four warps: a warp keeps only a few cp.async
+//     in flight, so the gather scales with their number), 6-13 epilogue 1, 14-21 epilogue 2;
+//   * dynamic shared memory is declared 1024-byte aligned (no manual alignment slack; checked at kernel start).
+#pragma once
+
+#include "gnn_fused3.cuh"
+
+namespace trk {
+namespace gf4 {
+
+using namespace tc;
+using gf::cp_async_16;
+using gf::cp_async_commit;
+using gf::cp_async_wait;
+using gf::FusedParams;
+using gf::kH;
+using gf::kKB;
+using gf::kTileRows;
+using gf::kWKB;
+using gf2::mbar_arrive_remote;
+using gf2::mbar_test;
+using gf2::tma_prefetch_l2_2d;
+
+constexpr int kThreads4 = 22 * 32;
+using gf3::f2;
+using gf3::kNode;
+constexpr int kOffW1 = 0;                       // 6 K blocks of this CTA's 64 output rows of W1
+constexpr int kOffW2 = kOffW1 + 6 * kWKB;       // 2 K blocks of W2
+constexpr int kOffRing = kOffW2 + 2 * kWKB;     // 4 K blocks: h_src (2), h_dst (2)
+constexpr int kOffEOp = kOffRing + 4 * kKB;     // 2 K blocks: the e tile as layer-1 operand
+constexpr int kOffRes = kOffEOp + 2 * kKB;      // 2 K blocks: the e tile as residual, overwritten in place and stored
+constexpr int kOffT = kOffRes + 2 * kKB;        // 2 K blocks: layer-1 output
+constexpr int kOffVec = kOffT + 2 * kKB;        // b1, b2, w_out: 3 x 128 fp32
+constexpr int kOffBar = kOffVec + 3 * kH * 4;
+constexpr int kSmemFused4 = kOffBar + 256;
+static_assert(kSmemFused4 <= 232448, "shared memory budget of one CTA");
+
+struct Bars {
+  uint64_t w_full;
+  uint64_t eopfull;       // L  tx: both CTAs' operand tiles
+  uint64_t eopempty;      //    own, multicast commit (MMA 1 has read the operand tile)
+  uint64_t resfull;       //    own, tx: this CTA's residual tile
+  uint64_t resempty;      //    own, 8 arrivals (epilogue-2 warps, after their rows have left shared memory)
+  uint64_t gfull[2];      // L  8 arrivals (4 gather warps x 2 CTAs), halves: h_src, h_dst (kNode: 1, tx)
+  uint64_t gempty[2];     //    own, multicast commit
+  uint64_t a1full[2];     //    own, multicast commit
+  uint64_t a1empty[2];    // L  16 arrivals
+  uint64_t tfull;         // L  16 arrivals
+  uint64_t tempty;        //    own, multicast commit
+  uint64_t a2full[2];     //    own, multicast commit
+  uint64_t a2empty[2];    // L  16 arrivals
+  uint32_t tmem_slot;
+};
+
+__device__ __forceinline__ void named_bar_sync(int id, int threads) {
+  asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(threads) : "memory");
+}
+
+// Half an accumulator row (this thread's TMEM lane, 64 fp32 columns from `taddr`) + bias -> 32 packed pairs, and the
+// partial sum / sum of squares of those 64 values.
+template <bool BIAS_GLOBAL>
+__device__ __forceinline__ void load_half(uint32_t taddr, const float* __restrict__ bias, float2 (&x)[32], float& ps, float& pq) {
+  uint32_t u0[32], u1[32];
+  tmem_ld32(taddr, u0);
+  tmem_ld32(taddr + 32, u1);
+  const float4* b4 = reinterpret_cast<const float4*>(bias);
+  float4 bb[16];
+#pragma unroll
+  for (int j = 0; j < 16; ++j) bb[j] = BIAS_GLOBAL ? __ldg(b4 + j) : b4[j];
+  tmem_ld_wait();
+#pragma unroll
+  for (int i = 0; i < 32; i += 4) {
+    x[i / 2] = __fadd2_rn(f2(__uint_as_float(u0[i]), __uint_as_float(u0[i + 1])), f2(bb[i / 4].x, bb[i / 4].y));
+    x[i / 2 + 1] = __fadd2_rn(f2(__uint_as_float(u0[i + 2]), __uint_as_float(u0[i + 3])), f2(bb[i / 4].z, bb[i / 4].w));
+    x[16 + i / 2] = __fadd2_rn(f2(__uint_as_float(u1[i]), __uint_as_float(u1[i + 1])), f2(bb[8 + i / 4].x, bb[8 + i / 4].y));
+    x[16 + i / 2 + 1] = __fadd2_rn(f2(__uint_as_float(u1[i + 2]), __uint_as_float(u1[i + 3])), f2(bb[8 + i / 4].z, bb[8 + i / 4].w));
+  }
+  float2 s0 = f2(0.f, 0.f), s1 = s0, q0 = s0, q1 = s0;
+#pragma unroll
+  for (int i = 0; i < 32; i += 2) {
+    s0 = __fadd2_rn(s0, x[i]); s1 = __fadd2_rn(s1, x[i + 1]);
+    q0 = __ffma2_rn(x[i], x[i], q0); q1 = __ffma2_rn(x[i + 1], x[i + 1], q1);
+  }
+  const float2 s = __fadd2_rn(s0, s1), q = __fadd2_rn(q0, q1);
+  ps = s.x + s.y;
+  pq = q.x + q.y;
+}
+
+__device__ __forceinline__ void ln_coeffs(float ps, float pq, float2 other, int use_ln, float2& rs, float2& sh) {
+  float mean = 0.f, rstd = 1.f;
+  if (use_ln) {
+    mean = (ps + other.x) * (1.f / kH);
+    const float var = fmaxf((pq + other.y) * (1.f / kH) - mean * mean, 0.f);
+    rstd = rsqrtf(var + 1e-5f);
+  }
+  rs = f2(rstd, rstd);
+  sh = f2(-mean * rstd, -mean * rstd);
+}
+
+template <int MODE>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads4, 1)
+gnn_edge_fused4_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constant__ CUtensorMap tmW2,
+                       const __grid_constant__ CUtensorMap tmE, const __grid_constant__ CUtensorMap tmEst, Rows rows, FusedParams p) {
+  extern __shared__ __align__(1024) uint8_t smem[];
+  if ((smem_u32(smem) & 1023u) != 0) __trap();   // the swizzled operand layout needs the 1024-byte alignment declared above
+  Bars* bar = reinterpret_cast<Bars*>(smem + kOffBar);
+  float* sb1 = reinterpret_cast<float*>(smem + kOffVec);
+  float* sb2 = sb1 + kH;
+  float* swo = sb2 + kH;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const uint32_t rank = cluster_ctarank();
+  const bool leader = rank == 0;
+  const int pair = blockIdx.x >> 1, n_pairs = gridDim.x >> 1;
+  const int64_t M = resolve_rows(rows);
+  const int64_t total = (M + 2 * kTileRows - 1) / (2 * kTileRows);
+  const int n_my = total > pair ? (int)((total - pair + n_pairs - 1) / n_pairs) : 0;
+  constexpr bool kTwoLayers = MODE != gf::kDecode;
+  // K blocks of W1 that go with the operand tile (e, or h in kNode) and with the two ring halves
+  constexpr int kbE = MODE == kNode ? 0 : 4;
+  constexpr int kbR = MODE == kNode ? 2 : 0;
+  constexpr int colE = 0;                        // first column of the operand / residual tile in its tensor
+#ifdef TRK_FUSED_PROF
+  long long pw[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+  const long long t_begin = clock64();
+#endif
+
+  if (warp == 0 && lane == 0) {
+    prefetch_tmap(&tmW1); prefetch_tmap(&tmW2); prefetch_tmap(&tmE); prefetch_tmap(&tmEst);
+    mbar_init(&bar->w_full, 1);
+    mbar_init(&bar->eopfull, 1);
+    mbar_init(&bar->eopempty, 1);
+    mbar_init(&bar->resfull, 1);
+    mbar_init(&bar->resempty, 8);
+    for (int i = 0; i < 2; ++i) {
+      mbar_init(&bar->gfull[i], MODE == kNode ? 1 : 8);
+      mbar_init(&bar->gempty[i], 1);
+      mbar_init(&bar->a1full[i], 1);
+      mbar_init(&bar->a1empty[i], 16);
+      mbar_init(&bar->a2full[i], 1);
+      mbar_init(&bar->a2empty[i], 16);
+    }
+    mbar_init(&bar->tfull, 16);
+    mbar_init(&bar->tempty, 1);
+    fence_barrier_init();
+    // this CTA's halves of the weights: output rows [64 rank, 64 rank + 64)
+    mbar_arrive_expect_tx(&bar->w_full, 8 * kWKB);
+    for (int kb = 0; kb < 6; ++kb) tma_load_2d(smem + kOffW1 + kb * kWKB, &tmW1, &bar->w_full, kb * 64, (int)rank * 64);
+    for (int kb = 0; kb < 2; ++kb) tma_load_2d(smem + kOffW2 + kb * kWKB, &tmW2, &bar->w_full, kb * 64, (int)rank * 64);
+  }
+  if (warp == 1) tmem_alloc_pair<512>(&bar->tmem_slot);
+  if (threadIdx.x >= 128 && threadIdx.x < 128 + kH) {
+    const int c = threadIdx.x - 128;
+    sb1[c] = p.b1[c];
+    sb2[c] = kTwoLayers ? p.b2[c] : 0.f;
+    swo[c] = MODE == gf::kDecode ? p.w_out[c] : 0.f;
+  }
+  __syncthreads();
+  mbar_wait(&bar->w_full, 0);
+  tc_fence_before();
+  cluster_sync_all();
+  tc_fence_after();
+  const uint32_t tmem_base = bar->tmem_slot;
+  const uint32_t sbase = smem_u32(smem);
+
+  if (warp == 0) {
+    // ---------------------------------------------------------------- TMA producer: operand and residual copies of the e tiles
+    if (lane == 0) {
+      auto row0_of = [&](int tl) { return (int)((pair + (int64_t)tl * n_pairs) * 2 * kTileRows + rank * kTileRows); };
+      auto prefetch = [&](int tl) {
+        if (tl < n_my)
+          for (int kb = 0; kb < (MODE == kNode ? 6 : 2); ++kb) tma_prefetch_l2_2d(&tmE, kb * 64, row0_of(tl));
+      };
+      prefetch(1);
+      prefetch(2);
+      const uint32_t eopfull_leader = mapa_u32(smem_u32(&bar->eopfull), 0);
+      const uint32_t gfull_leader[2] = {mapa_u32(smem_u32(&bar->gfull[0]), 0), mapa_u32(smem_u32(&bar->gfull[1]), 0)};
+      int n_op = 0, n_res = 0, n_g[2] = {0, 0};
+      const int res_end = kTwoLayers ? n_my : 0;
+      const int g_end = MODE == kNode ? n_my : 0;
+      while (n_op < n_my || n_res < res_end || n_g[0] < g_end || n_g[1] < g_end) {
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {              // kNode: m_in | m_out blocks into the ring halves
+          if (n_g[h] < g_end && mbar_test(&bar->gempty[h], (uint32_t)(n_g[h] & 1) ^ 1)) {
+            if (leader) mbar_arrive_expect_tx(&bar->gfull[h], 2 * 2 * kKB);
+            for (int kb = 0; kb < 2; ++kb)
+              tma_load_2d_pair(smem + kOffRing + (h * 2 + kb) * kKB, &tmE, gfull_leader[h], kH + h * kH + kb * 64, row0_of(n_g[h]));
+            ++n_g[h];
+          }
+        }
+        if (n_op < n_my && mbar_test(&bar->eopempty, (uint32_t)(n_op & 1) ^ 1)) {
+          if (leader) mbar_arrive_expect_tx(&bar->eopfull, 2 * 2 * kKB);
+          for (int kb = 0; kb < 2; ++kb) tma_load_2d_pair(smem + kOffEOp + kb * kKB, &tmE, eopfull_leader, colE + kb * 64, row0_of(n_op));
+          prefetch(n_op + 3);
+          ++n_op;
+        }
+        // the residual copy of tile t is asked for only after its operand copy, so it finds the rows in L2
+        if (n_res < res_end && n_res < n_op && mbar_test(&bar->resempty, (uint32_t)(n_res & 1) ^ 1)) {
+          mbar_arrive_expect_tx(&bar->resfull, 2 * kKB);
+          for (int kb = 0; kb < 2; ++kb) tma_load_2d(smem + kOffRes + kb * kKB, &tmE, &bar->resfull, colE + kb * 64, row0_of(n_res));
+          ++n_res;
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ---------------------------------------------------------------- MMA issuer (leader CTA): polls, issues what is ready
+    if (leader && lane == 0) {
+      constexpr uint32_t idesc = make_idesc_pair(kH);
+      auto kblock = [&](uint32_t d_tmem, uint32_t a_addr, uint32_t b_addr, bool first) {
+        const uint64_t adesc = make_smem_desc(a_addr), bdesc = make_smem_desc(b_addr);
+#pragma unroll
+        for (int k = 0; k < BK / UMMA_K; ++k)
+          tc_mma_bf16_pair(d_tmem, adesc + (uint64_t)(k * 2), bdesc + (uint64_t)(k * 2), idesc, (!first || k != 0) ? 1u : 0u);
+      };
+      int n1 = 0, n2 = 0;      // next tile of layer 1 / layer 2
+      int stage1 = 0;          // 0: waiting for the accumulator and h_src, 1: for h_dst, 2: for the e operand tile
+      const int n2_end = kTwoLayers ? n_my : 0;
+      while (n1 < n_my || n2 < n2_end) {
+        if (n2 < n2_end && n2 < n1) {
+          const int b = n2 & 1;
+          const uint32_t ph = (n2 >> 1) & 1;
+          if (mbar_test(&bar->tfull, (uint32_t)(n2 & 1)) && mbar_test(&bar->a2empty[b], ph ^ 1)) {
+            tc_fence_after();
+            const uint32_t d = tmem_base + (uint32_t)(2 * kH + b * kH);
+            for (int kb = 0; kb < 2; ++kb) kblock(d, sbase + kOffT + kb * kKB, sbase + kOffW2 + kb * kWKB, kb == 0);
+            tc_commit_pair(&bar->tempty);
+            tc_commit_pair(&bar->a2full[b]);
+            ++n2;
+          }
+        }
+        if (n1 < n_my) {
+          const int b = n1 & 1;
+          const uint32_t ph = (n1 >> 1) & 1;
+          const uint32_t d = tmem_base + (uint32_t)(b * kH);
+          if (stage1 == 0) {
+            if (mbar_test(&bar->a1empty[b], ph ^ 1) && mbar_test(&bar->gfull[0], (uint32_t)(n1 & 1))) {
+              tc_fence_after();
+              for (int kb = 0; kb < 2; ++kb) kblock(d, sbase + kOffRing + kb * kKB, sbase + kOffW1 + (kbR + kb) * kWKB, kb == 0);
+              tc_commit_pair(&bar->gempty[0]);
+              stage1 = 1;
+            }
+          }
+          if (stage1 == 1) {
+            if (mbar_test(&bar->gfull[1], (uint32_t)(n1 & 1))) {
+              tc_fence_after();
+              for (int kb = 0; kb < 2; ++kb) kblock(d, sbase + kOffRing + (2 + kb) * kKB, sbase + kOffW1 + (kbR + 2 + kb) * kWKB, false);
+              tc_commit_pair(&bar->gempty[1]);
+              stage1 = 2;
+            }
+          }
+          if (stage1 == 2) {
+            if (mbar_test(&bar->eopfull, (uint32_t)(n1 & 1))) {
+              tc_fence_after();
+              for (int kb = 0; kb < 2; ++kb) kblock(d, sbase + kOffEOp + kb * kKB, sbase + kOffW1 + (kbE + kb) * kWKB, false);
+              tc_commit_pair(&bar->eopempty);
+              tc_commit_pair(&bar->a1full[b]);
+              stage1 = 0;
+              ++n1;
+            }
+          }
+        }
+      }
+    }
+  } else if (warp < 6) {
+    // ---------------------------------------------------------------- gather: h[src], h[dst] rows -> ring (32 rows per warp)
+    const int gw = warp - 2;
+    const uint32_t gfull0 = mapa_u32(smem_u32(&bar->gfull[0]), 0), gfull1 = mapa_u32(smem_u32(&bar->gfull[1]), 0);
+    const int half = lane >> 4, chunk = lane & 15;
+    const int kb = chunk >> 3, ch = chunk & 7;
+    // iteration i copies chunk `chunk` of row rr = 2 i + half of this warp's 32 rows; (rr & 7) = 2 (i & 3) + half
+    uint32_t sw[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) sw[j] = (uint32_t)((ch ^ (2 * j + half)) << 4);
+    const uint32_t dst0 = sbase + kOffRing + kb * kKB + (gw * 32 + half) * 128;
+    const char* xb = reinterpret_cast<const char*>(p.X) + chunk * 16;
+    const int64_t ldb = p.ldx * 2;
+    for (int tl = 0; tl < (MODE == kNode ? 0 : n_my); ++tl) {
+      const int64_t tile = pair + (int64_t)tl * n_pairs;
+      const int64_t row = tile * 2 * kTileRows + rank * kTileRows + gw * 32 + lane;
+      // rows beyond M gather node 0: their results are computed but never read (segment sums and scores stop at M)
+      const int s_i = row < M ? p.src[row] : 0, d_i = row < M ? p.dst[row] : 0;
+#pragma unroll 1
+      for (int h = 0; h < 2; ++h) {
+        FPW(h, mbar_wait(&bar->gempty[h], (uint32_t)(tl & 1) ^ 1));
+        const int mine = h == 0 ? s_i : d_i;
+        const uint32_t dsth = dst0 + h * 2 * kKB;
+#pragma unroll
+        for (int i = 0; i < 16; ++i) {
+          const int idx = __shfl_sync(0xffffffffu, mine, 2 * i + half);
+          cp_async_16(dsth + i * 256 + sw[i & 3], xb + (int64_t)idx * ldb, 16);
+        }
+        cp_async_commit();
+      }
+      FPW(2, cp_async_wait<1>());
+      fence_proxy_async();
+      __syncwarp();
+      if (lane == 0) mbar_arrive_remote(gfull0);
+      FPW(3, cp_async_wait<0>());
+      fence_proxy_async();
+      __syncwarp();
+      if (lane == 0) mbar_arrive_remote(gfull1);
+    }
+  } else if (warp < 14) {
+    // ---------------------------------------------------------------- epilogue 1: acc1 -> LNR -> T (or score), 64 columns per thread
+    const int quad = warp & 3, half = (warp - 6) >> 2;
+    const int r = quad * 32 + lane;   // row of this thread inside the CTA's 128-row tile == TMEM lane
+    const int bid = 1 + quad;         // named barrier of the two warps that share this quadrant's rows
+    const uint32_t a1empty0 = mapa_u32(smem_u32(&bar->a1empty[0]), 0), a1empty1 = mapa_u32(smem_u32(&bar->a1empty[1]), 0);
+    const uint32_t tfull_l = mapa_u32(smem_u32(&bar->tfull), 0);
+    // exchange slots inside this quadrant's own rows of T (K block 0: statistics, K block 1: the decoder's partial dots)
+    float2* xs = reinterpret_cast<float2*>(smem + kOffT + quad * 32 * 128);
+    float* xd = reinterpret_cast<float*>(smem + kOffT + kKB + quad * 32 * 128);
+    for (int tl = 0; tl < n_my; ++tl) {
+      const int64_t tile = pair + (int64_t)tl * n_pairs;
+      const int b = tl & 1;
+      const uint32_t ph = (tl >> 1) & 1;
+      FPW(0, mbar_wait(&bar->a1full[b], ph));
+      tc_fence_after();
+      float2 x[32];
+      float ps, pq;
+      FPW(2, load_half<false>(tmem_base + ((uint32_t)(quad * 32) << 16) + (uint32_t)(b * kH + half * 64), sb1 + half * 64, x, ps, pq));
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive_remote(b == 0 ? a1empty0 : a1empty1);     // the accumulator is in registers now
+      if (kTwoLayers) FPW(1, mbar_wait(&bar->tempty, (uint32_t)(tl & 1) ^ 1));   // the layer-2 MMA of the previous tile has read T
+      xs[half * 32 + lane] = f2(ps, pq);
+      named_bar_sync(bid, 64);
+      const float2 other = xs[(half ^ 1) * 32 + lane];
+      float2 rs, sh;
+      ln_coeffs(ps, pq, other, p.use_ln, rs, sh);
+      if (MODE == gf::kDecode) {
+        float2 d0 = f2(0.f, 0.f), d1 = d0;
+        const float4* w4 = reinterpret_cast<const float4*>(swo + half * 64);
+#pragma unroll
+        for (int c = 0; c < 64; c += 4) {
+          const float4 w = w4[c / 4];
+          float2 v0 = __ffma2_rn(x[c / 2], rs, sh), v1 = __ffma2_rn(x[c / 2 + 1], rs, sh);
+          v0.x = fmaxf(v0.x, 0.f); v0.y = fmaxf(v0.y, 0.f); v1.x = fmaxf(v1.x, 0.f); v1.y = fmaxf(v1.y, 0.f);
+          d0 = __ffma2_rn(v0, f2(w.x, w.y), d0);
+          d1 = __ffma2_rn(v1, f2(w.z, w.w), d1);
+        }
+        const float d = (d0.x + d0.y) + (d1.x + d1.y);
+        if (half == 1) xd[lane] = d;
+        named_bar_sync(bid, 64);          // also: both warps have read this tile's statistics slots
+        if (half == 0) {
+          const int64_t row = tile * 2 * kTileRows + rank * kTileRows + r;
+          if (row < M) p.score[row] = fast_sigmoid(p.b_out + d + xd[lane]);
+        }
+        named_bar_sync(bid, 64);          // the partial dot has been read: the slot may be rewritten for the next tile
+      } else {
+        named_bar_sync(bid, 64);          // both warps have read the slots: the rows of T may be written
+#pragma unroll
+        for (int c = 0; c < 64; c += 8) {                  // 8 columns = one 16-byte chunk of the swizzled K block `half`
+          uint32_t w[4];
+#pragma unroll
+          for (int i = 0; i < 4; ++i) {
+            const float2 v = __ffma2_rn(x[c / 2 + i], rs, sh);
+            w[i] = pack_bf16(fmaxf(v.x, 0.f), fmaxf(v.y, 0.f));
+          }
+          const int ch = c >> 3;
+          *reinterpret_cast<uint4*>(smem + kOffT + half * kKB + r * 128 + ((ch ^ (r & 7)) << 4)) = make_uint4(w[0], w[1], w[2], w[3]);
+        }
+        fence_proxy_async();
+        __syncwarp();
+        if (lane == 0) mbar_arrive_remote(tfull_l);
+      }
+    }
+  } else {
+    // ---------------------------------------------------------------- epilogue 2: acc2 -> LNR -> + residual -> store, 64 columns per thread
+    if (kTwoLayers) {
+      const int quad = warp & 3, half = (warp - 14) >> 2;
+      const int r = quad * 32 + lane;
+      const int bid = 5 + quad;
+      const uint32_t a2empty0 = mapa_u32(smem_u32(&bar->a2empty[0]), 0), a2empty1 = mapa_u32(smem_u32(&bar->a2empty[1]), 0);
+      uint8_t* res = smem + kOffRes + half * kKB;
+      for (int tl = 0; tl < n_my; ++tl) {
+        const int64_t tile = pair + (int64_t)tl * n_pairs;
+        const int b = tl & 1;
+        const uint32_t ph = (tl >> 1) & 1;
+        FPW(0, mbar_wait(&bar->a2full[b], ph));
+        tc_fence_after();
+        float2 x[32];
+        float ps, pq;
+        FPW(2, load_half<false>(tmem_base + ((uint32_t)(quad * 32) << 16) + (uint32_t)(2 * kH + b * kH + half * 64), sb2 + half * 64, x, ps, pq));
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive_remote(b == 0 ? a2empty0 : a2empty1);
+        FPW(3, mbar_wait(&bar->resfull, (uint32_t)(tl & 1)));        // the residual copy of this tile has landed
+        // exchange of the half-row statistics through the first cell of this thread's residual row (its values wait in e0)
+        uint4* cell0 = reinterpret_cast<uint4*>(res + r * 128 + ((0 ^ (r & 7)) << 4));
+        const uint4 e0 = *cell0;
+        *reinterpret_cast<float2*>(cell0) = f2(ps, pq);
+        named_bar_sync(bid, 64);
+        const float2 other = *reinterpret_cast<const float2*>(smem + kOffRes + (half ^ 1) * kKB + r * 128 + ((0 ^ (r & 7)) << 4));
+        named_bar_sync(bid, 64);            // both have read: the cells may be overwritten with results
+        float2 rs, sh;
+        ln_coeffs(ps, pq, other, p.use_ln, rs, sh);
+#pragma unroll
+        for (int c = 0; c < 64; c += 8) {
+          const int ch = c >> 3;
+          uint4* cell = reinterpret_cast<uint4*>(res + r * 128 + ((ch ^ (r & 7)) << 4));
+          const uint4 e = c == 0 ? e0 : *cell;
+          const __nv_bfloat162* e2 = reinterpret_cast<const __nv_bfloat162*>(&e);
+          uint32_t w[4];
+#pragma unroll
+          for (int i = 0; i < 4; ++i) {
+            float2 v = __ffma2_rn(x[c / 2 + i], rs, sh);
+            v.x = fmaxf(v.x, 0.f);
+            v.y = fmaxf(v.y, 0.f);
+            v = __fadd2_rn(v, __bfloat1622float2(e2[i]));
+            w[i] = pack_bf16(v.x, v.y);
+          }
+          *cell = make_uint4(w[0], w[1], w[2], w[3]);
+        }
+        fence_proxy_async();
+        __syncwarp();
+        if (lane == 0) {
+          const int row0 = (int)(tile * 2 * kTileRows + rank * kTileRows + quad * 32);
+          tma_store_2d(&tmEst, res + quad * 32 * 128, colE + half * 64, row0);
+          bulk_commit();
+          FPW(1, bulk_wait_read<0>());  // the rows have left shared memory: the buffer may be refilled
+          mbar_arrive(&bar->resempty);
+        }
+      }
+      if (lane == 0) bulk_wait_all();
+    }
+  }
+#ifdef TRK_FUSED_PROF
+  if (MODE == gf::kUpdate && blockIdx.x < 4 && lane == 0) {
+    for (int i = 0; i < 7; ++i) gf2::g_fused_prof[blockIdx.x][warp][i] = (unsigned long long)pw[i];
+    gf2::g_fused_prof[blockIdx.x][warp][7] = (unsigned long long)(clock64() - t_begin);
+  }
+#endif
+  tc_fence_before();
+  cluster_sync_all();
+  if (warp == 1) {
+    tc_fence_after();
+    tmem_dealloc_pair<512>(tmem_base);
+  }
+}
+
+}  // namespace gf4
+}  // namespace trk

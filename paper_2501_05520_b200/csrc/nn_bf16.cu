@@ -18,6 +18,7 @@
 #include "gnn_fused.cuh"
 #include "gnn_fused2.cuh"
 #include "gnn_fused3.cuh"
+#include "gnn_fused4.cuh"
 #include "graph.cuh"
 #include "nn.cuh"
 
@@ -174,8 +175,11 @@ trk_status launch_edge_fused(trk_ctx* ctx, const bf16* X, int64_t ldx, bf16* E, 
   auto kern = gf::gnn_edge_fused_kernel<MODE>;
   auto kern2 = gf2::gnn_edge_fused2_kernel<MODE>;
   auto kern3 = gf3::gnn_edge_fused3_kernel<MODE>;
+  // version 4 (eight-warp epilogues) serves the update; the decoder is a single launch per call and keeps version 3
+  auto kern4 = gf4::gnn_edge_fused4_kernel<gf::kUpdate>;
   if (!attr_set) {
     TRK_CUDA(ctx, cudaFuncSetAttribute(kern3, cudaFuncAttributeMaxDynamicSharedMemorySize, gf3::kSmemFused3));
+    TRK_CUDA(ctx, cudaFuncSetAttribute(kern4, cudaFuncAttributeMaxDynamicSharedMemorySize, gf4::kSmemFused4));
     TRK_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, gf::kSmemFused));
     TRK_CUDA(ctx, cudaFuncSetAttribute(kern2, cudaFuncAttributeMaxDynamicSharedMemorySize, gf2::kSmemFused2));
     attr_set = true;
@@ -188,7 +192,9 @@ trk_status launch_edge_fused(trk_ctx* ctx, const bf16* X, int64_t ldx, bf16* E, 
   gf::FusedParams p{X, ldx, src, dst, L1.b_f32, L2.b_f32, ctx->cfg.gnn_layernorm, w_out, b_out, score};
   const int64_t ptiles = ceil_div(rows.m_cap, 2 * gf::kTileRows);
   const unsigned grid = 2u * (unsigned)std::min<int64_t>(ptiles, ctx->sm_count / 2);
-  if (debug_knob(kKnobGnnFused) >= 3) {
+  if (MODE == gf::kUpdate && debug_knob(kKnobGnnFused) >= 4) {
+    TRK_LAUNCH(ctx, kern4, grid, gf4::kThreads4, gf4::kSmemFused4, st, tw1, tw2, te, test, rows, p);
+  } else if (debug_knob(kKnobGnnFused) >= 3) {
     TRK_LAUNCH(ctx, kern3, grid, gf3::kThreads3, gf3::kSmemFused3, st, tw1, tw2, te, test, rows, p);
   } else if (debug_knob(kKnobGnnFused) >= 2) {
     TRK_LAUNCH(ctx, kern2, grid, gf2::kThreads2, gf2::kSmemFused2, st, tw1, tw2, te, test, rows, p);
@@ -204,8 +210,10 @@ trk_status launch_node_fused(trk_ctx* ctx, bf16* X, int64_t x_rows, const DevLin
   if (rows.m_cap <= 0) return TRK_OK;
   static bool attr_set = false;
   auto kern = gf3::gnn_edge_fused3_kernel<gf3::kNode>;
+  auto kern4 = gf4::gnn_edge_fused4_kernel<gf3::kNode>;
   if (!attr_set) {
     TRK_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, gf3::kSmemFused3));
+    TRK_CUDA(ctx, cudaFuncSetAttribute(kern4, cudaFuncAttributeMaxDynamicSharedMemorySize, gf4::kSmemFused4));
     attr_set = true;
   }
   CUtensorMap tw1, tw2, tx, txst;
@@ -216,7 +224,11 @@ trk_status launch_node_fused(trk_ctx* ctx, bf16* X, int64_t x_rows, const DevLin
   gf::FusedParams p{X, 3 * gf::kH, nullptr, nullptr, L1.b_f32, L2.b_f32, ctx->cfg.gnn_layernorm, nullptr, 0.f, nullptr};
   const int64_t ptiles = ceil_div(rows.m_cap, 2 * gf::kTileRows);
   const unsigned grid = 2u * (unsigned)std::min<int64_t>(ptiles, ctx->sm_count / 2);
-  TRK_LAUNCH(ctx, kern, grid, gf3::kThreads3, gf3::kSmemFused3, st, tw1, tw2, tx, txst, rows, p);
+  if (debug_knob(kKnobGnnFused) >= 4) {
+    TRK_LAUNCH(ctx, kern4, grid, gf4::kThreads4, gf4::kSmemFused4, st, tw1, tw2, tx, txst, rows, p);
+  } else {
+    TRK_LAUNCH(ctx, kern, grid, gf3::kThreads3, gf3::kSmemFused3, st, tw1, tw2, tx, txst, rows, p);
+  }
   return TRK_OK;
 }
 
