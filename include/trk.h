@@ -209,9 +209,12 @@ trk_status trk_gemm_bf16(const void* a, const void* w, const float* bias, void* 
  *   "gnn_fused"  2: with gnn_hidden == 128 the S4 edge update and the decoder run as one fused CTA-pair kernel
  *                per iteration (gathered endpoint rows, both layers, LayerNorm, residual; gnn_fused2.cuh); 1: the first
  *                version of that kernel (gnn_fused.cuh); 0: layer-by-layer GEMM launches.
- *                3 (default): its third version (gnn_fused3.cuh) -- see that value's description in DESIGN.md section 6.
+ *                3: its third version (gnn_fused3.cuh), which also fuses the node update; 4 (default): the fourth
+ *                (gnn_fused4.cuh, eight-warp epilogues) for the edge and node updates -- DESIGN.md section 6.
  *   "epi_split"  1 (default): bf16-output layers with 256-column tiles and a single 64-wide K block (the first layer of the S3
- *                filter MLP) run their epilogue on eight warps (two per TMEM lane quadrant); 0: four warps.
+ *                filter MLP) run their epilogue on eight warps (two per TMEM lane quadrant); 2: in addition that layer's input
+ *                rows [e_src ; e_dst] are gathered inside the GEMM kernel instead of by a separate launch (measured slower on
+ *                the pileup-200 event: 1.36 ms against 1.01 + 0.25 ms, so not the default); 0: four warps.
  * Returns TRK_ERR_INVALID_ARG for an unknown key.  Not thread safe against running trk_* calls. */
 trk_status trk_debug_set(const char* key, int64_t value);
 

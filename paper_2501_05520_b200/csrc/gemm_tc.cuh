@@ -163,7 +163,17 @@ constexpr int num_stages(int bn, int split = 1) {
 constexpr int smem_bytes(int bn, bool tma_store = false, int split = 1) {
   return num_stages(bn, split) * stage_bytes(bn) + (tma_store ? split * kEpiWarps * kStoreStage : 0) + 1024 /*alignment*/ + 256 /*barriers*/;
 }
-constexpr int threads_for(int split) { return 64 + 32 * kEpiWarps * split; }
+constexpr int kGatherWarps = 4;
+constexpr int threads_for(int split, bool gather = false) { return 64 + 32 * kEpiWarps * split + (gather ? 32 * kGatherWarps : 0); }
+
+// GATHER_A: the A tile of a one-K-block layer is not loaded by TMA but assembled by four gather warps straight into the
+// swizzled operand layout: row m = bf16([feat[src[m]] ; feat[dst[m]]]) zero padded to 64 columns (the S3 filter input).
+struct AGather {
+  const float* feat;      // fp32 [n][u]
+  const int32_t* src;     // indexed by rows.m_off + m
+  const int32_t* dst;
+  int u;                  // 2 u <= 64
+};
 
 // What an epilogue may use besides its own parameters: a per-warp staging area and the output tensor map.
 struct EpiShared {
@@ -176,10 +186,12 @@ struct EpiShared {
 // Epi::run(params, tmem_tile_addr (lane and column base of this warp's quadrant), row0 (first row of the
 //          tile), col0 (first column of the tile), n_blk, rows M, lane-row index r, release()) must call
 //          `release` exactly once after its last TMEM read.
-template <int BN, class Epi, int SPLIT = 1>
-__global__ void __launch_bounds__(threads_for(SPLIT), 1)
+__device__ __forceinline__ uint32_t pack_bf16(float a, float b);
+
+template <int BN, class Epi, int SPLIT = 1, bool GATHER_A = false>
+__global__ void __launch_bounds__(threads_for(SPLIT, GATHER_A), 1)
 gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, const __grid_constant__ CUtensorMap tmC,
-               Rows rows, int n_tiles, int k_blocks, typename Epi::Params ep) {
+               Rows rows, int n_tiles, int k_blocks, typename Epi::Params ep, AGather ag) {
   constexpr int STAGES = num_stages(BN, SPLIT);
   constexpr int A_BYTES = BM * BK * 2;
   constexpr int STAGE = stage_bytes(BN);
@@ -196,13 +208,28 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int64_t M = resolve_rows(rows);
-  const int64_t total = ((M + BM - 1) / BM) * n_tiles;
+  const int64_t m_tiles = (M + BM - 1) / BM;
+  const int64_t total = m_tiles * n_tiles;
+  // This CTA's j-th tile.  Default: tiles in grid strides, n fastest (co-resident CTAs share A rows in L2).  GATHER_A: a CTA
+  // takes row blocks in grid strides and walks all their column tiles, so the gathered rows are loaded once per row block.
+  const int64_t n_iter = GATHER_A ? ((int64_t)blockIdx.x < m_tiles ? (m_tiles - blockIdx.x + gridDim.x - 1) / gridDim.x * n_tiles : 0)
+                                  : ((int64_t)blockIdx.x < total ? (total - blockIdx.x + gridDim.x - 1) / gridDim.x : 0);
+  auto tile_of = [&](int64_t j, int& m_blk, int& n_blk) {
+    if (GATHER_A) {
+      m_blk = (int)(blockIdx.x + (j / n_tiles) * gridDim.x);
+      n_blk = (int)(j % n_tiles);
+    } else {
+      const int64_t tile = blockIdx.x + j * gridDim.x;
+      m_blk = (int)(tile / n_tiles);
+      n_blk = (int)(tile % n_tiles);
+    }
+  };
 
   if (warp == 0 && lane == 0) {
     prefetch_tmap(&tmA);
     prefetch_tmap(&tmB);
     for (int s = 0; s < STAGES; ++s) {
-      mbar_init(&full_bar[s], 1);
+      mbar_init(&full_bar[s], GATHER_A ? 1 + kGatherWarps : 1);
       mbar_init(&empty_bar[s], 1);
     }
     for (int s = 0; s < 2; ++s) {
@@ -221,13 +248,14 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     if (lane == 0) {
       int stage = 0;
       uint32_t phase = 0;
-      for (int64_t tile = blockIdx.x; tile < total; tile += gridDim.x) {
-        const int m_blk = (int)(tile / n_tiles), n_blk = (int)(tile % n_tiles);
+      for (int64_t j = 0; j < n_iter; ++j) {
+        int m_blk, n_blk;
+        tile_of(j, m_blk, n_blk);
         for (int kb = 0; kb < k_blocks; ++kb) {
           mbar_wait(&empty_bar[stage], phase ^ 1);
-          mbar_arrive_expect_tx(&full_bar[stage], STAGE);
+          mbar_arrive_expect_tx(&full_bar[stage], GATHER_A ? STAGE - A_BYTES : STAGE);
           uint8_t* sa = smem + stage * STAGE;
-          tma_load_2d(sa, &tmA, &full_bar[stage], kb * BK, m_blk * BM);
+          if (!GATHER_A) tma_load_2d(sa, &tmA, &full_bar[stage], kb * BK, m_blk * BM);
           tma_load_2d(sa + A_BYTES, &tmB, &full_bar[stage], kb * BK, n_blk * BN);
           if (++stage == STAGES) { stage = 0; phase ^= 1; }
         }
@@ -240,7 +268,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
       uint32_t phase = 0;
       int as = 0;
       uint32_t aphase = 0;
-      for (int64_t tile = blockIdx.x; tile < total; tile += gridDim.x) {
+      for (int64_t j = 0; j < n_iter; ++j) {
         mbar_wait(&tempty_bar[as], aphase ^ 1);
         tc_fence_after();
         const uint32_t d_tmem = tmem_base + (uint32_t)(as * BN);
@@ -260,6 +288,49 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
         if (++as == 2) { as = 0; aphase ^= 1; }
       }
     }
+  } else if (GATHER_A && warp >= 2 + kEpiWarps * SPLIT) {
+    // gather warps: one row per thread (k_blocks == 1).  The row of the NEXT row block is loaded (2 u scalar loads, packed to
+    // bf16 pairs) while the current one is written into the ring once per column tile, so no load latency is exposed.
+    const int r = (warp - 2 - kEpiWarps * SPLIT) * 32 + lane;
+    int stage = 0;
+    uint32_t phase = 0;
+    auto load_row = [&](int64_t m_blk, uint32_t (&pk)[BK / 2]) {
+      const int64_t m = m_blk * BM + r;
+      float v[BK];
+#pragma unroll
+      for (int c = 0; c < BK; ++c) v[c] = 0.f;
+      if (m_blk < m_tiles && m < M) {
+        const int64_t si = ag.src[rows.m_off + m], di = ag.dst[rows.m_off + m];
+        const float* fs = ag.feat + si * ag.u;
+        const float* fd = ag.feat + di * ag.u;
+#pragma unroll
+        for (int c = 0; c < BK / 2; ++c)
+          if (c < ag.u) v[c] = __ldg(fs + c);
+#pragma unroll
+        for (int c = 0; c < BK; ++c)
+          if (c >= ag.u && c < 2 * ag.u) v[c] = __ldg(fd + (c - ag.u));
+      }
+#pragma unroll
+      for (int c = 0; c < BK / 2; ++c) pk[c] = pack_bf16(v[2 * c], v[2 * c + 1]);
+    };
+    uint32_t cur[BK / 2], nxt[BK / 2];
+    load_row(blockIdx.x, cur);
+    for (int64_t mb = blockIdx.x; mb < m_tiles; mb += gridDim.x) {
+      load_row(mb + gridDim.x, nxt);
+      for (int nb = 0; nb < n_tiles; ++nb) {
+        mbar_wait(&empty_bar[stage], phase ^ 1);
+        uint8_t* sa = smem + stage * STAGE;
+#pragma unroll
+        for (int q = 0; q < 8; ++q)
+          *reinterpret_cast<uint4*>(sa + r * 128 + ((q ^ (r & 7)) << 4)) = make_uint4(cur[q * 4], cur[q * 4 + 1], cur[q * 4 + 2], cur[q * 4 + 3]);
+        fence_proxy_async();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&full_bar[stage]);
+        if (++stage == STAGES) { stage = 0; phase ^= 1; }
+      }
+#pragma unroll
+      for (int c = 0; c < BK / 2; ++c) cur[c] = nxt[c];
+    }
   } else {
     const int quad = warp & 3;   // TMEM lane quadrant this warp may access
     const int chalf = (warp - 2) >> 2;   // SPLIT == 2: which half of the tile's columns
@@ -267,8 +338,9 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     int as = 0;
     uint32_t aphase = 0;
     EpiShared es{store_stage + (warp - 2) * kStoreStage, &tmC, 0u};
-    for (int64_t tile = blockIdx.x; tile < total; tile += gridDim.x) {
-      const int m_blk = (int)(tile / n_tiles), n_blk = (int)(tile % n_tiles);
+    for (int64_t j = 0; j < n_iter; ++j) {
+      int m_blk, n_blk;
+      tile_of(j, m_blk, n_blk);
       mbar_wait(&tfull_bar[as], aphase);
       tc_fence_after();
       const uint32_t taddr = tmem_base + ((uint32_t)(quad * 32) << 16) + (uint32_t)(as * BN + chalf * BNE);

@@ -70,7 +70,7 @@ struct OutBf16 {
 // A [a_rows][K] bf16 (row stride lda), W [n_pad][K] bf16 K-major; rows of the product resolved on the device.
 template <int BN, class Epi>
 trk_status launch_gemm(trk_ctx* ctx, const bf16* A, int64_t a_rows, int64_t lda, int K, const bf16* W, int n_pad, tc::Rows rows,
-                       const typename Epi::Params& ep, cudaStream_t st, OutBf16 out = OutBf16()) {
+                       const typename Epi::Params& ep, cudaStream_t st, OutBf16 out = OutBf16(), const tc::AGather* ag = nullptr) {
   if (rows.m_cap <= 0) return TRK_OK;
   if (K % tc::BK != 0 || n_pad % BN != 0) return fail(ctx, TRK_ERR_SHAPE, "gemm: K must be a multiple of 64 and N of the tile");
   static bool attr_set = false;
@@ -110,6 +110,17 @@ trk_status launch_gemm(trk_ctx* ctx, const bf16* A, int64_t a_rows, int64_t lda,
   const unsigned grid = (unsigned)std::min<int64_t>(tiles, ctx->sm_count);
   if constexpr (BN == 256 && Epi::kTmaStore) {
     // a single K block per tile: the bf16-store epilogue paces the kernel, so it gets eight warps (column split)
+    if (K == tc::BK && ag && debug_knob(kKnobEpiSplit) >= 2) {
+      // ... and its A operand is gathered in the kernel (S3 first layer: no separate gather launch, no staging buffer)
+      static bool attr4_set = false;
+      auto kern4 = tc::gemm_tc_kernel<BN, Epi, 2, true>;
+      if (!attr4_set) {
+        TRK_CUDA(ctx, cudaFuncSetAttribute(kern4, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::smem_bytes(BN, true, 2)));
+        attr4_set = true;
+      }
+      TRK_LAUNCH(ctx, kern4, grid, tc::threads_for(2, true), tc::smem_bytes(BN, true, 2), st, ta, tb, tc_out, rows, n_tiles, K / tc::BK, ep, *ag);
+      return TRK_OK;
+    }
     if (K == tc::BK && debug_knob(kKnobEpiSplit) != 0) {
       static bool attr3_set = false;
       auto kern3 = tc::gemm_tc_kernel<BN, Epi, 2>;
@@ -117,11 +128,11 @@ trk_status launch_gemm(trk_ctx* ctx, const bf16* A, int64_t a_rows, int64_t lda,
         TRK_CUDA(ctx, cudaFuncSetAttribute(kern3, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::smem_bytes(BN, true, 2)));
         attr3_set = true;
       }
-      TRK_LAUNCH(ctx, kern3, grid, tc::threads_for(2), tc::smem_bytes(BN, true, 2), st, ta, tb, tc_out, rows, n_tiles, K / tc::BK, ep);
+      TRK_LAUNCH(ctx, kern3, grid, tc::threads_for(2), tc::smem_bytes(BN, true, 2), st, ta, tb, tc_out, rows, n_tiles, K / tc::BK, ep, tc::AGather{});
       return TRK_OK;
     }
   }
-  TRK_LAUNCH(ctx, kern, grid, tc::kThreads, tc::smem_bytes(BN, Epi::kTmaStore), st, ta, tb, tc_out, rows, n_tiles, K / tc::BK, ep);
+  TRK_LAUNCH(ctx, kern, grid, tc::kThreads, tc::smem_bytes(BN, Epi::kTmaStore), st, ta, tb, tc_out, rows, n_tiles, K / tc::BK, ep, tc::AGather{});
   return TRK_OK;
 }
 
@@ -129,11 +140,11 @@ int pick_bn(int n_pad) { return n_pad % 256 == 0 ? 256 : (n_pad % 128 == 0 ? 128
 
 // out: bf16 [out_rows][ldo]; every 128-row tile that holds a valid row is written in full (rows beyond out_rows are clipped).
 trk_status gemm_bias_act(trk_ctx* ctx, const bf16* A, int64_t a_rows, int64_t lda, const DevLinear& L, bf16* out, int64_t out_rows,
-                         int ldo, int relu, tc::Rows rows, cudaStream_t st) {
+                         int ldo, int relu, tc::Rows rows, cudaStream_t st, const tc::AGather* ag = nullptr) {
   tc::EpiBiasActBf16::Params ep{L.b_f32, relu};
   const OutBf16 o{out, out_rows, ldo};
   switch (pick_bn(L.out_pad)) {
-    case 256: return launch_gemm<256, tc::EpiBiasActBf16>(ctx, A, a_rows, lda, L.in_pad, L.w_bf16, L.out_pad, rows, ep, st, o);
+    case 256: return launch_gemm<256, tc::EpiBiasActBf16>(ctx, A, a_rows, lda, L.in_pad, L.w_bf16, L.out_pad, rows, ep, st, o, ag);
     case 128: return launch_gemm<128, tc::EpiBiasActBf16>(ctx, A, a_rows, lda, L.in_pad, L.w_bf16, L.out_pad, rows, ep, st, o);
     default: return launch_gemm<64, tc::EpiBiasActBf16>(ctx, A, a_rows, lda, L.in_pad, L.w_bf16, L.out_pad, rows, ep, st, o);
   }
@@ -423,7 +434,11 @@ trk_status filter_forward_bf16(trk_ctx* ctx, const float* feat, const int32_t* s
   for (int64_t off = 0; off < n_edges_cap; off += ctx->filter_chunk) {
     const int64_t cap = std::min<int64_t>(ctx->filter_chunk, n_edges_cap - off);
     tc::Rows rows{n_edges_dev, off, cap};
-    TRK_LAUNCH(ctx, filter_gather_kernel, (unsigned)ceil_div(cap * 8, 256), 256, 0, st, feat, u, src, dst, n_edges_dev, off, cap, gin);
+    // first layer with 256-column tiles: its A operand is gathered inside the GEMM (gemm_tc.cuh GATHER_A)
+    const bool fuse_gather = nl >= 3 && pick_bn(L[0].out_pad) == 256 && debug_knob(kKnobEpiSplit) >= 2;
+    const tc::AGather ag{feat, src, dst, u};
+    if (!fuse_gather)
+      TRK_LAUNCH(ctx, filter_gather_kernel, (unsigned)ceil_div(cap * 8, 256), 256, 0, st, feat, u, src, dst, n_edges_dev, off, cap, gin);
     const bf16* in = gin;
     int64_t in_rows = ctx->filter_chunk;
     int cur = 0;
@@ -452,7 +467,8 @@ trk_status filter_forward_bf16(trk_ctx* ctx, const float* feat, const int32_t* s
       if (l == nl - 2) {
         TRK_TRY(gemm_relu_dot(ctx, in, in_rows, lda, Ll, L[nl - 1].w_f32, ctx->partial, &n_tiles, rows, st));
       } else {
-        TRK_TRY(gemm_bias_act(ctx, in, in_rows, lda, Ll, bufs[cur], ctx->act_rows, Ll.out_pad, 1, rows, st));
+        TRK_TRY(gemm_bias_act(ctx, in, in_rows, lda, Ll, bufs[cur], ctx->act_rows, Ll.out_pad, 1, rows, st,
+                              l == 0 && fuse_gather ? &ag : nullptr));
         in = bufs[cur];
         in_rows = ctx->act_rows;
         cur ^= 1;
