@@ -391,6 +391,9 @@ def main():
     s4 = stage_roofline["s4_gnn"]
     s4["hbm_view"] = {"achieved_gbs": gnn_bytes(n, e_k, cfg["gnn_hidden"], cfg["gnn_iters"]) / (st["s4_gnn"] * 1e-3) / 1e9}
     s4["hbm_view"]["frac_of_measured"] = s4["hbm_view"]["achieved_gbs"] / hbm
+    stage_roofline["s2_frnn"]["note"] = ("nominally HBM; really instruction-issue bound (tables live in L2/L1, no DRAM traffic): "
+                                         "ncu issue 63 %, profiles/r1_full_v4.md")
+    stage_roofline["s5_cc"]["note"] = "nominally HBM; really bound by the latency of atomics on the L2-resident parent array"
     s4["note"] = "on the tensor/HBM ridge: the flop count is the split-first-layer minimum, the byte count the bf16-state minimum"
     for k, v in stage_roofline.items():
         v["ms"] = st[k]
