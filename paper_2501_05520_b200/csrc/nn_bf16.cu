@@ -280,25 +280,39 @@ embed_first_layer_kernel(const float* __restrict__ hits, const float* __restrict
   }
 }
 
-// S3 input rows: out[m][0..64) = bf16([feat[src] ; feat[dst]]) zero padded; 8 columns per thread.
-__global__ void filter_gather_kernel(const float* __restrict__ feat, int u, const int32_t* __restrict__ src,
+// S3 input rows: out[m][0..2u) = bf16([feat[src] ; feat[dst]]); 8 columns per thread, 2^cpr_log2 threads per row cover the
+// 16-byte chunks that hold data.  Columns [2u, 64) are the zero padding of K: the buffer is zeroed once in trk_create and
+// nothing ever writes there.  Rows beyond M keep stale (finite) values; no result of theirs is ever read.
+__global__ void filter_gather_kernel(const float* __restrict__ feat, int u, int cpr_log2, const int32_t* __restrict__ src,
                                      const int32_t* __restrict__ dst, const int32_t* __restrict__ m_dev, int64_t m_off, int64_t m_cap,
                                      bf16* __restrict__ out) {
   const int64_t M = rows_of(m_dev, m_off, m_cap);
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  const int64_t row = i >> 3;
-  if (row >= m_cap) return;
-  const int c0 = (int)(i & 7) * 8;
+  const int64_t row = i >> cpr_log2;
+  const int c0 = (int)(i & ((1 << cpr_log2) - 1)) * 8;
+  if (row >= M || c0 >= 2 * u) return;
   float v[8];
 #pragma unroll
   for (int j = 0; j < 8; ++j) v[j] = 0.f;
-  if (row < M) {
+  {
     const int64_t s = src[m_off + row], d = dst[m_off + row];
+    if ((u & 3) == 0 && (reinterpret_cast<uintptr_t>(feat) & 15) == 0) {
+      // rows of feat are 16-byte aligned: the thread's eight columns are two float4 pieces, each from one endpoint
 #pragma unroll
-    for (int j = 0; j < 8; ++j) {
-      const int c = c0 + j;
-      if (c < u) v[j] = feat[s * u + c];
-      else if (c < 2 * u) v[j] = feat[d * u + (c - u)];
+      for (int h = 0; h < 2; ++h) {
+        const int c = c0 + 4 * h;
+        if (c < 2 * u) {
+          const float4 x = __ldg(reinterpret_cast<const float4*>(c < u ? feat + s * u + c : feat + d * u + (c - u)));
+          v[4 * h] = x.x; v[4 * h + 1] = x.y; v[4 * h + 2] = x.z; v[4 * h + 3] = x.w;
+        }
+      }
+    } else {
+#pragma unroll
+      for (int j = 0; j < 8; ++j) {
+        const int c = c0 + j;
+        if (c < u) v[j] = feat[s * u + c];
+        else if (c < 2 * u) v[j] = feat[d * u + (c - u)];
+      }
     }
   }
   *reinterpret_cast<uint4*>(out + row * 64 + c0) =
@@ -435,10 +449,13 @@ trk_status filter_forward_bf16(trk_ctx* ctx, const float* feat, const int32_t* s
     const int64_t cap = std::min<int64_t>(ctx->filter_chunk, n_edges_cap - off);
     tc::Rows rows{n_edges_dev, off, cap};
     // first layer with 256-column tiles: its A operand is gathered inside the GEMM (gemm_tc.cuh GATHER_A)
+    int cpr_log2 = 0;                                   // threads per gathered row: the 16-byte chunks that hold data, rounded up to 2^k
+    while ((8 << cpr_log2) < 2 * u) ++cpr_log2;
     const bool fuse_gather = nl >= 3 && pick_bn(L[0].out_pad) == 256 && debug_knob(kKnobEpiSplit) >= 2;
     const tc::AGather ag{feat, src, dst, u};
     if (!fuse_gather)
-      TRK_LAUNCH(ctx, filter_gather_kernel, (unsigned)ceil_div(cap * 8, 256), 256, 0, st, feat, u, src, dst, n_edges_dev, off, cap, gin);
+      TRK_LAUNCH(ctx, filter_gather_kernel, (unsigned)ceil_div(cap << cpr_log2, 256), 256, 0, st, feat, u, cpr_log2, src, dst, n_edges_dev,
+                 off, cap, gin);
     const bf16* in = gin;
     int64_t in_rows = ctx->filter_chunk;
     int cur = 0;
