@@ -25,9 +25,9 @@ if ROOT not in sys.path:
 
 FILTER_FLOP_PER_EDGE = 2 * (24 * 1024 + 1024 * 1024 * 2 + 1024)          # 4 245 504
 EMBED_FLOP_PER_HIT = 2 * (3 * 1024 + 1024 * 1024 * 2 + 1024 * 12)        # 4 225 024
-# DRAM bytes of one full-chunk launch (303 104 rows) of the dominant kernel, from the ncu --set full capture summarised in
-# profiles/r1_full_v2.md (dram__bytes_read.sum + dram__bytes_write.sum)
-NCU_TRAFFIC_BYTES = {"bias_act": 622.89e6 + 580.31e6, "relu_dot": 622.89e6 + 7.75e6}
+# DRAM bytes of one full-chunk launch (1 212 416 rows) of the dominant kernel, from the ncu --set full capture summarised in
+# profiles/r1_full_v6.md (dram__bytes_read.sum + dram__bytes_write.sum)
+NCU_TRAFFIC_BYTES = {"bias_act": 2578.13e6 + 2441.02e6, "relu_dot": 2490.36e6 + 23.02e6}
 
 
 def gnn_flops(n, e, H=128, T=8):
@@ -415,11 +415,11 @@ def main():
                 "launches_timed": k_n, "avg_launch_ms": k_ms / max(1, k_n), "flop_per_full_launch": 2.0 * chunk_rows * width * width,
                 "how": "algorithmic flops of the non-empty launches (2 x rows x 1024 x 1024 each) / their summed durations, CUDA-event pairs "
                        "around each launch on the launch stream inside the timed steps (trk_profile_kernel_ms)",
-                # ncu --set full, profiles/r1_full_v2.md: dram__bytes_read.sum + dram__bytes_write.sum of one full-chunk launch
+                # ncu --set full, profiles/r1_full_v6.md: dram__bytes_read.sum + dram__bytes_write.sum of one full-chunk launch
                 "traffic": NCU_TRAFFIC_BYTES["bias_act"], "traffic_unit": "bytes per full-chunk launch (EpiBiasActBf16 variant)",
                 "traffic_detail": dict(NCU_TRAFFIC_BYTES, algorithmic_bias_act=2 * chunk_rows * width * 2 + width * width * 2,
                                        algorithmic_relu_dot=chunk_rows * width * 2 + width * width * 2 + chunk_rows * 16,
-                                       source="profiles/r1_full_v2.md"),
+                                       source="profiles/r1_full_v6.md"),
                 "whole_stage": {"achieved": s3_tflops, "frac": s3_tflops / peaks["bf16_sustained"],
                                 "how": "algorithmic flops of S3 (E_c x 4 245 504) / S3 stage time (gather, 3 GEMMs, finish, compaction)"},
                 "isolated_launch": {"shape": [m_chunk, 1024, 1024], "ms": iso_ms, "achieved": iso_tflops,

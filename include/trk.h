@@ -215,6 +215,9 @@ trk_status trk_gemm_bf16(const void* a, const void* w, const float* bias, void* 
  *                filter MLP) run their epilogue on eight warps (two per TMEM lane quadrant); 2: in addition that layer's input
  *                rows [e_src ; e_dst] are gathered inside the GEMM kernel instead of by a separate launch (measured slower on
  *                the pileup-200 event: 1.36 ms against 1.01 + 0.25 ms, so not the default); 0: four warps.
+ *   "gemm_row_major"  16 (default): a CTA pair of the pair GEMM walks all column tiles of one row block before the next row
+ *                block when there are at least 16 row blocks per pair (A rows re-read from L2, no DRAM re-reads); 0: tiles in
+ *                pair strides, column fastest.
  * Returns TRK_ERR_INVALID_ARG for an unknown key.  Not thread safe against running trk_* calls. */
 trk_status trk_debug_set(const char* key, int64_t value);
 

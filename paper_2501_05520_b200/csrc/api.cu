@@ -24,7 +24,7 @@ trk_status fail(trk_ctx* ctx, trk_status s, const std::string& msg) {
   return s;
 }
 
-static int64_t g_knobs[kKnobCount] = {1, 4, 1, 0, 0, 0, 0, 0};
+static int64_t g_knobs[kKnobCount] = {1, 4, 1, 16, 0, 0, 0, 0};
 int64_t debug_knob(int which) { return g_knobs[which]; }
 
 trk_status gemm_bf16_hook(trk_ctx* ctx, const void* a, const void* w, const float* bias, void* out, int64_t m, int n, int k, int relu,
@@ -642,6 +642,7 @@ trk_status trk_debug_set(const char* key, int64_t value) {
   if (std::strcmp(key, "gemm_pair") == 0) { g_knobs[kKnobGemmPair] = value; return TRK_OK; }
   if (std::strcmp(key, "gnn_fused") == 0) { g_knobs[kKnobGnnFused] = value; return TRK_OK; }
   if (std::strcmp(key, "epi_split") == 0) { g_knobs[kKnobEpiSplit] = value; return TRK_OK; }
+  if (std::strcmp(key, "gemm_row_major") == 0) { g_knobs[kKnobRowMajor] = value; return TRK_OK; }
   return fail(nullptr, TRK_ERR_INVALID_ARG, std::string("trk_debug_set: unknown key ") + key);
 }
 

@@ -13,11 +13,12 @@ __global__ void cc_init_kernel(int32_t* __restrict__ parent, int64_t n, int32_t*
 }
 
 __device__ __forceinline__ int32_t find_root(int32_t* parent, int32_t x) {
-  // path halving with plain stores: every value ever stored is an ancestor, hence valid and smaller
+  // path halving with plain stores: every value ever stored is an ancestor of x (links are only ever added at roots and
+  // point to smaller indices), hence valid whatever the interleaving; only the hook below needs an atomic
   int32_t p = ((volatile int32_t*)parent)[x];
   while (p != x) {
     int32_t gp = ((volatile int32_t*)parent)[p];
-    if (gp != p) atomicMin(&parent[x], gp);
+    if (gp != p) ((volatile int32_t*)parent)[x] = gp;
     x = p;
     p = gp;
   }

@@ -15,7 +15,8 @@ namespace trk {
 constexpr int kMaxEmbDim = 16;      // d_e is padded to a multiple of 4, at most 16
 constexpr int kMaxEvents = 1024;    // event offsets travel as a kernel parameter
 constexpr int64_t kMaxCells = 1 << 21;  // FRNN grid cells summed over the events of a call
-constexpr int kFilterChunkRows = 128 * 148 * 16;  // S3 rows per pass (upper bound; ctx->filter_chunk is the per-context value)
+constexpr int kFilterChunkRows = 128 * 148 * 64;  // S3 rows per pass (upper bound; ctx->filter_chunk is the per-context value):
+                                                  // 2.5 GB per activation buffer buys 5 launches per 1.2 M candidate edges
 
 // One Linear layer resident on the device.
 struct DevLinear {
@@ -170,7 +171,7 @@ trk_status fail(trk_ctx* ctx, trk_status s, const std::string& msg);
 inline int64_t ceil_div(int64_t a, int64_t b) { return (a + b - 1) / b; }
 
 // ---- tuning / test knobs (trk_debug_set) ----
-enum { kKnobGemmPair = 0, kKnobGnnFused = 1, kKnobEpiSplit = 2, kKnobCount = 8 };
+enum { kKnobGemmPair = 0, kKnobGnnFused = 1, kKnobEpiSplit = 2, kKnobRowMajor = 3, kKnobCount = 8 };
 int64_t debug_knob(int which);
 
 // ---- util_kernels.cu ----

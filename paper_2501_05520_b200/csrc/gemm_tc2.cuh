@@ -98,7 +98,7 @@ constexpr int smem_bytes_pair(int bn, bool tma_store = false) {
 template <int BN, class Epi>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
 gemm_tc2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, const __grid_constant__ CUtensorMap tmC,
-                Rows rows, int n_tiles, int k_blocks, typename Epi::Params ep) {
+                Rows rows, int n_tiles, int k_blocks, typename Epi::Params ep, int row_major_min) {
   constexpr int STAGES = num_stages_pair(BN);
   constexpr int A_BYTES = BM * BK * 2;
   constexpr int STAGE = stage_bytes_pair(BN);
@@ -117,7 +117,25 @@ gemm_tc2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
   const bool leader = rank == 0;
   const int pair = blockIdx.x >> 1, n_pairs = gridDim.x >> 1;
   const int64_t M = resolve_rows(rows);
-  const int64_t total = ((M + kPairBM - 1) / kPairBM) * n_tiles;
+  const int64_t m_tiles = (M + kPairBM - 1) / kPairBM;
+  const int64_t total = m_tiles * n_tiles;
+  // This pair's j-th tile.  With many row blocks a pair walks all column tiles of one row block before it takes the next
+  // (its A rows are re-read from L2 a few microseconds apart: ncu showed 1.37x the algorithmic DRAM reads when the column
+  // tiles of a row block were spread over four pairs that drift apart during a 1.7 ms launch); with few row blocks the
+  // tiles are dealt out in pair strides so that every pair has work.
+  const bool row_major = row_major_min > 0 && m_tiles >= (int64_t)row_major_min * n_pairs;   // imbalance <= 1 / row_major_min
+  const int64_t n_iter = row_major ? (pair < m_tiles ? (m_tiles - pair + n_pairs - 1) / n_pairs * n_tiles : 0)
+                                   : (pair < total ? (total - pair + n_pairs - 1) / n_pairs : 0);
+  auto tile_of = [&](int64_t j, int& m_blk, int& n_blk) {
+    if (row_major) {
+      m_blk = (int)(pair + (j / n_tiles) * n_pairs);
+      n_blk = (int)(j % n_tiles);
+    } else {
+      const int64_t tile = pair + j * n_pairs;
+      m_blk = (int)(tile / n_tiles);
+      n_blk = (int)(tile % n_tiles);
+    }
+  };
 
   if (warp == 0 && lane == 0) {
     prefetch_tmap(&tmA);
@@ -142,8 +160,9 @@ gemm_tc2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
     if (lane == 0) {
       int stage = 0;
       uint32_t phase = 0;
-      for (int64_t tile = pair; tile < total; tile += n_pairs) {
-        const int m_blk = (int)(tile / n_tiles), n_blk = (int)(tile % n_tiles);
+      for (int64_t j = 0; j < n_iter; ++j) {
+        int m_blk, n_blk;
+        tile_of(j, m_blk, n_blk);
         for (int kb = 0; kb < k_blocks; ++kb) {
           mbar_wait(&empty_bar[stage], phase ^ 1);
           if (leader) mbar_arrive_expect_tx(&full_bar[stage], 2 * STAGE);
@@ -162,7 +181,7 @@ gemm_tc2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
       uint32_t phase = 0;
       int as = 0;
       uint32_t aphase = 0;
-      for (int64_t tile = pair; tile < total; tile += n_pairs) {
+      for (int64_t j = 0; j < n_iter; ++j) {
         mbar_wait_cluster(&tempty_bar[as], aphase ^ 1);
         tc_fence_after();
         const uint32_t d_tmem = tmem_base + (uint32_t)(as * BN);
@@ -189,8 +208,9 @@ gemm_tc2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
     EpiShared es{store_stage + (warp - 2) * kStoreStage, &tmC, 0u};
     const uint32_t tempty_leader0 = mapa_u32(smem_u32(&tempty_bar[0]), 0);
     const uint32_t tempty_leader1 = mapa_u32(smem_u32(&tempty_bar[1]), 0);
-    for (int64_t tile = pair; tile < total; tile += n_pairs) {
-      const int m_blk = (int)(tile / n_tiles), n_blk = (int)(tile % n_tiles);
+    for (int64_t j = 0; j < n_iter; ++j) {
+      int m_blk, n_blk;
+      tile_of(j, m_blk, n_blk);
       mbar_wait(&tfull_bar[as], aphase);
       tc_fence_after();
       const uint32_t taddr = tmem_base + ((uint32_t)(quad * 32) << 16) + (uint32_t)(as * BN);

@@ -2,7 +2,7 @@
 // (gemm_tc.cuh); layers whose K is 3 or 4 run on the plain ALUs in fp32 (they are <0.1% of the flops).
 //
 // S1   hits -> [SIMT 3->W] -> GEMM+ReLU ... -> GEMM (N padded to 16, fp32 out) = embedding
-// S3   per chunk of 18944 edges (one 128-row tile per SM and N-tile column, activations L2 resident):
+// S3   per chunk of ctx->filter_chunk edges (up to 64 row tiles per SM; the activations of a chunk stream through HBM):
 //        gather [e_src ; e_dst] -> bf16 [rows][64] (K zero-padded) -> GEMM+ReLU ... -> last hidden GEMM
 //        with the final Linear(W->1) folded into its epilogue as per-tile partial dots -> sigmoid
 // S4   the first layer of edge_net / edge_dec is split exactly:
@@ -102,7 +102,8 @@ trk_status launch_gemm(trk_ctx* ctx, const bf16* A, int64_t a_rows, int64_t lda,
       }
       const int64_t ptiles = ceil_div(rows.m_cap, tc::kPairBM) * n_tiles;
       const unsigned grid2 = 2u * (unsigned)std::min<int64_t>(ptiles, ctx->sm_count / 2);
-      TRK_LAUNCH(ctx, kern2, grid2, tc::kThreads, tc::smem_bytes_pair(BN, Epi::kTmaStore), st, ta, tb, tc_out, rows, n_tiles, K / tc::BK, ep);
+      TRK_LAUNCH(ctx, kern2, grid2, tc::kThreads, tc::smem_bytes_pair(BN, Epi::kTmaStore), st, ta, tb, tc_out, rows, n_tiles, K / tc::BK, ep,
+                 (int)debug_knob(kKnobRowMajor));
       return TRK_OK;
     }
   }

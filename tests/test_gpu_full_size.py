@@ -1,5 +1,5 @@
 """-m gpu parity at BASELINE.json's FULL sizes (configs[2] pileup-200, configs[3] 16-event batch, configs[4] pileup-300),
-in the launch configuration bench.py times (one context sized for the whole event, 303 104-row filter chunks, CTA-pair
+in the launch configuration bench.py times (one context sized for the whole event, 1 212 416-row filter chunks, CTA-pair
 GEMMs, fused edge kernel).  Every stage is fed inputs that come from the oracle or from synth/ only.
 
 What is compared, per config (oracle cost on the box's host cores in brackets):
@@ -109,7 +109,7 @@ class Full:
             src, dst, _ = self.cand
             e = len(src)
             idx = np.unique((Stream(7, f"sample:{self.name}").uniform(np.arange(N_SAMPLE, dtype=np.uint64)) * e).astype(np.int64))
-            idx = np.unique(np.concatenate([idx, [0, e - 1], np.arange(303104 - 64, 303104 + 64) % e]))   # chunk seam of S3
+            idx = np.unique(np.concatenate([idx, [0, e - 1], np.arange(1212416 - 64, 1212416 + 64) % e]))   # chunk seam of S3
             return idx, s3_filter.filter_scores(self.emb, src[idx], dst[idx], self.model["filter"]).astype(np.float32)
         return self._memo("filter_sample", f)
 

@@ -141,7 +141,7 @@ def test_paper_s3_scores_sampled_and_compaction(paper):
     gpu = score.cpu().numpy()
     assert np.all(np.isfinite(gpu))
     idx = np.unique((Stream(7, "sample:paper350k").uniform(np.arange(20000, dtype=np.uint64)) * e).astype(np.int64))
-    seams = np.concatenate([np.arange(c * 303104 - 32, c * 303104 + 32) for c in range(1, e // 303104 + 1)])
+    seams = np.concatenate([np.arange(c * 1212416 - 32, c * 1212416 + 32) for c in range(1, e // 1212416 + 1)])
     idx = np.unique(np.concatenate([idx, [0, e - 1], seams[seams < e]]))
     ref = s3_filter.filter_scores(p.emb, osrc[idx], odst[idx], p.model["filter"]).astype(np.float32)
     G.check_scores(gpu[idx], ref, "bf16", f"filter score ({len(idx)} sampled edges)")
