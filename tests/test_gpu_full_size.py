@@ -281,3 +281,12 @@ def test_full_infer_invariants(full):
     jac = len(np.intersect1d(gkeys, okeys)) / len(np.union1d(gkeys, okeys))
     print(f"{f.name}: E_c={ec} E_k={ek} E_t={et}; candidate-edge Jaccard vs oracle {jac:.4f}")
     assert jac > 0.9
+    # run-to-run identity at full size: no atomics on floats, fixed summation orders, and the in-kernel
+    # exchanges of the fused S4 kernels are race free -- three more calls give the same bits
+    first = {k: res[k].clone() for k in ("labels", "counts", "edge_score", "cand_score")}
+    for _ in range(3):
+        again = trk.infer(_dev(f.hits), f.off, want_edges=True, want_cand=True)
+        torch.cuda.synchronize()
+        assert torch.equal(again["counts"], first["counts"]) and torch.equal(again["labels"], first["labels"])
+        assert torch.equal(again["edge_score"][:ek], first["edge_score"][:ek])
+        assert torch.equal(again["cand_score"][:ec], first["cand_score"][:ec])
