@@ -5,8 +5,9 @@
 //   * a thread reads 64 accumulator columns, adds the bias, forms the partial (sum, sum of squares) of its half row and
 //     exchanges it with the thread that holds the other half through shared memory (named barriers of 64 threads);
 //     variance = E[x^2] - mean^2 in fp32 (the values are LayerNorm-scale, no cancellation problem);
-//   * no extra shared memory: epilogue 1 exchanges inside its own rows of the T buffer before it writes them, epilogue 2
-//     inside the first 16-byte cell of its row of the residual tile (the cell's residual values wait in registers);
+//   * 1 KB of extra shared memory: in epilogue 1 the upper half sends its statistics to the lower half through one float2
+//     per row and reads the LayerNorm coefficients back from the same slot; epilogue 2 exchanges inside the first 16-byte
+//     cell of its row of the residual tile (the cell's residual values wait in registers);
 //   * 22 warps (704 threads, 88 registers): 0 TMA, 1 MMA issuer, 2-5 gather (four warps: a warp keeps only a few cp.async
 //     in flight, so the gather scales with their number), 6-13 epilogue 1, 14-21 epilogue 2;
 //   * dynamic shared memory is declared 1024-byte aligned (no manual alignment slack; checked at kernel start).
@@ -40,7 +41,8 @@ constexpr int kOffEOp = kOffRing + 4 * kKB;     // 2 K blocks: the e tile as lay
 constexpr int kOffRes = kOffEOp + 2 * kKB;      // 2 K blocks: the e tile as residual, overwritten in place and stored
 constexpr int kOffT = kOffRes + 2 * kKB;        // 2 K blocks: layer-1 output
 constexpr int kOffVec = kOffT + 2 * kKB;        // b1, b2, w_out: 3 x 128 fp32
-constexpr int kOffBar = kOffVec + 3 * kH * 4;
+constexpr int kOffX1 = kOffVec + 3 * kH * 4;     // epilogue 1: one float2 per row, half-row statistics one way, coefficients back
+constexpr int kOffBar = kOffX1 + kTileRows * 8;
 constexpr int kSmemFused4 = kOffBar + 256;
 static_assert(kSmemFused4 <= 232448, "shared memory budget of one CTA");
 
@@ -315,9 +317,8 @@ gnn_edge_fused4_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_co
     const int bid = 1 + quad;         // named barrier of the two warps that share this quadrant's rows
     const uint32_t a1empty0 = mapa_u32(smem_u32(&bar->a1empty[0]), 0), a1empty1 = mapa_u32(smem_u32(&bar->a1empty[1]), 0);
     const uint32_t tfull_l = mapa_u32(smem_u32(&bar->tfull), 0);
-    // exchange slots inside this quadrant's own rows of T (K block 0: statistics, K block 1: the decoder's partial dots)
-    float2* xs = reinterpret_cast<float2*>(smem + kOffT + quad * 32 * 128);
-    float* xd = reinterpret_cast<float*>(smem + kOffT + kKB + quad * 32 * 128);
+    float2* slot = reinterpret_cast<float2*>(smem + kOffX1) + r;
+    float* xd = reinterpret_cast<float*>(smem + kOffT + kKB + quad * 32 * 128);   // kDecode only (T is unused there)
     for (int tl = 0; tl < n_my; ++tl) {
       const int64_t tile = pair + (int64_t)tl * n_pairs;
       const int b = tl & 1;
@@ -330,12 +331,20 @@ gnn_edge_fused4_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_co
       tc_fence_before();
       __syncwarp();
       if (lane == 0) mbar_arrive_remote(b == 0 ? a1empty0 : a1empty1);     // the accumulator is in registers now
-      if (kTwoLayers) FPW(1, mbar_wait(&bar->tempty, (uint32_t)(tl & 1) ^ 1));   // the layer-2 MMA of the previous tile has read T
-      xs[half * 32 + lane] = f2(ps, pq);
-      named_bar_sync(bid, 64);
-      const float2 other = xs[(half ^ 1) * 32 + lane];
+      // upper half -> lower half: (sum, sum of squares); lower half -> upper half: (rstd, -mean rstd)
       float2 rs, sh;
-      ln_coeffs(ps, pq, other, p.use_ln, rs, sh);
+      if (half == 1) *slot = f2(ps, pq);
+      named_bar_sync(bid, 64);
+      if (half == 0) {
+        ln_coeffs(ps, pq, *slot, p.use_ln, rs, sh);
+        *slot = f2(rs.x, sh.x);
+      }
+      named_bar_sync(bid, 64);
+      if (half == 1) {
+        const float2 c = *slot;
+        rs = f2(c.x, c.x);
+        sh = f2(c.y, c.y);
+      }
       if (MODE == gf::kDecode) {
         float2 d0 = f2(0.f, 0.f), d1 = d0;
         const float4* w4 = reinterpret_cast<const float4*>(swo + half * 64);
@@ -349,14 +358,14 @@ gnn_edge_fused4_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_co
         }
         const float d = (d0.x + d0.y) + (d1.x + d1.y);
         if (half == 1) xd[lane] = d;
-        named_bar_sync(bid, 64);          // also: both warps have read this tile's statistics slots
+        named_bar_sync(bid, 64);
         if (half == 0) {
           const int64_t row = tile * 2 * kTileRows + rank * kTileRows + r;
           if (row < M) p.score[row] = fast_sigmoid(p.b_out + d + xd[lane]);
         }
         named_bar_sync(bid, 64);          // the partial dot has been read: the slot may be rewritten for the next tile
       } else {
-        named_bar_sync(bid, 64);          // both warps have read the slots: the rows of T may be written
+        FPW(1, mbar_wait(&bar->tempty, (uint32_t)(tl & 1) ^ 1));   // the layer-2 MMA of the previous tile has read T
 #pragma unroll
         for (int c = 0; c < 64; c += 8) {                  // 8 columns = one 16-byte chunk of the swizzled K block `half`
           uint32_t w[4];
