@@ -44,6 +44,12 @@ CONFIGS = {
                       embed_dims=_BIG_EMBED, filter_dims=_BIG_FILTER, filter_input="emb",
                       degree=48, frnn_k=128, keep_frac=2.5e6 / 8.0e6, gnn_hidden=128, gnn_iters=8, gnn_cut=0.5,
                       calibration="pileup300"),
+    # SURVEY.md section 8(c) reading C-2, secondary "size-matched" run of configs[2]: BASELINE.json's nominal ~110 k hits need
+    # 13 600 particles with the literal geometry (7.3 hits per particle); same architecture, its own calibrated radius and cut
+    "pileup200_nominal": dict(n_particles=13600, noise_frac=0.10, seeds=[0], weight_seed=0, precision="bf16",
+                              embed_dims=_BIG_EMBED, filter_dims=_BIG_FILTER, filter_input="emb",
+                              degree=32, frnn_k=64, keep_frac=1.0e6 / 3.5e6, gnn_hidden=128, gnn_iters=8, gnn_cut=0.5,
+                              calibration="pileup200_nominal"),
     # an event of the paper's own size (~350 k spacepoints per ttbar
     # <mu>=200 event), same detector, generator and architecture as pileup-200; 43 500 particles x 7.3 hits x 1.10 noise
     "paper350k": dict(n_particles=43500, noise_frac=0.10, seeds=[0], weight_seed=0, precision="bf16",
