@@ -172,7 +172,7 @@ frnn_search_kernel(const float* __restrict__ semb, const float4* __restrict__ sm
   __shared__ unsigned long long s_d2[kWarpsPerBlock][CAP];
   __shared__ int s_idx[kWarpsPerBlock][CAP];
   __shared__ int s_queue[kWarpsPerBlock][64];
-  __shared__ int s_queue0[kWarpsPerBlock][64];
+  __shared__ int s_queue0[kWarpsPerBlock][128];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int64_t q = (int64_t)blockIdx.x * kWarpsPerBlock + warp;
   if (q >= n) return;
@@ -200,8 +200,9 @@ frnn_search_kernel(const float* __restrict__ semb, const float4* __restrict__ sm
   }
 
   int count = 0;  // warp-uniform number of buffered neighbours
-  int qn = 0;     // warp-uniform number of queued level-1 survivors
-  int qn0 = 0;    // warp-uniform number of queued level-0 survivors
+  // both queues are rings (64 and 128 entries): entry i lives at (head + i) & (size - 1), so draining moves nothing
+  int qn = 0, qh = 0;     // warp-uniform number / head of queued level-1 survivors
+  int qn0 = 0, qh0 = 0;   // warp-uniform number / head of queued level-0 survivors
   // Thresholds shrink once K neighbours are known: after a prune the K-th smallest d2 so far bounds every later accept
   // (a candidate with a larger d2 can never enter the K nearest; equal d2 is kept and settled by the (d2, j) order).
   double r2 = r2_in;
@@ -225,7 +226,7 @@ frnn_search_kernel(const float* __restrict__ semb, const float4* __restrict__ sm
     double d2 = 0.0;
     int c_i = 0;
     if (lane < take) {
-      const int pos = queue[lane];
+      const int pos = queue[(qh + lane) & 63];
       const float4 cm = smeta[pos];
       c_i = __float_as_int(cm.z);
       // outer(i,j): (r_i, |z_i|, i) < (r_j, |z_j|, j)
@@ -244,11 +245,7 @@ frnn_search_kernel(const float* __restrict__ semb, const float4* __restrict__ sm
         ok = d2 <= r2;
       }
     }
-    __syncwarp();
-    if (qn > 32 && lane < qn - 32) {   // keep the tail of the queue
-      const int moved = queue[32 + lane];
-      queue[lane] = moved;
-    }
+    qh = (qh + take) & 63;
     qn -= take;
     const unsigned m = __ballot_sync(0xffffffffu, ok);
     if (m) {
@@ -276,7 +273,7 @@ frnn_search_kernel(const float* __restrict__ semb, const float4* __restrict__ sm
     bool pre = false;
     int pos = 0;
     if (lane < take) {
-      pos = queue0[lane];
+      pos = queue0[(qh0 + lane) & 127];
       const float4* ce = reinterpret_cast<const float4*>(semb + (int64_t)pos * D);
       float d2f = 0.f;
 #pragma unroll
@@ -290,15 +287,11 @@ frnn_search_kernel(const float* __restrict__ semb, const float4* __restrict__ sm
       }
       pre = d2f <= r2_loose;
     }
-    __syncwarp();
-    if (qn0 > 32 && lane < qn0 - 32) {   // keep the tail of the queue
-      const int moved = queue0[32 + lane];
-      queue0[lane] = moved;
-    }
+    qh0 = (qh0 + take) & 127;
     qn0 -= take;
     const unsigned m = __ballot_sync(0xffffffffu, pre);
     if (m) {
-      if (pre) queue[qn + __popc(m & ((1u << lane) - 1u))] = pos;
+      if (pre) queue[(qh + qn + __popc(m & ((1u << lane) - 1u))) & 63] = pos;
       qn += __popc(m);
       __syncwarp();
       if (qn >= 32) drain();
@@ -320,20 +313,30 @@ frnn_search_kernel(const float* __restrict__ semb, const float4* __restrict__ sm
   }
   for (int rr = 0; rr < 9; ++rr) {
     const int lo = __shfl_sync(0xffffffffu, my_lo, rr), hi = __shfl_sync(0xffffffffu, my_hi, rr);
-    for (int base = lo; base < hi; base += 32) {
-      const int pos = base + lane;
-      bool pre = false;
-      if (pos < hi) {
-        const float4 cp = __ldg(sproj + pos);
-        const float tx = qp.x - cp.x, ty = qp.y - cp.y, tz = qp.z - cp.z;
-        pre = fmaf(tz, tz, fmaf(ty, ty, tx * tx)) <= r2_proj;
+    // two 32-candidate groups per trip: their loads are independent, the loop and queue bookkeeping is paid once
+    for (int base = lo; base < hi; base += 64) {
+      const int pos0 = base + lane, pos1 = base + 32 + lane;
+      bool pre0 = false, pre1 = false;
+      float4 cp0, cp1;
+      if (pos0 < hi) cp0 = __ldg(sproj + pos0);
+      if (pos1 < hi) cp1 = __ldg(sproj + pos1);
+      if (pos0 < hi) {
+        const float tx = qp.x - cp0.x, ty = qp.y - cp0.y, tz = qp.z - cp0.z;
+        pre0 = fmaf(tz, tz, fmaf(ty, ty, tx * tx)) <= r2_proj;
       }
-      const unsigned m = __ballot_sync(0xffffffffu, pre);
-      if (m) {
-        if (pre) queue0[qn0 + __popc(m & ((1u << lane) - 1u))] = pos;
-        qn0 += __popc(m);
+      if (pos1 < hi) {
+        const float tx = qp.x - cp1.x, ty = qp.y - cp1.y, tz = qp.z - cp1.z;
+        pre1 = fmaf(tz, tz, fmaf(ty, ty, tx * tx)) <= r2_proj;
+      }
+      const unsigned m0 = __ballot_sync(0xffffffffu, pre0), m1 = __ballot_sync(0xffffffffu, pre1);
+      if (m0 | m1) {
+        const unsigned lt = (1u << lane) - 1u;
+        const int n0 = __popc(m0);
+        if (pre0) queue0[(qh0 + qn0 + __popc(m0 & lt)) & 127] = pos0;
+        if (pre1) queue0[(qh0 + qn0 + n0 + __popc(m1 & lt)) & 127] = pos1;
+        qn0 += n0 + __popc(m1);
         __syncwarp();
-        if (qn0 >= 32) drain0();
+        while (qn0 >= 32) drain0();       // at most 31 + 64 entries were queued: the ring of 128 cannot overflow
       }
     }
   }
