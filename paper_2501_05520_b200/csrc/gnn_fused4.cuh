@@ -371,8 +371,10 @@ gnn_edge_fused4_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_co
           uint32_t w[4];
 #pragma unroll
           for (int i = 0; i < 4; ++i) {
+            // ReLU after the rounding: max(bf16(v), 0) == bf16(max(v, 0)), one packed instruction for the pair
             const float2 v = __ffma2_rn(x[c / 2 + i], rs, sh);
-            w[i] = pack_bf16(fmaxf(v.x, 0.f), fmaxf(v.y, 0.f));
+            const __nv_bfloat162 t = __hmax2(__floats2bfloat162_rn(v.x, v.y), __floats2bfloat162_rn(0.f, 0.f));
+            w[i] = *reinterpret_cast<const uint32_t*>(&t);
           }
           const int ch = c >> 3;
           *reinterpret_cast<uint4*>(smem + kOffT + half * kKB + r * 128 + ((ch ^ (r & 7)) << 4)) = make_uint4(w[0], w[1], w[2], w[3]);
