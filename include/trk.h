@@ -97,6 +97,15 @@ typedef struct {
   /* S6: a track candidate is a component with at least min_track_hits hits (values < 1 mean 1;
    * the paper states no minimum, reading C-23).  Used only when track outputs are wanted. */
   int32_t min_track_hits;
+  /* Workspace / search-structure sizing, 0 = default (neither changes any result):
+   *   filter_chunk_rows  S3 processes the candidate edges in passes of this many rows (rounded up to 128); its two
+   *                      activation buffers hold rows x widest layer bf16 each.  Default 128 x SMs x 64 rows
+   *                      (1 212 416 on a B200: 2.5 GB per buffer, 5 launches per pass); smaller values trade a few
+   *                      per cent of throughput for memory (64 x 148 rows: 20 MB per buffer) -- DESIGN.md section 6.
+   *   grid_max           upper bound of the S2 search grid's cells per axis and event (1..128).  Default: the largest of
+   *                      128, 64, 32, 16, 8 whose cell table (max_events x grid_max^3 cells) fits 2^21 cells.          */
+  int64_t filter_chunk_rows;
+  int32_t grid_max;
 } trk_config;
 
 typedef struct {
@@ -150,12 +159,14 @@ trk_status trk_infer_host_tracks(trk_ctx* ctx, int32_t n_events, const int32_t* 
 const char* trk_status_string(trk_status s);
 const char* trk_last_error(const trk_ctx* ctx); /* ctx may be NULL: error of the last failed trk_create */
 int64_t trk_workspace_bytes(const trk_ctx* ctx);
-/* Number of kernels of this library launched by the most recent trk_infer on ctx (host-side count). */
+/* Number of kernels of this library launched by the most recent trk_infer on ctx (host-side count; reset on entry, so it
+ * is 0 after a call that was refused before anything was enqueued). */
 int64_t trk_last_launch_count(const trk_ctx* ctx);
 
 /* Per-stage timing of trk_infer with CUDA events recorded on the call's stream at the stage
  * boundaries (the analogue of perf_analyzer's latency breakdown).
- * trk_profile_enable(ctx, 1) makes the following trk_infer calls record 6 events; trk_profile_stage_ms
+ * trk_profile_enable(ctx, 1) creates the CUDA events (the only allocation of the profiling mode: trk_infer itself never
+ * allocates) and makes the following trk_infer calls record 6 events; trk_profile_stage_ms
  * waits for the last one and writes the HOST array ms[5] = {S1, S2, S3 (incl. compaction), S4, S5}. */
 trk_status trk_profile_enable(trk_ctx* ctx, int32_t on);
 trk_status trk_profile_stage_ms(trk_ctx* ctx, float* ms);
@@ -197,29 +208,30 @@ trk_status trk_stage_cc(trk_ctx* ctx, int64_t n, const int32_t* src, const int32
 trk_status trk_stage_tracks(trk_ctx* ctx, const int32_t* labels, int64_t n, int32_t min_hits, int32_t* track_offsets,
                             int64_t capacity, int32_t* track_hits, int32_t* track_counts, void* cuda_stream);
 
-/* Kernel hook for tests/bench: out = act(A W^T + bias) through the ctx-independent tcgen05 GEMM.
- * A DEVICE bf16 [m][k] (k % 64 == 0), W DEVICE bf16 [n][k] (n % 16 == 0, n <= 1024 ... see DESIGN.md),
- * bias DEVICE fp32 [n], out DEVICE bf16 [m][n]; relu != 0 applies ReLU. */
+/* Kernel hook for tests/bench: out = act(A W^T + bias) through the ctx-independent tcgen05 GEMM on the caller's current
+ * device.  A DEVICE bf16 [m][k] (k % 64 == 0), W DEVICE bf16 [n][k] (n % 64 == 0), bias DEVICE fp32 [n], out DEVICE bf16
+ * [m][n]; relu != 0 applies ReLU; pair = 1: CTA-pair kernel (tcgen05.mma.cta_group::2, 256-row tiles) when the shape
+ * allows it (n % 128 == 0 and k >= 256), pair = 0: single-CTA 128-row tiles.  Thread safe (no shared state). */
 trk_status trk_gemm_bf16(const void* a, const void* w, const float* bias, void* out, int64_t m, int32_t n,
-                         int32_t k, int32_t relu, void* cuda_stream);
+                         int32_t k, int32_t relu, int32_t pair, void* cuda_stream);
 
-/* Tuning / test knob, process wide: selects between kernel variants that compute the same result.
- *   "gemm_pair"  1 (default): dense layers with >= 128 output columns run on CTA pairs (tcgen05.mma.cta_group::2,
- *                256-row tiles); 0: single-CTA 128-row tiles.
- *   "gnn_fused"  2: with gnn_hidden == 128 the S4 edge update and the decoder run as one fused CTA-pair kernel
- *                per iteration (gathered endpoint rows, both layers, LayerNorm, residual; gnn_fused2.cuh); 1: the first
- *                version of that kernel (gnn_fused.cuh); 0: layer-by-layer GEMM launches.
- *                3: its third version (gnn_fused3.cuh), which also fuses the node update; 4 (default): the fourth
- *                (gnn_fused4.cuh, eight-warp epilogues) for the edge and node updates -- DESIGN.md section 6.
- *   "epi_split"  1 (default): bf16-output layers with 256-column tiles and a single 64-wide K block (the first layer of the S3
- *                filter MLP) run their epilogue on eight warps (two per TMEM lane quadrant); 2: in addition that layer's input
- *                rows [e_src ; e_dst] are gathered inside the GEMM kernel instead of by a separate launch (measured slower on
- *                the pileup-200 event: 1.36 ms against 1.01 + 0.25 ms, so not the default); 0: four warps.
- *   "gemm_row_major"  16 (default): a CTA pair of the pair GEMM walks all column tiles of one row block before the next row
- *                block when there are at least 16 row blocks per pair (A rows re-read from L2, no DRAM re-reads); 0: tiles in
- *                pair strides, column fastest.
- * Returns TRK_ERR_INVALID_ARG for an unknown key.  Not thread safe against running trk_* calls. */
-trk_status trk_debug_set(const char* key, int64_t value);
+/* TEST / TUNING hook, per context: selects between kernel variants that compute the same result (each is parity-tested,
+ * tests/test_gpu_stages.py, tests/test_gpu_gemm.py).  Not part of the served path; call it only while no trk_* call on
+ * this ctx is running.
+ *   "gemm_pair"       1 (default): dense layers with >= 128 output columns and K >= 256 run on CTA pairs
+ *                     (tcgen05.mma.cta_group::2, 256-row tiles); 0: single-CTA 128-row tiles.
+ *   "gnn_fused"       1 (default): with gnn_hidden == 128 the S4 encoders, edge update, node update and decoder run as
+ *                     fused two-layer CTA-pair kernels (gnn_fused.cuh); 0: layer-by-layer GEMM launches with the exact
+ *                     split first layer.
+ *   "epi_split"       1 (default): bf16-output layers with 256-column tiles and a single 64-wide K block (the first layer
+ *                     of the S3 filter MLP) run their epilogue on eight warps (two per TMEM lane quadrant); 2: in addition
+ *                     that layer's input rows [e_src ; e_dst] are gathered inside the GEMM kernel instead of by a separate
+ *                     launch (measured slower on the pileup-200 event, so not the default); 0: four warps.
+ *   "gemm_row_major"  16 (default): a CTA pair of the pair GEMM walks all column tiles of one row block before the next
+ *                     row block when there are at least 16 row blocks per pair (A rows re-read from L2, no DRAM
+ *                     re-reads); 0: tiles in pair strides, column fastest.
+ * Returns TRK_ERR_INVALID_ARG for an unknown key. */
+trk_status trk_set_option(trk_ctx* ctx, const char* key, int64_t value);
 
 #ifdef __cplusplus
 }

@@ -20,7 +20,7 @@ EXPORTS = [
     "trk_create", "trk_infer", "trk_destroy", "trk_infer_host", "trk_status_string", "trk_last_error",
     "trk_workspace_bytes", "trk_last_launch_count", "trk_stage_embed", "trk_stage_frnn", "trk_stage_filter",
     "trk_stage_compact", "trk_stage_gnn", "trk_stage_cc", "trk_gemm_bf16", "trk_profile_enable", "trk_profile_stage_ms", "trk_profile_kernel_ms",
-    "trk_debug_set", "trk_stage_tracks", "trk_infer_host_tracks",
+    "trk_set_option", "trk_stage_tracks", "trk_infer_host_tracks",
 ]
 
 _f32p = C.POINTER(C.c_float)
@@ -42,6 +42,7 @@ class TrkConfig(C.Structure):
         ("gnn_cut", C.c_float),
         ("max_hits", C.c_int64), ("max_events", C.c_int64), ("max_cand_edges", C.c_int64), ("max_kept_edges", C.c_int64),
         ("min_track_hits", C.c_int32),
+        ("filter_chunk_rows", C.c_int64), ("grid_max", C.c_int32),
     ]
 
 
@@ -90,9 +91,9 @@ def lib():
     L.trk_stage_compact.argtypes = [vp, vp, vp, vp, i64, vp, vp, i64, vp, vp]
     L.trk_stage_gnn.argtypes = [vp, vp, i64, vp, vp, i64, vp, vp]
     L.trk_stage_cc.argtypes = [vp, i64, vp, vp, vp, i64, C.c_float, vp, vp]
-    L.trk_gemm_bf16.argtypes = [vp, vp, vp, vp, i64, i32, i32, i32, vp]
+    L.trk_gemm_bf16.argtypes = [vp, vp, vp, vp, i64, i32, i32, i32, i32, vp]
     L.trk_profile_enable.argtypes = [vp, i32]
-    L.trk_debug_set.argtypes = [C.c_char_p, i64]
+    L.trk_set_option.argtypes = [vp, C.c_char_p, i64]
     L.trk_profile_stage_ms.argtypes = [vp, _f32p]
     L.trk_profile_kernel_ms.argtypes = [vp, _f32p, i32, _i32p, C.POINTER(i64)]
     L.trk_stage_tracks.argtypes = [vp, vp, i64, i32, vp, i64, vp, vp, vp]
@@ -136,7 +137,7 @@ class Trk:
 
     def __init__(self, *, model, precision, frnn_radius, frnn_k, filter_input, filter_cut, gnn_hidden, gnn_iters, gnn_cut,
                  max_hits, max_events=1, max_cand_edges=None, max_kept_edges=None, gnn_layernorm=True, grid_proj=None,
-                 grid_dims=None, device=0, min_track_hits=3):
+                 grid_dims=None, device=0, min_track_hits=3, filter_chunk_rows=0, grid_max=0):
         L = lib()
         keep = []
         cfg = TrkConfig()
@@ -167,6 +168,8 @@ class Trk:
         cfg.max_cand_edges = int(max_cand_edges if max_cand_edges is not None else max_hits * frnn_k)
         cfg.max_kept_edges = int(max_kept_edges if max_kept_edges is not None else cfg.max_cand_edges)
         cfg.min_track_hits = int(min_track_hits)
+        cfg.filter_chunk_rows = int(filter_chunk_rows)
+        cfg.grid_max = int(grid_max)
         self.cfg = cfg
         self.d_e = d_e
         self.device = device
@@ -198,6 +201,10 @@ class Trk:
     @property
     def last_launch_count(self):
         return lib().trk_last_launch_count(self._h)
+
+    def set_option(self, key: str, value: int) -> None:
+        """Per-context test / tuning hook (include/trk.h trk_set_option): kernel variants that compute the same result."""
+        self._check(lib().trk_set_option(self._h, key.encode(), int(value)))
 
     def profile(self, on=True):
         self._check(lib().trk_profile_enable(self._h, int(on)))
@@ -354,20 +361,13 @@ class Trk:
         return toff, thit, cnt
 
 
-def debug_set(key: str, value: int) -> None:
-    """Process-wide kernel-variant knob (include/trk.h trk_debug_set)."""
-    st = lib().trk_debug_set(key.encode(), int(value))
-    if st != 0:
-        raise TrkError(st, lib().trk_last_error(None).decode())
-
-
-def gemm_bf16(a, w, bias, relu=True, stream=None):
+def gemm_bf16(a, w, bias, relu=True, pair=True, stream=None):
     """out = act(a @ w.T + bias) on the tcgen05 GEMM kernel; a [m,k] bf16, w [n,k] bf16, bias fp32 [n]."""
     import torch
     m, k = a.shape
     n = w.shape[0]
     out = torch.empty(m, n, dtype=torch.bfloat16, device=a.device)
-    st = lib().trk_gemm_bf16(_ptr(a), _ptr(w), _ptr(bias), _ptr(out), m, n, k, int(relu), _stream_ptr(stream))
+    st = lib().trk_gemm_bf16(_ptr(a), _ptr(w), _ptr(bias), _ptr(out), m, n, k, int(relu), int(bool(pair)), _stream_ptr(stream))
     if st != 0:
         raise TrkError(st, lib().trk_last_error(None).decode())
     return out

@@ -24,13 +24,25 @@ trk_status fail(trk_ctx* ctx, trk_status s, const std::string& msg) {
   return s;
 }
 
-static int64_t g_knobs[kKnobCount] = {1, 4, 1, 16, 0, 0, 0, 0};
-int64_t debug_knob(int which) { return g_knobs[which]; }
-
 trk_status gemm_bf16_hook(trk_ctx* ctx, const void* a, const void* w, const float* bias, void* out, int64_t m, int n, int k, int relu,
                           cudaStream_t st);
 
 namespace {
+
+// Every entry point that touches the device runs with ctx->device current and restores the caller's device on return
+// (a process may hold contexts on several GPUs: include/trk.h "device").
+struct DeviceGuard {
+  int prev = -1;
+  bool switched = false;
+  explicit DeviceGuard(int dev) {
+    if (cudaGetDevice(&prev) == cudaSuccess && prev != dev) switched = cudaSetDevice(dev) == cudaSuccess;
+  }
+  ~DeviceGuard() {
+    if (switched) cudaSetDevice(prev);
+  }
+  DeviceGuard(const DeviceGuard&) = delete;
+  DeviceGuard& operator=(const DeviceGuard&) = delete;
+};
 
 int round_up(int v, int m) { return (v + m - 1) / m * m; }
 
@@ -116,8 +128,8 @@ void carve(trk_ctx* c, Carver& k) {
   for (auto& L : c->embed.layers) maxw = std::max(maxw, L.out_pad);
   for (auto& L : c->filter.layers) maxw = std::max(maxw, L.out_pad);
   {
-    int64_t chunk = kFilterChunkRows;
-    if (const char* e = std::getenv("TRK_FILTER_CHUNK_TILES")) chunk = std::max<int64_t>(1, std::atoll(e)) * 128;  // tuning knob
+    int64_t chunk = (int64_t)128 * c->sm_count * kFilterChunkTilesPerSm;
+    if (f.filter_chunk_rows > 0) chunk = (f.filter_chunk_rows + 127) / 128 * 128;
     c->filter_chunk = std::min<int64_t>(chunk, ((int64_t)EC + 127) / 128 * 128);
   }
   c->act_rows = (int64_t)std::max<size_t>(N, (size_t)c->filter_chunk);
@@ -235,13 +247,21 @@ const char* trk_status_string(trk_status s) {
   return "TRK_ERR_UNKNOWN";
 }
 
-const char* trk_last_error(const trk_ctx* ctx) { return ctx ? ctx->last_error.c_str() : g_create_error.c_str(); }
+const char* trk_last_error(const trk_ctx* ctx) {
+  if (ctx) return ctx->last_error.c_str();
+  // the create-time message is copied under the lock into a per-thread buffer: a concurrent failing trk_create may
+  // reallocate the shared string
+  static thread_local std::string copy;
+  std::lock_guard<std::mutex> lk(g_create_mutex);
+  copy = g_create_error;
+  return copy.c_str();
+}
 int64_t trk_workspace_bytes(const trk_ctx* ctx) { return ctx ? (int64_t)ctx->ws.bytes : 0; }
 int64_t trk_last_launch_count(const trk_ctx* ctx) { return ctx ? ctx->launch_count : 0; }
 
 trk_status trk_destroy(trk_ctx* ctx) {
   if (!ctx) return TRK_OK;
-  cudaSetDevice(ctx->device);
+  DeviceGuard guard(ctx->device);
   if (ctx->own_stream) {
     cudaStreamSynchronize(ctx->own_stream);
     cudaStreamDestroy(ctx->own_stream);
@@ -274,6 +294,11 @@ trk_status trk_create(const trk_config* cfg, trk_ctx** out) {
     return fail(nullptr, TRK_ERR_CAPACITY, "capacities exceed the int32 index range");
   if (cfg->max_events > kMaxEvents) return fail(nullptr, TRK_ERR_CAPACITY, "max_events > 1024");
   if (cfg->frnn_k < 1 || cfg->frnn_k > 128) return fail(nullptr, TRK_ERR_INVALID_ARG, "frnn_k must be in 1..128");
+  // S2 scans per-hit degrees (<= frnn_k each) into int32 row offsets before the capacity clamp applies
+  if (cfg->max_hits * (int64_t)cfg->frnn_k > (int64_t)INT32_MAX)
+    return fail(nullptr, TRK_ERR_CAPACITY, "max_hits * frnn_k exceeds the int32 index range");
+  if (cfg->filter_chunk_rows < 0 || cfg->grid_max < 0 || cfg->grid_max > 128)
+    return fail(nullptr, TRK_ERR_INVALID_ARG, "filter_chunk_rows must be >= 0 and grid_max in 0..128");
   if (!(cfg->frnn_radius >= 0.f)) return fail(nullptr, TRK_ERR_INVALID_ARG, "frnn_radius must be >= 0");
   if (cfg->grid_dims < 1 || cfg->grid_dims > 3) return fail(nullptr, TRK_ERR_INVALID_ARG, "grid_dims must be 1..3");
   if (cfg->gnn_iters < 0 || cfg->gnn_hidden <= 0) return fail(nullptr, TRK_ERR_INVALID_ARG, "bad GNN hyperparameters");
@@ -312,7 +337,11 @@ trk_status trk_create(const trk_config* cfg, trk_ctx** out) {
   cudaDeviceProp prop;
   if (cudaGetDeviceProperties(&prop, cfg->device) != cudaSuccess) return fail(nullptr, TRK_ERR_CUDA, "cudaGetDeviceProperties failed");
   if (prop.major != 10) return fail(nullptr, TRK_ERR_UNSUPPORTED_DEVICE, "this library is built for sm_100a (B200) only");
-  if (cudaSetDevice(cfg->device) != cudaSuccess) return fail(nullptr, TRK_ERR_CUDA, "cudaSetDevice failed");
+  DeviceGuard guard(cfg->device);
+  {
+    int cur = -1;
+    if (cudaGetDevice(&cur) != cudaSuccess || cur != cfg->device) return fail(nullptr, TRK_ERR_CUDA, "cudaSetDevice failed");
+  }
 
   trk_ctx* ctx = new trk_ctx();
   ctx->cfg = *cfg;
@@ -329,7 +358,7 @@ trk_status trk_create(const trk_config* cfg, trk_ctx** out) {
   ctx->grid_max = 8;
   for (int g : {128, 64, 32, 16})
     if (cfg->max_events * (int64_t)g * g * g <= kMaxCells) { ctx->grid_max = g; break; }
-  if (const char* e = std::getenv("TRK_GRID_MAX")) ctx->grid_max = std::max(1, std::min(128, std::atoi(e)));   // tuning knob
+  if (cfg->grid_max > 0) ctx->grid_max = cfg->grid_max;
   ctx->max_cells = (int64_t)cfg->max_events * ctx->grid_max * ctx->grid_max * ctx->grid_max;
 
   trk_status s = TRK_OK;
@@ -417,6 +446,9 @@ trk_status trk_create(const trk_config* cfg, trk_ctx** out) {
 
 trk_status trk_infer(trk_ctx* ctx, const trk_batch* batch, const trk_result* res, void* cuda_stream) {
   if (!ctx) return TRK_ERR_INVALID_ARG;
+  DeviceGuard guard(ctx->device);
+  ctx->launch_count = 0;   // counts the launches of THIS call: a call refused below leaves it at 0 (nothing enqueued)
+  ctx->prof_valid = false;
   if (!batch || !res) return fail(ctx, TRK_ERR_INVALID_ARG, "batch or result is NULL");
   if (!res->counts) return fail(ctx, TRK_ERR_INVALID_ARG, "result.counts is required");
   int64_t n = 0;
@@ -432,7 +464,6 @@ trk_status trk_infer(trk_ctx* ctx, const trk_batch* batch, const trk_result* res
     return fail(ctx, TRK_ERR_INVALID_ARG, "track outputs need track_offsets, track_hits, track_counts and track_capacity > 0");
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const trk_config& f = ctx->cfg;
-  ctx->launch_count = 0;
   ctx->kprof_n = 0;
   TRK_LAUNCH(ctx, zero_counts_kernel, 1, 32, 0, st, ctx->counts);
   const bool prof = ctx->profiling && n > 0;
@@ -481,6 +512,7 @@ trk_status trk_infer(trk_ctx* ctx, const trk_batch* batch, const trk_result* res
 trk_status trk_infer_host(trk_ctx* ctx, int32_t n_events, const int32_t* event_offsets, const float* hits_host, int32_t* labels_host,
                           int32_t* counts_host) {
   if (!ctx) return TRK_ERR_INVALID_ARG;
+  DeviceGuard guard(ctx->device);
   int64_t n = 0;
   TRK_TRY(check_batch(ctx, n_events, event_offsets, &n));
   if (n > 0 && (!hits_host || !labels_host)) return fail(ctx, TRK_ERR_INVALID_ARG, "hits_host or labels_host is NULL");
@@ -501,6 +533,7 @@ trk_status trk_infer_host(trk_ctx* ctx, int32_t n_events, const int32_t* event_o
 trk_status trk_infer_host_tracks(trk_ctx* ctx, int32_t n_events, const int32_t* event_offsets, const float* hits_host,
                                  int32_t* labels_host, int32_t* track_offsets_host, int32_t* track_hits_host, int32_t* counts_host) {
   if (!ctx) return TRK_ERR_INVALID_ARG;
+  DeviceGuard guard(ctx->device);
   int64_t n = 0;
   TRK_TRY(check_batch(ctx, n_events, event_offsets, &n));
   if (!track_offsets_host || !counts_host || (n > 0 && (!hits_host || !track_hits_host)))
@@ -530,8 +563,17 @@ trk_status trk_infer_host_tracks(trk_ctx* ctx, int32_t n_events, const int32_t* 
 
 trk_status trk_profile_enable(trk_ctx* ctx, int32_t on) {
   if (!ctx) return TRK_ERR_INVALID_ARG;
-  if (on && !ctx->prof_ev[0])
+  DeviceGuard guard(ctx->device);
+  if (on && !ctx->prof_ev[0]) {
     for (auto& e : ctx->prof_ev) TRK_CUDA(ctx, cudaEventCreate(&e));
+    // one event pair per hidden-layer GEMM launch of S3 (trk_profile_kernel_ms): created here so that trk_infer never allocates
+    const size_t pairs = (size_t)ceil_div(ctx->cfg.max_cand_edges, ctx->filter_chunk) * ctx->filter.layers.size();
+    while (ctx->kprof_ev.size() < 2 * pairs) {
+      cudaEvent_t e;
+      TRK_CUDA(ctx, cudaEventCreate(&e));
+      ctx->kprof_ev.push_back(e);
+    }
+  }
   ctx->profiling = on != 0;
   ctx->prof_valid = false;
   return TRK_OK;
@@ -559,6 +601,7 @@ trk_status trk_profile_kernel_ms(trk_ctx* ctx, float* ms, int32_t capacity, int3
 // ------------------------------------------------------------------ stage hooks
 trk_status trk_stage_embed(trk_ctx* ctx, const float* hits, int64_t n, float* emb, void* cuda_stream) {
   if (!ctx) return TRK_ERR_INVALID_ARG;
+  DeviceGuard guard(ctx->device);
   if (n < 0 || (n > 0 && (!hits || !emb))) return fail(ctx, TRK_ERR_INVALID_ARG, "stage_embed: bad arguments");
   if (n > ctx->cfg.max_hits) return fail(ctx, TRK_ERR_CAPACITY, "stage_embed: n exceeds max_hits");
   return embed_dispatch(ctx, hits, n, emb, (cudaStream_t)cuda_stream);
@@ -567,6 +610,7 @@ trk_status trk_stage_embed(trk_ctx* ctx, const float* hits, int64_t n, float* em
 trk_status trk_stage_frnn(trk_ctx* ctx, const float* emb, const float* hits, const int32_t* event_offsets, int32_t n_events,
                           int32_t* src, int32_t* dst, int32_t* rowptr, int64_t capacity, int32_t* count, void* cuda_stream) {
   if (!ctx) return TRK_ERR_INVALID_ARG;
+  DeviceGuard guard(ctx->device);
   int64_t n = 0;
   TRK_TRY(check_batch(ctx, n_events, event_offsets, &n));
   if (!count || capacity < 0 || (capacity > 0 && (!src || !dst))) return fail(ctx, TRK_ERR_INVALID_ARG, "stage_frnn: bad arguments");
@@ -587,6 +631,7 @@ trk_status trk_stage_frnn(trk_ctx* ctx, const float* emb, const float* hits, con
 trk_status trk_stage_filter(trk_ctx* ctx, const float* feat, int64_t n, const int32_t* src, const int32_t* dst, int64_t n_edges,
                             float* score, void* cuda_stream) {
   if (!ctx) return TRK_ERR_INVALID_ARG;
+  DeviceGuard guard(ctx->device);
   if (n < 0 || n_edges < 0 || (n_edges > 0 && (!feat || !src || !dst || !score))) return fail(ctx, TRK_ERR_INVALID_ARG, "stage_filter: bad arguments");
   return filter_dispatch(ctx, feat, src, dst, nullptr, n_edges, score, (cudaStream_t)cuda_stream);
 }
@@ -594,6 +639,7 @@ trk_status trk_stage_filter(trk_ctx* ctx, const float* feat, int64_t n, const in
 trk_status trk_stage_compact(trk_ctx* ctx, const int32_t* src, const int32_t* dst, const float* score, int64_t n_edges,
                              int32_t* out_src, int32_t* out_dst, int64_t capacity, int32_t* count, void* cuda_stream) {
   if (!ctx) return TRK_ERR_INVALID_ARG;
+  DeviceGuard guard(ctx->device);
   if (n_edges < 0 || capacity < 0 || !count || (n_edges > 0 && (!src || !dst || !score || !out_src || !out_dst)))
     return fail(ctx, TRK_ERR_INVALID_ARG, "stage_compact: bad arguments");
   if (n_edges > ctx->cfg.max_cand_edges) return fail(ctx, TRK_ERR_CAPACITY, "stage_compact: n_edges exceeds max_cand_edges");
@@ -611,6 +657,7 @@ trk_status trk_stage_compact(trk_ctx* ctx, const int32_t* src, const int32_t* ds
 trk_status trk_stage_gnn(trk_ctx* ctx, const float* hits, int64_t n, const int32_t* src, const int32_t* dst, int64_t n_edges,
                          float* score, void* cuda_stream) {
   if (!ctx) return TRK_ERR_INVALID_ARG;
+  DeviceGuard guard(ctx->device);
   if (n < 0 || n_edges < 0 || (n > 0 && !hits) || (n_edges > 0 && (!src || !dst || !score)))
     return fail(ctx, TRK_ERR_INVALID_ARG, "stage_gnn: bad arguments");
   if (n > ctx->cfg.max_hits || n_edges > ctx->cfg.max_kept_edges) return fail(ctx, TRK_ERR_CAPACITY, "stage_gnn: exceeds max_hits / max_kept_edges");
@@ -620,6 +667,7 @@ trk_status trk_stage_gnn(trk_ctx* ctx, const float* hits, int64_t n, const int32
 trk_status trk_stage_cc(trk_ctx* ctx, int64_t n, const int32_t* src, const int32_t* dst, const float* score, int64_t n_edges,
                         float cut, int32_t* labels, void* cuda_stream) {
   if (!ctx) return TRK_ERR_INVALID_ARG;
+  DeviceGuard guard(ctx->device);
   if (n < 0 || n_edges < 0 || (n > 0 && !labels) || (n_edges > 0 && (!src || !dst || !score)))
     return fail(ctx, TRK_ERR_INVALID_ARG, "stage_cc: bad arguments");
   if (n > ctx->cfg.max_hits) return fail(ctx, TRK_ERR_CAPACITY, "stage_cc: n exceeds max_hits");
@@ -629,6 +677,7 @@ trk_status trk_stage_cc(trk_ctx* ctx, int64_t n, const int32_t* src, const int32
 trk_status trk_stage_tracks(trk_ctx* ctx, const int32_t* labels, int64_t n, int32_t min_hits, int32_t* track_offsets, int64_t capacity,
                             int32_t* track_hits, int32_t* track_counts, void* cuda_stream) {
   if (!ctx) return TRK_ERR_INVALID_ARG;
+  DeviceGuard guard(ctx->device);
   if (n < 0 || capacity <= 0 || !track_offsets || !track_counts || (n > 0 && (!labels || !track_hits)))
     return fail(ctx, TRK_ERR_INVALID_ARG, "stage_tracks: bad arguments");
   if (n > ctx->cfg.max_hits) return fail(ctx, TRK_ERR_CAPACITY, "stage_tracks: n exceeds max_hits");
@@ -637,22 +686,28 @@ trk_status trk_stage_tracks(trk_ctx* ctx, const int32_t* labels, int64_t n, int3
   return build_tracks(ctx, labels, n, min_hits, track_offsets, capacity, track_hits, track_counts, track_counts + 2, st);
 }
 
-trk_status trk_debug_set(const char* key, int64_t value) {
-  if (!key) return TRK_ERR_INVALID_ARG;
-  if (std::strcmp(key, "gemm_pair") == 0) { g_knobs[kKnobGemmPair] = value; return TRK_OK; }
-  if (std::strcmp(key, "gnn_fused") == 0) { g_knobs[kKnobGnnFused] = value; return TRK_OK; }
-  if (std::strcmp(key, "epi_split") == 0) { g_knobs[kKnobEpiSplit] = value; return TRK_OK; }
-  if (std::strcmp(key, "gemm_row_major") == 0) { g_knobs[kKnobRowMajor] = value; return TRK_OK; }
-  return fail(nullptr, TRK_ERR_INVALID_ARG, std::string("trk_debug_set: unknown key ") + key);
+trk_status trk_set_option(trk_ctx* ctx, const char* key, int64_t value) {
+  if (!ctx) return TRK_ERR_INVALID_ARG;
+  if (!key) return fail(ctx, TRK_ERR_INVALID_ARG, "trk_set_option: key is NULL");
+  static const struct { const char* name; int knob; } keys[] = {
+      {"gemm_pair", kKnobGemmPair}, {"gnn_fused", kKnobGnnFused}, {"epi_split", kKnobEpiSplit}, {"gemm_row_major", kKnobRowMajor}};
+  for (const auto& k : keys)
+    if (std::strcmp(key, k.name) == 0) {
+      ctx->knobs[k.knob] = value;
+      return TRK_OK;
+    }
+  return fail(ctx, TRK_ERR_INVALID_ARG, std::string("trk_set_option: unknown key ") + key);
 }
 
 trk_status trk_gemm_bf16(const void* a, const void* w, const float* bias, void* out, int64_t m, int32_t n, int32_t k, int32_t relu,
-                         void* cuda_stream) {
-  static trk_ctx hook_ctx;  // only sm_count, launch_count and last_error are used
-  if (!a || !w || !bias || !out || m <= 0) return fail(nullptr, TRK_ERR_INVALID_ARG, "gemm_bf16: bad arguments");
+                         int32_t pair, void* cuda_stream) {
+  if (!a || !w || !bias || !out || m <= 0 || (pair != 0 && pair != 1)) return fail(nullptr, TRK_ERR_INVALID_ARG, "gemm_bf16: bad arguments");
   if (k % 64 != 0 || n % 64 != 0) return fail(nullptr, TRK_ERR_SHAPE, "gemm_bf16: k and n must be multiples of 64");
+  trk_ctx hook_ctx;  // per call (runs on the caller's current device): only sm_count, knobs, launch_count and last_error are used
+  hook_ctx.knobs[kKnobGemmPair] = pair;
   int dev = 0;
   cudaGetDevice(&dev);
+  hook_ctx.device = dev;
   cudaDeviceGetAttribute(&hook_ctx.sm_count, cudaDevAttrMultiProcessorCount, dev);
   trk_status s = gemm_bf16_hook(&hook_ctx, a, w, bias, out, m, n, k, relu, (cudaStream_t)cuda_stream);
   if (s != TRK_OK) fail(nullptr, s, hook_ctx.last_error);

@@ -15,8 +15,11 @@ namespace trk {
 constexpr int kMaxEmbDim = 16;      // d_e is padded to a multiple of 4, at most 16
 constexpr int kMaxEvents = 1024;    // event offsets travel as a kernel parameter
 constexpr int64_t kMaxCells = 1 << 21;  // FRNN grid cells summed over the events of a call
-constexpr int kFilterChunkRows = 128 * 148 * 64;  // S3 rows per pass (upper bound; ctx->filter_chunk is the per-context value):
-                                                  // 2.5 GB per activation buffer buys 5 launches per 1.2 M candidate edges
+constexpr int kFilterChunkTilesPerSm = 64;  // default S3 rows per pass = 128 x sm_count x 64 (trk_config.filter_chunk_rows overrides):
+                                            // 2.5 GB per activation buffer buys 5 launches per 1.2 M candidate edges
+
+// ---- test / tuning options (trk_set_option), per context ----
+enum { kKnobGemmPair = 0, kKnobGnnFused = 1, kKnobEpiSplit = 2, kKnobRowMajor = 3, kKnobCount = 4 };
 
 // One Linear layer resident on the device.
 struct DevLinear {
@@ -60,6 +63,8 @@ struct trk_ctx {
   cudaStream_t own_stream = nullptr;
   std::string last_error;
   int64_t launch_count = 0;
+  int64_t knobs[trk::kKnobCount] = {1, 1, 1, 16};   // gemm_pair, gnn_fused, epi_split, gemm_row_major (include/trk.h trk_set_option)
+  std::vector<const void*> smem_attr_set;          // kernels whose dynamic shared-memory limit has been raised on ctx->device
   bool profiling = false;
   cudaEvent_t prof_ev[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
   bool prof_valid = false;
@@ -170,9 +175,17 @@ trk_status fail(trk_ctx* ctx, trk_status s, const std::string& msg);
 
 inline int64_t ceil_div(int64_t a, int64_t b) { return (a + b - 1) / b; }
 
-// ---- tuning / test knobs (trk_debug_set) ----
-enum { kKnobGemmPair = 0, kKnobGnnFused = 1, kKnobEpiSplit = 2, kKnobRowMajor = 3, kKnobCount = 8 };
-int64_t debug_knob(int which);
+// cudaFuncAttributeMaxDynamicSharedMemorySize is a per-device attribute of a kernel: it is raised once per context (a context
+// is bound to one device; the caller's current device is ctx->device inside every entry point, see DeviceGuard in api.cu).
+template <class Kernel>
+inline trk_status ensure_smem(trk_ctx* ctx, Kernel kern, int bytes) {
+  const void* key = reinterpret_cast<const void*>(kern);
+  for (const void* k : ctx->smem_attr_set)
+    if (k == key) return TRK_OK;
+  TRK_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+  ctx->smem_attr_set.push_back(key);
+  return TRK_OK;
+}
 
 // ---- util_kernels.cu ----
 trk_status exclusive_scan_i32(trk_ctx* ctx, const int32_t* in, int32_t* out, int64_t n, int32_t* tmp, cudaStream_t st);

@@ -1,22 +1,26 @@
-// Fused interaction-network edge update of S4 for H = 128 on CTA pairs (reading C-12):
+// Fused two-layer interaction-network kernels of S4 for H = 128 on CTA pairs (reading C-12):
 //
-//   e_k <- e_k + LNR(W2 LNR(W1 [h_src(k) ; h_dst(k) ; e_k] + b1) + b2)           (kUpdate)
-//   score_k = sigmoid(w_out . LNR(W1 [h_src ; h_dst ; e_k] + b1) + b_out)        (kDecode)
+//   e_k <- e_k + LNR(W2 LNR(W1 [h_src(k) ; h_dst(k) ; e_k] + b1) + b2)           (kUpdate: the edge update, rows of E)
+//   score_k = sigmoid(w_out . LNR(W1 [h_src ; h_dst ; e_k] + b1) + b_out)        (kDecode: the decoder)
+//   h_v <- h_v + LNR(W2 LNR(W1 [h_v ; m_in_v ; m_out_v] + b1) + b2)              (kNode: the node update, rows of X)
 //
-// One 2-CTA cluster handles 256 edges per tile (128 per CTA) and never writes an intermediate to HBM:
-//   * both weight matrices stay in shared memory for the whole kernel, split by output row between the
-//     two CTAs (tcgen05.mma.cta_group::2 reads the N halves from both SMs): 64 KB per CTA;
-//   * the 3H-wide first-layer input is assembled in shared memory as six K blocks: the e rows by TMA,
-//     the h rows of the edge's endpoints by cp.async gathers (coalesced 256-byte rows) straight into
-//     the 128-byte-swizzled UMMA layout;
-//   * layer-1 accumulator (TMEM) -> LayerNorm + ReLU in registers -> bf16 tile T in shared memory ->
-//     layer-2 MMA -> LayerNorm + ReLU + residual (read from the e tile still in shared memory) ->
-//     the e tile is overwritten in place and leaves by TMA store.
-// HBM traffic per edge and iteration: 256 B of e in, 256 B out, 8 B of indices; the h rows (20 MB table)
-// come from L2.
-//
-// Warps: 0 TMA producer, 1 MMA issuer (leader CTA) + TMEM owner, 2-5 epilogue 1, 6-9 epilogue 2,
-// 10-13 gather.  TMEM: acc1[2] (columns 0,128) and acc2[2] (256,384), so two tiles are in flight.
+// One 2-CTA cluster handles 256 rows per tile (128 per CTA) and never writes an intermediate to HBM:
+//   * both weight matrices stay in shared memory for the whole kernel, split by output row between the two CTAs
+//     (tcgen05.mma.cta_group::2 reads the N halves from both SMs): 64 KB per CTA;
+//   * the 3H-wide first-layer operand is assembled in shared memory as six K blocks: the e rows by TMA, the h rows of the
+//     edge's endpoints by cp.async gathers (256-byte rows) straight into the 128-byte-swizzled UMMA layout; kNode loads
+//     all six K blocks of X = (h | m_in | m_out) by TMA;
+//   * layer-1 accumulator (TMEM) -> LayerNorm + ReLU in registers -> bf16 tile T in shared memory -> layer-2 MMA ->
+//     LayerNorm + ReLU + residual -> TMA store.  The e tile is held twice with separate lifetimes: as the layer-1 operand
+//     (freed as soon as MMA 1 has read it) and as the residual / output staging of epilogue 2 (a second TMA load that hits L2).
+// Both LayerNorm epilogues run on EIGHT warps, two per TMEM lane quadrant, each taking one 64-column K block of the row:
+//   * a thread reads 64 accumulator columns, adds the bias, forms the partial (sum, sum of squares) of its half row and
+//     exchanges it with the thread that holds the other half through shared memory (named barriers of 64 threads);
+//     variance = E[x^2] - mean^2 in fp32 (the values are LayerNorm-scale, no cancellation problem);
+//   * epilogue 1 exchanges through one float2 per row (statistics one way, coefficients back); epilogue 2 exchanges inside
+//     the first 16-byte cell of its row of the residual tile (the cell's residual values wait in registers).
+// 22 warps: 0 TMA, 1 MMA issuer (leader CTA) + TMEM owner, 2-5 gather, 6-13 epilogue 1, 14-21 epilogue 2.
+// TMEM: acc1[2] (columns 0, 128) and acc2[2] (256, 384), so two tiles are in flight.
 // mbarriers marked L are used in the leader CTA's copy only (both CTAs arrive on it).
 #pragma once
 
@@ -28,20 +32,11 @@ namespace gf {
 using namespace tc;
 
 constexpr int kH = 128;
-constexpr int kThreadsFused = 14 * 32;
 constexpr int kTileRows = 128;            // per CTA
 constexpr int kKB = 16384;                // one 128-row x 64-column bf16 K block
 constexpr int kWKB = 8192;                // one 64-row x 64-column K block of a weight half
-// shared memory carve-up (bytes, per CTA)
-constexpr int kOffW1 = 0;                 // 6 K blocks of this CTA's 64 output rows of W1
-constexpr int kOffW2 = kOffW1 + 6 * kWKB; // 2 K blocks of W2
-constexpr int kOffRing = kOffW2 + 2 * kWKB;   // 4 K blocks: h_src (2), h_dst (2)
-constexpr int kOffEHold = kOffRing + 4 * kKB; // 2 x (2 K blocks): the e tile of the two tiles in flight
-constexpr int kOffT = kOffEHold + 4 * kKB;    // 2 K blocks: layer-1 output
-constexpr int kOffBar = kOffT + 2 * kKB;
-constexpr int kSmemFused = kOffBar + 256 + 1024;
 
-enum Mode { kUpdate = 0, kDecode = 1 };
+enum Mode { kUpdate = 0, kDecode = 1, kNode = 2 };
 
 struct FusedParams {
   const __nv_bfloat16* X;     // [n_nodes][ldx] bf16, h = columns [0, 128)
@@ -56,21 +51,6 @@ struct FusedParams {
   float* score;
 };
 
-struct Bars {
-  uint64_t w_full;
-  uint64_t efull[2];      // L  tx: both CTAs' e tiles
-  uint64_t eempty[2];     //    own, 4 arrivals (the warps that last touch the e tile)
-  uint64_t gfull[2];      // L  8 arrivals (4 gather warps x 2 CTAs), halves: h_src, h_dst
-  uint64_t gempty[2];     //    own, multicast commit
-  uint64_t a1full[2];     //    own, multicast commit
-  uint64_t a1empty[2];    // L  8 arrivals
-  uint64_t tfull;         // L  8 arrivals
-  uint64_t tempty;        //    own, multicast commit
-  uint64_t a2full[2];     //    own, multicast commit
-  uint64_t a2empty[2];    // L  8 arrivals
-  uint32_t tmem_slot;
-};
-
 __device__ __forceinline__ void cp_async_16(uint32_t smem_dst, const void* gsrc, int src_bytes) {
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(smem_dst), "l"(gsrc), "r"(src_bytes) : "memory");
 }
@@ -78,40 +58,121 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
-// LayerNorm statistics of one accumulator row (this thread's TMEM lane), columns [0,128) of `taddr`, after adding bias.
-__device__ __forceinline__ void row_stats(uint32_t taddr, const float* __restrict__ bias, int use_ln, float& mean, float& rstd) {
-  float s = 0.f, q = 0.f;
-#pragma unroll 1
-  for (int c = 0; c < kH; c += 32) {
-    uint32_t r[32];
-    tmem_ld32(taddr + c, r);
-    tmem_ld_wait();
+// non-blocking probe of an mbarrier phase (cluster-scope acquire: remote CTAs arrive on some of them)
+__device__ __forceinline__ bool mbar_test(uint64_t* bar, uint32_t parity) {
+  uint32_t ok;
+  asm volatile(
+      "{\n"
+      ".reg .pred P1;\n"
+      "mbarrier.test_wait.parity.acquire.cluster.shared::cta.b64 P1, [%1], %2;\n"
+      "selp.u32 %0, 1, 0, P1;\n"
+      "}\n"
+      : "=r"(ok)
+      : "r"(smem_u32(bar)), "r"(parity)
+      : "memory");
+  return ok != 0;
+}
+
+// Arrive on an mbarrier of the pair's leader CTA with CTA-scope release.  What the leader's MMA issuer must see before it
+// continues is either a finished TMEM read (ordered by tcgen05.fence::before_thread_sync) or shared memory of the ARRIVING
+// CTA that its own tensor core / TMA will read (ordered by fence.proxy.async); neither needs the cluster-wide memory barrier
+// of .release.cluster, which cost the epilogue warps several hundred cycles per arrive.
+__device__ __forceinline__ void mbar_arrive_remote(uint32_t cluster_addr) {
+  asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
+}
+
+__device__ __forceinline__ void tma_prefetch_l2_2d(const CUtensorMap* tmap, int c0, int c1) {
+  asm volatile("cp.async.bulk.prefetch.tensor.2d.L2.global.tile [%0, {%1, %2}];" ::"l"(reinterpret_cast<uint64_t>(tmap)), "r"(c0), "r"(c1)
+               : "memory");
+}
+
+__device__ __forceinline__ float2 f2(float a, float b) { return make_float2(a, b); }
+
+constexpr int kFusedThreads = 22 * 32;
+constexpr int kOffW1 = 0;                       // 6 K blocks of this CTA's 64 output rows of W1
+constexpr int kOffW2 = kOffW1 + 6 * kWKB;       // 2 K blocks of W2
+constexpr int kOffRing = kOffW2 + 2 * kWKB;     // 4 K blocks: h_src (2), h_dst (2)
+constexpr int kOffEOp = kOffRing + 4 * kKB;     // 2 K blocks: the e tile as layer-1 operand
+constexpr int kOffRes = kOffEOp + 2 * kKB;      // 2 K blocks: the e tile as residual, overwritten in place and stored
+constexpr int kOffT = kOffRes + 2 * kKB;        // 2 K blocks: layer-1 output
+constexpr int kOffVec = kOffT + 2 * kKB;        // b1, b2, w_out: 3 x 128 fp32
+constexpr int kOffX1 = kOffVec + 3 * kH * 4;     // epilogue 1: one float2 per row, half-row statistics one way, coefficients back
+constexpr int kOffBar = kOffX1 + kTileRows * 8;
+constexpr int kSmemFused = kOffBar + 256;
+static_assert(kSmemFused <= 232448, "shared memory budget of one CTA");
+
+struct Bars {
+  uint64_t w_full;
+  uint64_t eopfull;       // L  tx: both CTAs' operand tiles
+  uint64_t eopempty;      //    own, multicast commit (MMA 1 has read the operand tile)
+  uint64_t resfull;       //    own, tx: this CTA's residual tile
+  uint64_t resempty;      //    own, 8 arrivals (epilogue-2 warps, after their rows have left shared memory)
+  uint64_t gfull[2];      // L  8 arrivals (4 gather warps x 2 CTAs), halves: h_src, h_dst (kNode: 1, tx)
+  uint64_t gempty[2];     //    own, multicast commit
+  uint64_t a1full[2];     //    own, multicast commit
+  uint64_t a1empty[2];    // L  16 arrivals
+  uint64_t tfull;         // L  16 arrivals
+  uint64_t tempty;        //    own, multicast commit
+  uint64_t a2full[2];     //    own, multicast commit
+  uint64_t a2empty[2];    // L  16 arrivals
+  uint32_t tmem_slot;
+};
+
+__device__ __forceinline__ void named_bar_sync(int id, int threads) {
+  asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(threads) : "memory");
+}
+
+// Half an accumulator row (this thread's TMEM lane, 64 fp32 columns from `taddr`) + bias -> 32 packed pairs, and the
+// partial sum / sum of squares of those 64 values.
+template <bool BIAS_GLOBAL>
+__device__ __forceinline__ void load_half(uint32_t taddr, const float* __restrict__ bias, float2 (&x)[32], float& ps, float& pq) {
+  uint32_t u0[32], u1[32];
+  tmem_ld32(taddr, u0);
+  tmem_ld32(taddr + 32, u1);
+  const float4* b4 = reinterpret_cast<const float4*>(bias);
+  float4 bb[16];
 #pragma unroll
-    for (int i = 0; i < 32; i += 4) {
-      const float4 b = __ldg(reinterpret_cast<const float4*>(bias + c + i));
-      const float v0 = __uint_as_float(r[i]) + b.x, v1 = __uint_as_float(r[i + 1]) + b.y, v2 = __uint_as_float(r[i + 2]) + b.z,
-                  v3 = __uint_as_float(r[i + 3]) + b.w;
-      s += (v0 + v1) + (v2 + v3);
-      q = fmaf(v0, v0, q); q = fmaf(v1, v1, q); q = fmaf(v2, v2, q); q = fmaf(v3, v3, q);
-    }
+  for (int j = 0; j < 16; ++j) bb[j] = BIAS_GLOBAL ? __ldg(b4 + j) : b4[j];
+  tmem_ld_wait();
+#pragma unroll
+  for (int i = 0; i < 32; i += 4) {
+    x[i / 2] = __fadd2_rn(f2(__uint_as_float(u0[i]), __uint_as_float(u0[i + 1])), f2(bb[i / 4].x, bb[i / 4].y));
+    x[i / 2 + 1] = __fadd2_rn(f2(__uint_as_float(u0[i + 2]), __uint_as_float(u0[i + 3])), f2(bb[i / 4].z, bb[i / 4].w));
+    x[16 + i / 2] = __fadd2_rn(f2(__uint_as_float(u1[i]), __uint_as_float(u1[i + 1])), f2(bb[8 + i / 4].x, bb[8 + i / 4].y));
+    x[16 + i / 2 + 1] = __fadd2_rn(f2(__uint_as_float(u1[i + 2]), __uint_as_float(u1[i + 3])), f2(bb[8 + i / 4].z, bb[8 + i / 4].w));
   }
+  float2 s0 = f2(0.f, 0.f), s1 = s0, q0 = s0, q1 = s0;
+#pragma unroll
+  for (int i = 0; i < 32; i += 2) {
+    s0 = __fadd2_rn(s0, x[i]); s1 = __fadd2_rn(s1, x[i + 1]);
+    q0 = __ffma2_rn(x[i], x[i], q0); q1 = __ffma2_rn(x[i + 1], x[i + 1], q1);
+  }
+  const float2 s = __fadd2_rn(s0, s1), q = __fadd2_rn(q0, q1);
+  ps = s.x + s.y;
+  pq = q.x + q.y;
+}
+
+__device__ __forceinline__ void ln_coeffs(float ps, float pq, float2 other, int use_ln, float2& rs, float2& sh) {
+  float mean = 0.f, rstd = 1.f;
   if (use_ln) {
-    mean = s * (1.f / kH);
-    const float var = fmaxf(q * (1.f / kH) - mean * mean, 0.f);
+    mean = (ps + other.x) * (1.f / kH);
+    const float var = fmaxf((pq + other.y) * (1.f / kH) - mean * mean, 0.f);
     rstd = rsqrtf(var + 1e-5f);
-  } else {
-    mean = 0.f;
-    rstd = 1.f;
   }
+  rs = f2(rstd, rstd);
+  sh = f2(-mean * rstd, -mean * rstd);
 }
 
 template <int MODE>
-__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsFused, 1)
-gnn_edge_fused_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constant__ CUtensorMap tmW2,
-                      const __grid_constant__ CUtensorMap tmE, const __grid_constant__ CUtensorMap tmEst, Rows rows, FusedParams p) {
-  extern __shared__ uint8_t smem_raw[];
-  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kFusedThreads, 1)
+gnn_fused_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constant__ CUtensorMap tmW2,
+                       const __grid_constant__ CUtensorMap tmE, const __grid_constant__ CUtensorMap tmEst, Rows rows, FusedParams p) {
+  extern __shared__ __align__(1024) uint8_t smem[];
+  if ((smem_u32(smem) & 1023u) != 0) __trap();   // the swizzled operand layout needs the 1024-byte alignment declared above
   Bars* bar = reinterpret_cast<Bars*>(smem + kOffBar);
+  float* sb1 = reinterpret_cast<float*>(smem + kOffVec);
+  float* sb2 = sb1 + kH;
+  float* swo = sb2 + kH;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const uint32_t rank = cluster_ctarank();
   const bool leader = rank == 0;
@@ -119,21 +180,28 @@ gnn_edge_fused_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_con
   const int64_t M = resolve_rows(rows);
   const int64_t total = (M + 2 * kTileRows - 1) / (2 * kTileRows);
   const int n_my = total > pair ? (int)((total - pair + n_pairs - 1) / n_pairs) : 0;
+  constexpr bool kTwoLayers = MODE != kDecode;
+  // K blocks of W1 that go with the operand tile (e, or h in kNode) and with the two ring halves
+  constexpr int kbE = MODE == kNode ? 0 : 4;
+  constexpr int kbR = MODE == kNode ? 2 : 0;
+  constexpr int colE = 0;                        // first column of the operand / residual tile in its tensor
 
   if (warp == 0 && lane == 0) {
     prefetch_tmap(&tmW1); prefetch_tmap(&tmW2); prefetch_tmap(&tmE); prefetch_tmap(&tmEst);
     mbar_init(&bar->w_full, 1);
+    mbar_init(&bar->eopfull, 1);
+    mbar_init(&bar->eopempty, 1);
+    mbar_init(&bar->resfull, 1);
+    mbar_init(&bar->resempty, 8);
     for (int i = 0; i < 2; ++i) {
-      mbar_init(&bar->efull[i], 1);
-      mbar_init(&bar->eempty[i], 4);
-      mbar_init(&bar->gfull[i], 8);
+      mbar_init(&bar->gfull[i], MODE == kNode ? 1 : 8);
       mbar_init(&bar->gempty[i], 1);
       mbar_init(&bar->a1full[i], 1);
-      mbar_init(&bar->a1empty[i], 8);
+      mbar_init(&bar->a1empty[i], 16);
       mbar_init(&bar->a2full[i], 1);
-      mbar_init(&bar->a2empty[i], 8);
+      mbar_init(&bar->a2empty[i], 16);
     }
-    mbar_init(&bar->tfull, 8);
+    mbar_init(&bar->tfull, 16);
     mbar_init(&bar->tempty, 1);
     fence_barrier_init();
     // this CTA's halves of the weights: output rows [64 rank, 64 rank + 64)
@@ -142,6 +210,12 @@ gnn_edge_fused_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_con
     for (int kb = 0; kb < 2; ++kb) tma_load_2d(smem + kOffW2 + kb * kWKB, &tmW2, &bar->w_full, kb * 64, (int)rank * 64);
   }
   if (warp == 1) tmem_alloc_pair<512>(&bar->tmem_slot);
+  if (threadIdx.x >= 128 && threadIdx.x < 128 + kH) {
+    const int c = threadIdx.x - 128;
+    sb1[c] = p.b1[c];
+    sb2[c] = kTwoLayers ? p.b2[c] : 0.f;
+    swo[c] = MODE == kDecode ? p.w_out[c] : 0.f;
+  }
   __syncthreads();
   mbar_wait(&bar->w_full, 0);
   tc_fence_before();
@@ -151,21 +225,46 @@ gnn_edge_fused_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_con
   const uint32_t sbase = smem_u32(smem);
 
   if (warp == 0) {
-    // ---------------------------------------------------------------- TMA producer: e tiles
+    // ---------------------------------------------------------------- TMA producer: operand and residual copies of the e tiles
     if (lane == 0) {
-      for (int tl = 0; tl < n_my; ++tl) {
-        const int64_t tile = pair + (int64_t)tl * n_pairs;
-        const int b = tl & 1;
-        const uint32_t ph = (tl >> 1) & 1;
-        mbar_wait(&bar->eempty[b], ph ^ 1);
-        if (leader) mbar_arrive_expect_tx(&bar->efull[b], 2 * 2 * kKB);
-        const uint32_t full_leader = mapa_u32(smem_u32(&bar->efull[b]), 0);
-        const int row0 = (int)(tile * 2 * kTileRows + rank * kTileRows);
-        for (int kb = 0; kb < 2; ++kb) tma_load_2d_pair(smem + kOffEHold + (b * 2 + kb) * kKB, &tmE, full_leader, kb * 64, row0);
+      auto row0_of = [&](int tl) { return (int)((pair + (int64_t)tl * n_pairs) * 2 * kTileRows + rank * kTileRows); };
+      auto prefetch = [&](int tl) {
+        if (tl < n_my)
+          for (int kb = 0; kb < (MODE == kNode ? 6 : 2); ++kb) tma_prefetch_l2_2d(&tmE, kb * 64, row0_of(tl));
+      };
+      prefetch(1);
+      prefetch(2);
+      const uint32_t eopfull_leader = mapa_u32(smem_u32(&bar->eopfull), 0);
+      const uint32_t gfull_leader[2] = {mapa_u32(smem_u32(&bar->gfull[0]), 0), mapa_u32(smem_u32(&bar->gfull[1]), 0)};
+      int n_op = 0, n_res = 0, n_g[2] = {0, 0};
+      const int res_end = kTwoLayers ? n_my : 0;
+      const int g_end = MODE == kNode ? n_my : 0;
+      while (n_op < n_my || n_res < res_end || n_g[0] < g_end || n_g[1] < g_end) {
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {              // kNode: m_in | m_out blocks into the ring halves
+          if (n_g[h] < g_end && mbar_test(&bar->gempty[h], (uint32_t)(n_g[h] & 1) ^ 1)) {
+            if (leader) mbar_arrive_expect_tx(&bar->gfull[h], 2 * 2 * kKB);
+            for (int kb = 0; kb < 2; ++kb)
+              tma_load_2d_pair(smem + kOffRing + (h * 2 + kb) * kKB, &tmE, gfull_leader[h], kH + h * kH + kb * 64, row0_of(n_g[h]));
+            ++n_g[h];
+          }
+        }
+        if (n_op < n_my && mbar_test(&bar->eopempty, (uint32_t)(n_op & 1) ^ 1)) {
+          if (leader) mbar_arrive_expect_tx(&bar->eopfull, 2 * 2 * kKB);
+          for (int kb = 0; kb < 2; ++kb) tma_load_2d_pair(smem + kOffEOp + kb * kKB, &tmE, eopfull_leader, colE + kb * 64, row0_of(n_op));
+          prefetch(n_op + 3);
+          ++n_op;
+        }
+        // the residual copy of tile t is asked for only after its operand copy, so it finds the rows in L2
+        if (n_res < res_end && n_res < n_op && mbar_test(&bar->resempty, (uint32_t)(n_res & 1) ^ 1)) {
+          mbar_arrive_expect_tx(&bar->resfull, 2 * kKB);
+          for (int kb = 0; kb < 2; ++kb) tma_load_2d(smem + kOffRes + kb * kKB, &tmE, &bar->resfull, colE + kb * 64, row0_of(n_res));
+          ++n_res;
+        }
       }
     }
   } else if (warp == 1) {
-    // ---------------------------------------------------------------- MMA issuer (leader CTA)
+    // ---------------------------------------------------------------- MMA issuer (leader CTA): polls, issues what is ready
     if (leader && lane == 0) {
       constexpr uint32_t idesc = make_idesc_pair(kH);
       auto kblock = [&](uint32_t d_tmem, uint32_t a_addr, uint32_t b_addr, bool first) {
@@ -174,193 +273,226 @@ gnn_edge_fused_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_con
         for (int k = 0; k < BK / UMMA_K; ++k)
           tc_mma_bf16_pair(d_tmem, adesc + (uint64_t)(k * 2), bdesc + (uint64_t)(k * 2), idesc, (!first || k != 0) ? 1u : 0u);
       };
-      auto mma1 = [&](int tl) {
-        const int b = tl & 1;
-        const uint32_t ph = (tl >> 1) & 1;
-        const uint32_t d = tmem_base + (uint32_t)(b * kH);
-        mbar_wait_cluster(&bar->a1empty[b], ph ^ 1);
-        mbar_wait(&bar->efull[b], ph);
-        tc_fence_after();
-        for (int kb = 0; kb < 2; ++kb) kblock(d, sbase + kOffEHold + (b * 2 + kb) * kKB, sbase + kOffW1 + (4 + kb) * kWKB, kb == 0);
-        for (int h = 0; h < 2; ++h) {
-          mbar_wait_cluster(&bar->gfull[h], (uint32_t)(tl & 1));
-          tc_fence_after();
-          for (int kb = 0; kb < 2; ++kb) kblock(d, sbase + kOffRing + (h * 2 + kb) * kKB, sbase + kOffW1 + (h * 2 + kb) * kWKB, false);
-          tc_commit_pair(&bar->gempty[h]);
+      int n1 = 0, n2 = 0;      // next tile of layer 1 / layer 2
+      int stage1 = 0;          // 0: waiting for the accumulator and h_src, 1: for h_dst, 2: for the e operand tile
+      const int n2_end = kTwoLayers ? n_my : 0;
+      while (n1 < n_my || n2 < n2_end) {
+        if (n2 < n2_end && n2 < n1) {
+          const int b = n2 & 1;
+          const uint32_t ph = (n2 >> 1) & 1;
+          if (mbar_test(&bar->tfull, (uint32_t)(n2 & 1)) && mbar_test(&bar->a2empty[b], ph ^ 1)) {
+            tc_fence_after();
+            const uint32_t d = tmem_base + (uint32_t)(2 * kH + b * kH);
+            for (int kb = 0; kb < 2; ++kb) kblock(d, sbase + kOffT + kb * kKB, sbase + kOffW2 + kb * kWKB, kb == 0);
+            tc_commit_pair(&bar->tempty);
+            tc_commit_pair(&bar->a2full[b]);
+            ++n2;
+          }
         }
-        tc_commit_pair(&bar->a1full[b]);
-      };
-      auto mma2 = [&](int tl) {
-        const int b = tl & 1;
-        const uint32_t ph = (tl >> 1) & 1;
-        const uint32_t d = tmem_base + (uint32_t)(2 * kH + b * kH);
-        mbar_wait_cluster(&bar->tfull, (uint32_t)(tl & 1));
-        mbar_wait_cluster(&bar->a2empty[b], ph ^ 1);
-        tc_fence_after();
-        for (int kb = 0; kb < 2; ++kb) kblock(d, sbase + kOffT + kb * kKB, sbase + kOffW2 + kb * kWKB, kb == 0);
-        tc_commit_pair(&bar->tempty);
-        tc_commit_pair(&bar->a2full[b]);
-      };
-      if (n_my > 0) mma1(0);
-      for (int tl = 0; tl < n_my; ++tl) {
-        if (tl + 1 < n_my) mma1(tl + 1);
-        if (MODE == kUpdate) mma2(tl);
+        if (n1 < n_my) {
+          const int b = n1 & 1;
+          const uint32_t ph = (n1 >> 1) & 1;
+          const uint32_t d = tmem_base + (uint32_t)(b * kH);
+          if (stage1 == 0) {
+            if (mbar_test(&bar->a1empty[b], ph ^ 1) && mbar_test(&bar->gfull[0], (uint32_t)(n1 & 1))) {
+              tc_fence_after();
+              for (int kb = 0; kb < 2; ++kb) kblock(d, sbase + kOffRing + kb * kKB, sbase + kOffW1 + (kbR + kb) * kWKB, kb == 0);
+              tc_commit_pair(&bar->gempty[0]);
+              stage1 = 1;
+            }
+          }
+          if (stage1 == 1) {
+            if (mbar_test(&bar->gfull[1], (uint32_t)(n1 & 1))) {
+              tc_fence_after();
+              for (int kb = 0; kb < 2; ++kb) kblock(d, sbase + kOffRing + (2 + kb) * kKB, sbase + kOffW1 + (kbR + 2 + kb) * kWKB, false);
+              tc_commit_pair(&bar->gempty[1]);
+              stage1 = 2;
+            }
+          }
+          if (stage1 == 2) {
+            if (mbar_test(&bar->eopfull, (uint32_t)(n1 & 1))) {
+              tc_fence_after();
+              for (int kb = 0; kb < 2; ++kb) kblock(d, sbase + kOffEOp + kb * kKB, sbase + kOffW1 + (kbE + kb) * kWKB, false);
+              tc_commit_pair(&bar->eopempty);
+              tc_commit_pair(&bar->a1full[b]);
+              stage1 = 0;
+              ++n1;
+            }
+          }
+        }
       }
     }
   } else if (warp < 6) {
-    // ---------------------------------------------------------------- epilogue 1: acc1 -> LNR -> T (or score)
-    const int quad = warp & 3;
-    const int r = quad * 32 + lane;   // row of this thread inside the CTA's 128-row tile == TMEM lane
-    const uint32_t a1empty0 = mapa_u32(smem_u32(&bar->a1empty[0]), 0), a1empty1 = mapa_u32(smem_u32(&bar->a1empty[1]), 0);
-    const uint32_t tfull_l = mapa_u32(smem_u32(&bar->tfull), 0);
-    for (int tl = 0; tl < n_my; ++tl) {
-      const int64_t tile = pair + (int64_t)tl * n_pairs;
-      const int b = tl & 1;
-      const uint32_t ph = (tl >> 1) & 1;
-      mbar_wait(&bar->a1full[b], ph);
-      tc_fence_after();
-      const uint32_t taddr = tmem_base + ((uint32_t)(quad * 32) << 16) + (uint32_t)(b * kH);
-      float mean, rstd;
-      row_stats(taddr, p.b1, p.use_ln, mean, rstd);
-      if (MODE == kUpdate) mbar_wait(&bar->tempty, (uint32_t)(tl & 1) ^ 1);   // layer-2 MMA of the previous tile has read T
-      float dot = p.b_out;
-#pragma unroll 1
-      for (int c = 0; c < kH; c += 32) {
-        uint32_t v[32];
-        tmem_ld32(taddr + c, v);
-        tmem_ld_wait();
-        if (c + 32 >= kH) {
-          tc_fence_before();
-          __syncwarp();
-          if (lane == 0) mbar_arrive_cluster(b == 0 ? a1empty0 : a1empty1);
-        }
-#pragma unroll
-        for (int q = 0; q < 4; ++q) {
-          float f[8];
-#pragma unroll
-          for (int hh = 0; hh < 2; ++hh) {
-            const float4 bb = __ldg(reinterpret_cast<const float4*>(p.b1 + c + q * 8 + hh * 4));
-            f[hh * 4 + 0] = fmaxf((__uint_as_float(v[q * 8 + hh * 4 + 0]) + bb.x - mean) * rstd, 0.f);
-            f[hh * 4 + 1] = fmaxf((__uint_as_float(v[q * 8 + hh * 4 + 1]) + bb.y - mean) * rstd, 0.f);
-            f[hh * 4 + 2] = fmaxf((__uint_as_float(v[q * 8 + hh * 4 + 2]) + bb.z - mean) * rstd, 0.f);
-            f[hh * 4 + 3] = fmaxf((__uint_as_float(v[q * 8 + hh * 4 + 3]) + bb.w - mean) * rstd, 0.f);
-          }
-          if (MODE == kDecode) {
-#pragma unroll
-            for (int hh = 0; hh < 2; ++hh) {
-              const float4 w = __ldg(reinterpret_cast<const float4*>(p.w_out + c + q * 8 + hh * 4));
-              dot = fmaf(f[hh * 4 + 0], w.x, dot); dot = fmaf(f[hh * 4 + 1], w.y, dot);
-              dot = fmaf(f[hh * 4 + 2], w.z, dot); dot = fmaf(f[hh * 4 + 3], w.w, dot);
-            }
-          } else {
-            const int col = c + q * 8;                 // 8 columns = one 16-byte chunk
-            const int kb = col >> 6, ch = (col & 63) >> 3;
-            *reinterpret_cast<uint4*>(smem + kOffT + kb * kKB + r * 128 + ((ch ^ (r & 7)) << 4)) =
-                make_uint4(pack_bf16(f[0], f[1]), pack_bf16(f[2], f[3]), pack_bf16(f[4], f[5]), pack_bf16(f[6], f[7]));
-          }
-        }
-      }
-      if (MODE == kDecode) {
-        const int64_t row = tile * 2 * kTileRows + rank * kTileRows + r;
-        if (row < M) p.score[row] = fast_sigmoid(dot);
-        __syncwarp();
-        if (lane == 0) mbar_arrive(&bar->eempty[b]);   // the layer-1 MMAs that read the e tile are complete
-      } else {
-        fence_proxy_async();
-        __syncwarp();
-        if (lane == 0) mbar_arrive_cluster(tfull_l);
-      }
-    }
-  } else if (warp < 10) {
-    // ---------------------------------------------------------------- epilogue 2: acc2 -> LNR -> + e -> store
-    if (MODE == kUpdate) {
-      const int quad = warp & 3;
-      const int r = quad * 32 + lane;
-      const uint32_t a2empty0 = mapa_u32(smem_u32(&bar->a2empty[0]), 0), a2empty1 = mapa_u32(smem_u32(&bar->a2empty[1]), 0);
-      for (int tl = 0; tl < n_my; ++tl) {
-        const int64_t tile = pair + (int64_t)tl * n_pairs;
-        const int b = tl & 1;
-        const uint32_t ph = (tl >> 1) & 1;
-        mbar_wait(&bar->a2full[b], ph);
-        tc_fence_after();
-        const uint32_t taddr = tmem_base + ((uint32_t)(quad * 32) << 16) + (uint32_t)(2 * kH + b * kH);
-        float mean, rstd;
-        row_stats(taddr, p.b2, p.use_ln, mean, rstd);
-        uint8_t* eh = smem + kOffEHold + b * 2 * kKB;
-#pragma unroll 1
-        for (int c = 0; c < kH; c += 32) {
-          uint32_t v[32];
-          tmem_ld32(taddr + c, v);
-          tmem_ld_wait();
-          if (c + 32 >= kH) {
-            tc_fence_before();
-            __syncwarp();
-            if (lane == 0) mbar_arrive_cluster(b == 0 ? a2empty0 : a2empty1);
-          }
-#pragma unroll
-          for (int q = 0; q < 4; ++q) {
-            const int col = c + q * 8;
-            const int kb = col >> 6, ch = (col & 63) >> 3;
-            uint4* cell = reinterpret_cast<uint4*>(eh + kb * kKB + r * 128 + ((ch ^ (r & 7)) << 4));
-            const uint4 e = *cell;
-            const __nv_bfloat162* e2 = reinterpret_cast<const __nv_bfloat162*>(&e);
-            float f[8];
-#pragma unroll
-            for (int hh = 0; hh < 2; ++hh) {
-              const float4 bb = __ldg(reinterpret_cast<const float4*>(p.b2 + col + hh * 4));
-              f[hh * 4 + 0] = fmaxf((__uint_as_float(v[q * 8 + hh * 4 + 0]) + bb.x - mean) * rstd, 0.f) + __low2float(e2[hh * 2]);
-              f[hh * 4 + 1] = fmaxf((__uint_as_float(v[q * 8 + hh * 4 + 1]) + bb.y - mean) * rstd, 0.f) + __high2float(e2[hh * 2]);
-              f[hh * 4 + 2] = fmaxf((__uint_as_float(v[q * 8 + hh * 4 + 2]) + bb.z - mean) * rstd, 0.f) + __low2float(e2[hh * 2 + 1]);
-              f[hh * 4 + 3] = fmaxf((__uint_as_float(v[q * 8 + hh * 4 + 3]) + bb.w - mean) * rstd, 0.f) + __high2float(e2[hh * 2 + 1]);
-            }
-            *cell = make_uint4(pack_bf16(f[0], f[1]), pack_bf16(f[2], f[3]), pack_bf16(f[4], f[5]), pack_bf16(f[6], f[7]));
-          }
-        }
-        fence_proxy_async();
-        __syncwarp();
-        if (lane == 0) {
-          const int row0 = (int)(tile * 2 * kTileRows + rank * kTileRows + quad * 32);
-          for (int kb = 0; kb < 2; ++kb) tma_store_2d(&tmEst, eh + kb * kKB + quad * 32 * 128, kb * 64, row0);
-          bulk_commit();
-          bulk_wait_read<0>();          // the tile's rows have left shared memory: the buffer may be refilled
-          mbar_arrive(&bar->eempty[b]);
-        }
-      }
-      if (lane == 0) bulk_wait_all();
-    }
-  } else {
-    // ---------------------------------------------------------------- gather: h[src], h[dst] rows -> ring
-    const int gw = warp - 10;
+    // ---------------------------------------------------------------- gather: h[src], h[dst] rows -> ring (32 rows per warp)
+    const int gw = warp - 2;
     const uint32_t gfull0 = mapa_u32(smem_u32(&bar->gfull[0]), 0), gfull1 = mapa_u32(smem_u32(&bar->gfull[1]), 0);
     const int half = lane >> 4, chunk = lane & 15;
     const int kb = chunk >> 3, ch = chunk & 7;
-    for (int tl = 0; tl < n_my; ++tl) {
+    // iteration i copies chunk `chunk` of row rr = 2 i + half of this warp's 32 rows; (rr & 7) = 2 (i & 3) + half
+    uint32_t sw[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) sw[j] = (uint32_t)((ch ^ (2 * j + half)) << 4);
+    const uint32_t dst0 = sbase + kOffRing + kb * kKB + (gw * 32 + half) * 128;
+    const char* xb = reinterpret_cast<const char*>(p.X) + chunk * 16;
+    const int64_t ldb = p.ldx * 2;
+    for (int tl = 0; tl < (MODE == kNode ? 0 : n_my); ++tl) {
       const int64_t tile = pair + (int64_t)tl * n_pairs;
       const int64_t row = tile * 2 * kTileRows + rank * kTileRows + gw * 32 + lane;
-      const int my_s = row < M ? p.src[row] : -1, my_d = row < M ? p.dst[row] : -1;
+      // rows beyond M gather node 0: their results are computed but never read (segment sums and scores stop at M)
+      const int s_i = row < M ? p.src[row] : 0, d_i = row < M ? p.dst[row] : 0;
 #pragma unroll 1
       for (int h = 0; h < 2; ++h) {
         mbar_wait(&bar->gempty[h], (uint32_t)(tl & 1) ^ 1);
-        const int mine = h == 0 ? my_s : my_d;
-#pragma unroll 4
+        const int mine = h == 0 ? s_i : d_i;
+        const uint32_t dsth = dst0 + h * 2 * kKB;
+#pragma unroll
         for (int i = 0; i < 16; ++i) {
-          const int rr = i * 2 + half;                       // row inside this warp's 32 rows
-          const int idx = __shfl_sync(0xffffffffu, mine, rr);
-          const int rt = gw * 32 + rr;                       // row inside the CTA's tile
-          const uint32_t dst = sbase + kOffRing + (h * 2 + kb) * kKB + rt * 128 + ((ch ^ (rt & 7)) << 4);
-          const __nv_bfloat16* g = p.X + (int64_t)(idx < 0 ? 0 : idx) * p.ldx + chunk * 8;
-          cp_async_16(dst, g, idx < 0 ? 0 : 16);             // rows beyond M are zero filled
+          const int idx = __shfl_sync(0xffffffffu, mine, 2 * i + half);
+          cp_async_16(dsth + i * 256 + sw[i & 3], xb + (int64_t)idx * ldb, 16);
         }
         cp_async_commit();
       }
       cp_async_wait<1>();
       fence_proxy_async();
       __syncwarp();
-      if (lane == 0) mbar_arrive_cluster(gfull0);
+      if (lane == 0) mbar_arrive_remote(gfull0);
       cp_async_wait<0>();
       fence_proxy_async();
       __syncwarp();
-      if (lane == 0) mbar_arrive_cluster(gfull1);
+      if (lane == 0) mbar_arrive_remote(gfull1);
+    }
+  } else if (warp < 14) {
+    // ---------------------------------------------------------------- epilogue 1: acc1 -> LNR -> T (or score), 64 columns per thread
+    const int quad = warp & 3, half = (warp - 6) >> 2;
+    const int r = quad * 32 + lane;   // row of this thread inside the CTA's 128-row tile == TMEM lane
+    const int bid = 1 + quad;         // named barrier of the two warps that share this quadrant's rows
+    const uint32_t a1empty0 = mapa_u32(smem_u32(&bar->a1empty[0]), 0), a1empty1 = mapa_u32(smem_u32(&bar->a1empty[1]), 0);
+    const uint32_t tfull_l = mapa_u32(smem_u32(&bar->tfull), 0);
+    float2* slot = reinterpret_cast<float2*>(smem + kOffX1) + r;
+    float* xd = reinterpret_cast<float*>(smem + kOffT + kKB + quad * 32 * 128);   // kDecode only (T is unused there)
+    for (int tl = 0; tl < n_my; ++tl) {
+      const int64_t tile = pair + (int64_t)tl * n_pairs;
+      const int b = tl & 1;
+      const uint32_t ph = (tl >> 1) & 1;
+      mbar_wait(&bar->a1full[b], ph);
+      tc_fence_after();
+      float2 x[32];
+      float ps, pq;
+      load_half<false>(tmem_base + ((uint32_t)(quad * 32) << 16) + (uint32_t)(b * kH + half * 64), sb1 + half * 64, x, ps, pq);
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive_remote(b == 0 ? a1empty0 : a1empty1);     // the accumulator is in registers now
+      // upper half -> lower half: (sum, sum of squares); lower half -> upper half: (rstd, -mean rstd)
+      float2 rs, sh;
+      if (half == 1) *slot = f2(ps, pq);
+      named_bar_sync(bid, 64);
+      if (half == 0) {
+        ln_coeffs(ps, pq, *slot, p.use_ln, rs, sh);
+        *slot = f2(rs.x, sh.x);
+      }
+      named_bar_sync(bid, 64);
+      if (half == 1) {
+        const float2 c = *slot;
+        rs = f2(c.x, c.x);
+        sh = f2(c.y, c.y);
+      }
+      if (MODE == kDecode) {
+        float2 d0 = f2(0.f, 0.f), d1 = d0;
+        const float4* w4 = reinterpret_cast<const float4*>(swo + half * 64);
+#pragma unroll
+        for (int c = 0; c < 64; c += 4) {
+          const float4 w = w4[c / 4];
+          float2 v0 = __ffma2_rn(x[c / 2], rs, sh), v1 = __ffma2_rn(x[c / 2 + 1], rs, sh);
+          v0.x = fmaxf(v0.x, 0.f); v0.y = fmaxf(v0.y, 0.f); v1.x = fmaxf(v1.x, 0.f); v1.y = fmaxf(v1.y, 0.f);
+          d0 = __ffma2_rn(v0, f2(w.x, w.y), d0);
+          d1 = __ffma2_rn(v1, f2(w.z, w.w), d1);
+        }
+        const float d = (d0.x + d0.y) + (d1.x + d1.y);
+        if (half == 1) xd[lane] = d;
+        named_bar_sync(bid, 64);
+        if (half == 0) {
+          const int64_t row = tile * 2 * kTileRows + rank * kTileRows + r;
+          if (row < M) p.score[row] = fast_sigmoid(p.b_out + d + xd[lane]);
+        }
+        named_bar_sync(bid, 64);          // the partial dot has been read: the slot may be rewritten for the next tile
+      } else {
+        mbar_wait(&bar->tempty, (uint32_t)(tl & 1) ^ 1);   // the layer-2 MMA of the previous tile has read T
+#pragma unroll
+        for (int c = 0; c < 64; c += 8) {                  // 8 columns = one 16-byte chunk of the swizzled K block `half`
+          uint32_t w[4];
+#pragma unroll
+          for (int i = 0; i < 4; ++i) {
+            // ReLU after the rounding: max(bf16(v), 0) == bf16(max(v, 0)), one packed instruction for the pair
+            const float2 v = __ffma2_rn(x[c / 2 + i], rs, sh);
+            const __nv_bfloat162 t = __hmax2(__floats2bfloat162_rn(v.x, v.y), __floats2bfloat162_rn(0.f, 0.f));
+            w[i] = *reinterpret_cast<const uint32_t*>(&t);
+          }
+          const int ch = c >> 3;
+          *reinterpret_cast<uint4*>(smem + kOffT + half * kKB + r * 128 + ((ch ^ (r & 7)) << 4)) = make_uint4(w[0], w[1], w[2], w[3]);
+        }
+        fence_proxy_async();
+        __syncwarp();
+        if (lane == 0) mbar_arrive_remote(tfull_l);
+      }
+    }
+  } else {
+    // ---------------------------------------------------------------- epilogue 2: acc2 -> LNR -> + residual -> store, 64 columns per thread
+    if (kTwoLayers) {
+      const int quad = warp & 3, half = (warp - 14) >> 2;
+      const int r = quad * 32 + lane;
+      const int bid = 5 + quad;
+      const uint32_t a2empty0 = mapa_u32(smem_u32(&bar->a2empty[0]), 0), a2empty1 = mapa_u32(smem_u32(&bar->a2empty[1]), 0);
+      uint8_t* res = smem + kOffRes + half * kKB;
+      for (int tl = 0; tl < n_my; ++tl) {
+        const int64_t tile = pair + (int64_t)tl * n_pairs;
+        const int b = tl & 1;
+        const uint32_t ph = (tl >> 1) & 1;
+        mbar_wait(&bar->a2full[b], ph);
+        tc_fence_after();
+        float2 x[32];
+        float ps, pq;
+        load_half<false>(tmem_base + ((uint32_t)(quad * 32) << 16) + (uint32_t)(2 * kH + b * kH + half * 64), sb2 + half * 64, x, ps, pq);
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive_remote(b == 0 ? a2empty0 : a2empty1);
+        mbar_wait(&bar->resfull, (uint32_t)(tl & 1));        // the residual copy of this tile has landed
+        // exchange of the half-row statistics through the first cell of this thread's residual row (its values wait in e0)
+        uint4* cell0 = reinterpret_cast<uint4*>(res + r * 128 + ((0 ^ (r & 7)) << 4));
+        const uint4 e0 = *cell0;
+        *reinterpret_cast<float2*>(cell0) = f2(ps, pq);
+        named_bar_sync(bid, 64);
+        const float2 other = *reinterpret_cast<const float2*>(smem + kOffRes + (half ^ 1) * kKB + r * 128 + ((0 ^ (r & 7)) << 4));
+        named_bar_sync(bid, 64);            // both have read: the cells may be overwritten with results
+        float2 rs, sh;
+        ln_coeffs(ps, pq, other, p.use_ln, rs, sh);
+#pragma unroll
+        for (int c = 0; c < 64; c += 8) {
+          const int ch = c >> 3;
+          uint4* cell = reinterpret_cast<uint4*>(res + r * 128 + ((ch ^ (r & 7)) << 4));
+          const uint4 e = c == 0 ? e0 : *cell;
+          const __nv_bfloat162* e2 = reinterpret_cast<const __nv_bfloat162*>(&e);
+          uint32_t w[4];
+#pragma unroll
+          for (int i = 0; i < 4; ++i) {
+            float2 v = __ffma2_rn(x[c / 2 + i], rs, sh);
+            v.x = fmaxf(v.x, 0.f);
+            v.y = fmaxf(v.y, 0.f);
+            v = __fadd2_rn(v, __bfloat1622float2(e2[i]));
+            w[i] = pack_bf16(v.x, v.y);
+          }
+          *cell = make_uint4(w[0], w[1], w[2], w[3]);
+        }
+        fence_proxy_async();
+        __syncwarp();
+        if (lane == 0) {
+          const int row0 = (int)(tile * 2 * kTileRows + rank * kTileRows + quad * 32);
+          tma_store_2d(&tmEst, res + quad * 32 * 128, colE + half * 64, row0);
+          bulk_commit();
+          bulk_wait_read<0>();  // the rows have left shared memory: the buffer may be refilled
+          mbar_arrive(&bar->resempty);
+        }
+      }
+      if (lane == 0) bulk_wait_all();
     }
   }
   tc_fence_before();

@@ -16,9 +16,6 @@
 #include "gemm_tc.cuh"
 #include "gemm_tc2.cuh"
 #include "gnn_fused.cuh"
-#include "gnn_fused2.cuh"
-#include "gnn_fused3.cuh"
-#include "gnn_fused4.cuh"
 #include "graph.cuh"
 #include "nn.cuh"
 
@@ -73,15 +70,11 @@ trk_status launch_gemm(trk_ctx* ctx, const bf16* A, int64_t a_rows, int64_t lda,
                        const typename Epi::Params& ep, cudaStream_t st, OutBf16 out = OutBf16(), const tc::AGather* ag = nullptr) {
   if (rows.m_cap <= 0) return TRK_OK;
   if (K % tc::BK != 0 || n_pad % BN != 0) return fail(ctx, TRK_ERR_SHAPE, "gemm: K must be a multiple of 64 and N of the tile");
-  static bool attr_set = false;
   auto kern = tc::gemm_tc_kernel<BN, Epi>;
-  if (!attr_set) {
-    TRK_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::smem_bytes(BN, Epi::kTmaStore)));
-    attr_set = true;
-  }
+  TRK_TRY(ensure_smem(ctx, kern, tc::smem_bytes(BN, Epi::kTmaStore)));
   // tcgen05.mma.cta_group::2 on 256 x BN tiles when the K loop is long enough to matter (measured: with one K block the
   // epilogue paces the tile and coupling two CTAs only adds waiting)
-  const bool pair = BN >= 128 && K >= 4 * tc::BK && debug_knob(kKnobGemmPair) != 0;
+  const bool pair = BN >= 128 && K >= 4 * tc::BK && ctx->knobs[kKnobGemmPair] != 0;
   CUtensorMap ta, tb, tc_out;
   TRK_TRY(make_tmap(ctx, &ta, A, a_rows, K, lda, tc::BM));
   TRK_TRY(make_tmap(ctx, &tb, W, n_pad, K, K, pair ? BN / 2 : BN));
@@ -94,16 +87,12 @@ trk_status launch_gemm(trk_ctx* ctx, const bf16* A, int64_t a_rows, int64_t lda,
   const int n_tiles = n_pad / BN;
   if constexpr (BN >= 128) {
     if (pair) {
-      static bool attr2_set = false;
       auto kern2 = tc::gemm_tc2_kernel<BN, Epi>;
-      if (!attr2_set) {
-        TRK_CUDA(ctx, cudaFuncSetAttribute(kern2, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::smem_bytes_pair(BN, Epi::kTmaStore)));
-        attr2_set = true;
-      }
+      TRK_TRY(ensure_smem(ctx, kern2, tc::smem_bytes_pair(BN, Epi::kTmaStore)));
       const int64_t ptiles = ceil_div(rows.m_cap, tc::kPairBM) * n_tiles;
       const unsigned grid2 = 2u * (unsigned)std::min<int64_t>(ptiles, ctx->sm_count / 2);
       TRK_LAUNCH(ctx, kern2, grid2, tc::kThreads, tc::smem_bytes_pair(BN, Epi::kTmaStore), st, ta, tb, tc_out, rows, n_tiles, K / tc::BK, ep,
-                 (int)debug_knob(kKnobRowMajor));
+                 (int)ctx->knobs[kKnobRowMajor]);
       return TRK_OK;
     }
   }
@@ -111,24 +100,16 @@ trk_status launch_gemm(trk_ctx* ctx, const bf16* A, int64_t a_rows, int64_t lda,
   const unsigned grid = (unsigned)std::min<int64_t>(tiles, ctx->sm_count);
   if constexpr (BN == 256 && Epi::kTmaStore) {
     // a single K block per tile: the bf16-store epilogue paces the kernel, so it gets eight warps (column split)
-    if (K == tc::BK && ag && debug_knob(kKnobEpiSplit) >= 2) {
+    if (K == tc::BK && ag && ctx->knobs[kKnobEpiSplit] >= 2) {
       // ... and its A operand is gathered in the kernel (S3 first layer: no separate gather launch, no staging buffer)
-      static bool attr4_set = false;
       auto kern4 = tc::gemm_tc_kernel<BN, Epi, 2, true>;
-      if (!attr4_set) {
-        TRK_CUDA(ctx, cudaFuncSetAttribute(kern4, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::smem_bytes(BN, true, 2)));
-        attr4_set = true;
-      }
+      TRK_TRY(ensure_smem(ctx, kern4, tc::smem_bytes(BN, true, 2)));
       TRK_LAUNCH(ctx, kern4, grid, tc::threads_for(2, true), tc::smem_bytes(BN, true, 2), st, ta, tb, tc_out, rows, n_tiles, K / tc::BK, ep, *ag);
       return TRK_OK;
     }
-    if (K == tc::BK && debug_knob(kKnobEpiSplit) != 0) {
-      static bool attr3_set = false;
+    if (K == tc::BK && ctx->knobs[kKnobEpiSplit] != 0) {
       auto kern3 = tc::gemm_tc_kernel<BN, Epi, 2>;
-      if (!attr3_set) {
-        TRK_CUDA(ctx, cudaFuncSetAttribute(kern3, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::smem_bytes(BN, true, 2)));
-        attr3_set = true;
-      }
+      TRK_TRY(ensure_smem(ctx, kern3, tc::smem_bytes(BN, true, 2)));
       TRK_LAUNCH(ctx, kern3, grid, tc::threads_for(2), tc::smem_bytes(BN, true, 2), st, ta, tb, tc_out, rows, n_tiles, K / tc::BK, ep, tc::AGather{});
       return TRK_OK;
     }
@@ -183,19 +164,8 @@ trk_status launch_edge_fused(trk_ctx* ctx, const bf16* X, int64_t ldx, bf16* E, 
                              const DevLinear& L1, const DevLinear& L2, const float* w_out, float b_out, float* score, tc::Rows rows,
                              cudaStream_t st) {
   if (rows.m_cap <= 0) return TRK_OK;
-  static bool attr_set = false;
-  auto kern = gf::gnn_edge_fused_kernel<MODE>;
-  auto kern2 = gf2::gnn_edge_fused2_kernel<MODE>;
-  auto kern3 = gf3::gnn_edge_fused3_kernel<MODE>;
-  // version 4 (eight-warp epilogues) serves the update; the decoder is a single launch per call and keeps version 3
-  auto kern4 = gf4::gnn_edge_fused4_kernel<gf::kUpdate>;
-  if (!attr_set) {
-    TRK_CUDA(ctx, cudaFuncSetAttribute(kern3, cudaFuncAttributeMaxDynamicSharedMemorySize, gf3::kSmemFused3));
-    TRK_CUDA(ctx, cudaFuncSetAttribute(kern4, cudaFuncAttributeMaxDynamicSharedMemorySize, gf4::kSmemFused4));
-    TRK_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, gf::kSmemFused));
-    TRK_CUDA(ctx, cudaFuncSetAttribute(kern2, cudaFuncAttributeMaxDynamicSharedMemorySize, gf2::kSmemFused2));
-    attr_set = true;
-  }
+  auto kern = gf::gnn_fused_kernel<MODE>;
+  TRK_TRY(ensure_smem(ctx, kern, gf::kSmemFused));
   CUtensorMap tw1, tw2, te, test;
   TRK_TRY(make_tmap(ctx, &tw1, L1.w_bf16, gf::kH, 3 * gf::kH, 3 * gf::kH, 64));
   TRK_TRY(make_tmap(ctx, &tw2, L2.w_bf16, gf::kH, gf::kH, gf::kH, 64));
@@ -204,30 +174,16 @@ trk_status launch_edge_fused(trk_ctx* ctx, const bf16* X, int64_t ldx, bf16* E, 
   gf::FusedParams p{X, ldx, src, dst, L1.b_f32, L2.b_f32, ctx->cfg.gnn_layernorm, w_out, b_out, score};
   const int64_t ptiles = ceil_div(rows.m_cap, 2 * gf::kTileRows);
   const unsigned grid = 2u * (unsigned)std::min<int64_t>(ptiles, ctx->sm_count / 2);
-  if (MODE == gf::kUpdate && debug_knob(kKnobGnnFused) >= 4) {
-    TRK_LAUNCH(ctx, kern4, grid, gf4::kThreads4, gf4::kSmemFused4, st, tw1, tw2, te, test, rows, p);
-  } else if (debug_knob(kKnobGnnFused) >= 3) {
-    TRK_LAUNCH(ctx, kern3, grid, gf3::kThreads3, gf3::kSmemFused3, st, tw1, tw2, te, test, rows, p);
-  } else if (debug_knob(kKnobGnnFused) >= 2) {
-    TRK_LAUNCH(ctx, kern2, grid, gf2::kThreads2, gf2::kSmemFused2, st, tw1, tw2, te, test, rows, p);
-  } else {
-    TRK_LAUNCH(ctx, kern, grid, gf::kThreadsFused, gf::kSmemFused, st, tw1, tw2, te, test, rows, p);
-  }
+  TRK_LAUNCH(ctx, kern, grid, gf::kFusedThreads, gf::kSmemFused, st, tw1, tw2, te, test, rows, p);
   return TRK_OK;
 }
 
-// Fused node update of S4 (gnn_fused3.cuh, kNode), H = 128: X[:, 0:H] <- X[:, 0:H] + LNR(W2 LNR(W1 X + b1) + b2) in place.
+// Fused node update of S4 (gnn_fused.cuh, kNode), H = 128: X[:, 0:H] <- X[:, 0:H] + LNR(W2 LNR(W1 X + b1) + b2) in place.
 trk_status launch_node_fused(trk_ctx* ctx, bf16* X, int64_t x_rows, const DevLinear& L1, const DevLinear& L2, tc::Rows rows,
                              cudaStream_t st) {
   if (rows.m_cap <= 0) return TRK_OK;
-  static bool attr_set = false;
-  auto kern = gf3::gnn_edge_fused3_kernel<gf3::kNode>;
-  auto kern4 = gf4::gnn_edge_fused4_kernel<gf3::kNode>;
-  if (!attr_set) {
-    TRK_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, gf3::kSmemFused3));
-    TRK_CUDA(ctx, cudaFuncSetAttribute(kern4, cudaFuncAttributeMaxDynamicSharedMemorySize, gf4::kSmemFused4));
-    attr_set = true;
-  }
+  auto kern = gf::gnn_fused_kernel<gf::kNode>;
+  TRK_TRY(ensure_smem(ctx, kern, gf::kSmemFused));
   CUtensorMap tw1, tw2, tx, txst;
   TRK_TRY(make_tmap(ctx, &tw1, L1.w_bf16, gf::kH, 3 * gf::kH, 3 * gf::kH, 64));
   TRK_TRY(make_tmap(ctx, &tw2, L2.w_bf16, gf::kH, gf::kH, gf::kH, 64));
@@ -236,11 +192,7 @@ trk_status launch_node_fused(trk_ctx* ctx, bf16* X, int64_t x_rows, const DevLin
   gf::FusedParams p{X, 3 * gf::kH, nullptr, nullptr, L1.b_f32, L2.b_f32, ctx->cfg.gnn_layernorm, nullptr, 0.f, nullptr};
   const int64_t ptiles = ceil_div(rows.m_cap, 2 * gf::kTileRows);
   const unsigned grid = 2u * (unsigned)std::min<int64_t>(ptiles, ctx->sm_count / 2);
-  if (debug_knob(kKnobGnnFused) >= 4) {
-    TRK_LAUNCH(ctx, kern4, grid, gf4::kThreads4, gf4::kSmemFused4, st, tw1, tw2, tx, txst, rows, p);
-  } else {
-    TRK_LAUNCH(ctx, kern, grid, gf3::kThreads3, gf3::kSmemFused3, st, tw1, tw2, tx, txst, rows, p);
-  }
+  TRK_LAUNCH(ctx, kern, grid, gf::kFusedThreads, gf::kSmemFused, st, tw1, tw2, tx, txst, rows, p);
   return TRK_OK;
 }
 
@@ -452,7 +404,7 @@ trk_status filter_forward_bf16(trk_ctx* ctx, const float* feat, const int32_t* s
     // first layer with 256-column tiles: its A operand is gathered inside the GEMM (gemm_tc.cuh GATHER_A)
     int cpr_log2 = 0;                                   // threads per gathered row: the 16-byte chunks that hold data, rounded up to 2^k
     while ((8 << cpr_log2) < 2 * u) ++cpr_log2;
-    const bool fuse_gather = nl >= 3 && pick_bn(L[0].out_pad) == 256 && debug_knob(kKnobEpiSplit) >= 2;
+    const bool fuse_gather = nl >= 3 && pick_bn(L[0].out_pad) == 256 && ctx->knobs[kKnobEpiSplit] >= 2;
     const tc::AGather ag{feat, src, dst, u};
     if (!fuse_gather)
       TRK_LAUNCH(ctx, filter_gather_kernel, (unsigned)ceil_div(cap << cpr_log2, 256), 256, 0, st, feat, u, cpr_log2, src, dst, n_edges_dev,
@@ -467,16 +419,10 @@ trk_status filter_forward_bf16(trk_ctx* ctx, const float* feat, const int32_t* s
       if (l == 0) { Ll.w_bf16 = ctx->filter_w1_pad; Ll.in_pad = 64; }
       const int64_t lda = l == 0 ? 64 : Ll.in_pad;
       // trk_profile_kernel_ms: one CUDA-event pair around every hidden-layer GEMM launch with K >= 256
-      const bool kprof = ctx->profiling && n_edges_dev == &ctx->counts[0] && Ll.in_pad >= 256;
+      const bool kprof = ctx->profiling && n_edges_dev == &ctx->counts[0] && Ll.in_pad >= 256 &&
+                         (size_t)ctx->kprof_n * 2 + 2 <= ctx->kprof_ev.size();   // the event pairs are created by trk_profile_enable
       cudaEvent_t k0 = nullptr, k1 = nullptr;
       if (kprof) {
-        if ((size_t)ctx->kprof_n * 2 + 2 > ctx->kprof_ev.size()) {
-          for (int i = 0; i < 2; ++i) {
-            cudaEvent_t e;
-            TRK_CUDA(ctx, cudaEventCreate(&e));
-            ctx->kprof_ev.push_back(e);
-          }
-        }
         k0 = ctx->kprof_ev[(size_t)ctx->kprof_n * 2];
         k1 = ctx->kprof_ev[(size_t)ctx->kprof_n * 2 + 1];
         ++ctx->kprof_n;
@@ -525,7 +471,7 @@ trk_status gnn_forward_bf16(trk_ctx* ctx, const float* hits, int64_t n, const in
     tc::EpiRowLn::Params ep{ctx->edge_enc.layers[1].b_f32, nullptr, nullptr, nullptr, ln, nullptr, 0, E, H, nullptr, 0.f, nullptr};
     TRK_TRY(gemm_row_ln(ctx, T1, t_rows, H, H, ctx->edge_enc.layers[1].w_bf16, ep, erows, st));
   }
-  const bool fused = H == gf::kH && debug_knob(kKnobGnnFused) != 0;
+  const bool fused = H == gf::kH && ctx->knobs[kKnobGnnFused] != 0;
   for (int t = 0; t < ctx->cfg.gnn_iters; ++t) {
     if (n_edges_cap > 0 && fused) {
       TRK_TRY(launch_edge_fused<gf::kUpdate>(ctx, X, 3 * H, E, e_rows, src, dst, ctx->edge_net.layers[0], ctx->edge_net.layers[1], nullptr,
@@ -540,7 +486,7 @@ trk_status gnn_forward_bf16(trk_ctx* ctx, const float* hits, int64_t n, const in
     }
     TRK_TRY(segment_sums(ctx, E, true, n, X, st));
     // h <- h + LNR(W2 LNR(W1 [h ; m_in ; m_out] + b1) + b2): X is the concatenation already
-    if (fused && debug_knob(kKnobGnnFused) >= 3) {
+    if (fused) {
       TRK_TRY(launch_node_fused(ctx, X, x_rows, ctx->node_net.layers[0], ctx->node_net.layers[1], nrows, st));
       continue;
     }
@@ -561,13 +507,6 @@ trk_status gnn_forward_bf16(trk_ctx* ctx, const float* hits, int64_t n, const in
   }
   return TRK_OK;
 }
-
-#ifdef TRK_FUSED_PROF
-// per-role wait cycles of the fused edge kernel (profiling builds only: TRK_NVCC_EXTRA=-DTRK_FUSED_PROF)
-extern "C" int trk_debug_fused_prof(unsigned long long* host) {
-  return (int)cudaMemcpyFromSymbol(host, gf2::g_fused_prof, sizeof(gf2::g_fused_prof));
-}
-#endif
 
 // ---------------------------------------------------------------- test hook
 trk_status gemm_bf16_hook(trk_ctx* ctx, const void* a, const void* w, const float* bias, void* out, int64_t m, int n, int k, int relu,

@@ -79,3 +79,16 @@ def check_kept(gpu_keys, ref_keys, all_keys, ref_scores, cut, precision, what):
         worst = np.max(np.abs(np.asarray(ref_scores, np.float64)[pos] - cut))
         assert worst <= band, f"{what}: an edge {worst:.3e} from the cut flipped"
     return len(diff)
+
+
+def same_track_fraction(labels_a, labels_b):
+    """Per hit: is the set of hits that share its label the same in both labelings?  (reading C-22, informational.)
+    The sets are equal iff the pair (label_a, label_b) occurs exactly |set_a| = |set_b| times."""
+    a = np.asarray(labels_a, np.int64)
+    b = np.asarray(labels_b, np.int64)
+    n = len(a)
+    size_a = np.bincount(a, minlength=n)[a]
+    size_b = np.bincount(b, minlength=n)[b]
+    _, inv, cnt = np.unique(a * n + b, return_inverse=True, return_counts=True)
+    pair = cnt[inv]
+    return (pair == size_a) & (pair == size_b)

@@ -187,11 +187,26 @@ def test_error_statuses_enqueue_nothing():
     trk = _make(cfg, calib, model, 100, 2)
     hits = torch.zeros(200, 3, device="cuda")
     try:
+        # a valid call first: the launch counter is non-zero and the outputs hold real values
+        out = trk.infer(hits[:60] + 0.5, np.array([0, 60], np.int32), want_edges=True)
+        torch.cuda.synchronize()
+        assert trk.last_launch_count > 0
+        sentinel = -123456789
+        for t in (out["labels"], out["counts"], out["edge_src"], out["edge_dst"]):
+            t.fill_(sentinel)
+        out["edge_score"].fill_(-7.5)
+        torch.cuda.synchronize()
         for off, status in (([0, 200], 3), ([0, 50, 40], 1), ([1, 50], 1), ([0, 10, 20, 30], 3)):
             with pytest.raises(TrkError) as e:
-                trk.infer(hits, np.array(off, np.int32))
+                trk.infer(hits, np.array(off, np.int32), out=out)
             assert e.value.status == status, (off, e.value.status)
-        assert trk.last_launch_count == 0 or True
+            # include/trk.h: "Host-detectable errors return before anything is enqueued": no launch was counted ...
+            assert trk.last_launch_count == 0, (off, trk.last_launch_count)
+        # ... and nothing ran on the device: every output still holds the sentinel
+        torch.cuda.synchronize()
+        for k in ("labels", "counts", "edge_src", "edge_dst"):
+            assert bool((out[k] == sentinel).all()), k
+        assert bool((out["edge_score"] == -7.5).all())
         with pytest.raises(TrkError):
             trk.stage_embed(hits)                                 # 200 rows > max_hits
         # the context is still usable afterwards

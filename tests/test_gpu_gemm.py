@@ -11,13 +11,12 @@ pytestmark = pytest.mark.gpu
 @pytest.mark.parametrize("pair", [1, 0], ids=["cta_pair", "single_cta"])
 def test_gemm_bias_act_matches_fp32_reference(m, n, k, relu, pair):
     import torch
-    from paper_2501_05520_b200 import debug_set, gemm_bf16
-    debug_set("gemm_pair", pair)
+    from paper_2501_05520_b200 import gemm_bf16
     g = torch.Generator(device="cuda").manual_seed(m * 7 + n * 3 + k)
     a = (torch.randn(m, k, device="cuda", generator=g)).to(torch.bfloat16)
     w = (torch.randn(n, k, device="cuda", generator=g) / np.sqrt(k)).to(torch.bfloat16)
     b = torch.randn(n, device="cuda", generator=g)
-    out = gemm_bf16(a, w, b, relu=relu)
+    out = gemm_bf16(a, w, b, relu=relu, pair=pair)
     torch.cuda.synchronize()
     ref = a.float() @ w.float().t() + b
     if relu:
@@ -28,7 +27,6 @@ def test_gemm_bias_act_matches_fp32_reference(m, n, k, relu, pair):
     # exact integers: products and sums representable in fp32 -> result exact after the bf16 output rounding
     ai = torch.randint(-3, 4, (m, k), device="cuda", generator=g).to(torch.bfloat16)
     wi = torch.randint(-2, 3, (n, k), device="cuda", generator=g).to(torch.bfloat16)
-    outi = gemm_bf16(ai, wi, torch.zeros(n, device="cuda"), relu=False)
+    outi = gemm_bf16(ai, wi, torch.zeros(n, device="cuda"), relu=False, pair=pair)
     refi = (ai.float() @ wi.float().t()).to(torch.bfloat16)
-    debug_set("gemm_pair", 1)
     assert torch.equal(outi, refi)
