@@ -25,9 +25,6 @@ if ROOT not in sys.path:
 
 FILTER_FLOP_PER_EDGE = 2 * (24 * 1024 + 1024 * 1024 * 2 + 1024)          # 4 245 504
 EMBED_FLOP_PER_HIT = 2 * (3 * 1024 + 1024 * 1024 * 2 + 1024 * 12)        # 4 225 024
-# DRAM bytes of one full-chunk launch (1 212 416 rows) of the dominant kernel, from the ncu --set full capture summarised in
-# profiles/r1_full_v6.md (dram__bytes_read.sum + dram__bytes_write.sum)
-NCU_TRAFFIC_BYTES = {"bias_act": 2578.13e6 + 2441.02e6, "relu_dot": 2490.36e6 + 23.02e6}
 
 
 def gnn_flops(n, e, H=128, T=8):
@@ -96,11 +93,13 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def build_workload(name):
+def build_workload(name, seed_offset=0):
     from synth.configs import get_config, load_calibration, make_events
     from synth.weights import make_model
     cfg = get_config(name)
     calib = load_calibration(cfg["calibration"])
+    if seed_offset:
+        cfg["seeds"] = [s + seed_offset for s in cfg["seeds"]]     # a different event of the same generator (replica r's own request)
     ev = make_events(cfg)
     model = make_model(cfg)
     # reading C-16: decoder bias centred so that the 0.5 cut has edges on both sides (a weight value, not an API change)
@@ -109,33 +108,7 @@ def build_workload(name):
     return cfg, calib, ev, model
 
 
-def oracle_sample(n_particles, arch_cfg_name="pileup200"):
-    """Times the oracle (as it stands) on a bounded sample: the pileup-50-density event of `n_particles` particles through
-    all five stages with the headline architecture; returns per-stage seconds and unit counts."""
-    from oracle import pipeline as opipe
-    from synth.configs import get_config, load_calibration, make_events
-    from synth.weights import make_model
-    cfg = get_config("pileup50")                       # same architecture as pileup200, its own calibrated radius/cut
-    calib = load_calibration("pileup50")
-    ev = make_events(cfg, n_particles=n_particles)
-    model = make_model(cfg)
-    timing = {}
-    t0 = time.perf_counter()
-    out = opipe.run(cfg, model, calib, ev["hits"], ev["event_offsets"], timing=timing)
-    wall = time.perf_counter() - t0
-    units = dict(n=len(ev["hits"]), e_c=len(out["cand_src"]), e_k=len(out["src"]))
-    return timing, units, wall
-
-
-def extrapolate_events_per_s(timing, units, target):
-    """Per-stage time scaled by the stage's unit count (S1,S2: hits; S3: candidate edges; S4,S5: kept edges)."""
-    t = (timing["s1_embed"] + timing["s2_frnn"]) * target["n"] / max(1, units["n"]) \
-        + timing["s3_filter"] * target["e_c"] / max(1, units["e_c"]) \
-        + (timing["s4_gnn"] + timing["s5_cc"]) * target["e_k"] / max(1, units["e_k"])
-    return 1.0 / t, t
-
-
-def cpu_threads():
+def blas_threads():
     try:
         from threadpoolctl import threadpool_info
         return max([i.get("num_threads", 1) for i in threadpool_info()] + [1])
@@ -143,30 +116,107 @@ def cpu_threads():
         return os.cpu_count() or 1
 
 
+# which of the oracle's stages run on how many threads: S1, S3, S4 are fp64 matmuls (NumPy's BLAS pool); S2 and S5 are
+# single-threaded Python loops over NumPy element-wise calls
+def stage_threads():
+    t = blas_threads()
+    return {"s1_embed": t, "s2_frnn": 1, "s3_filter": t, "s4_gnn": t, "s5_cc": 1}
+
+
+def oracle_full_event(name, n_particles=None):
+    """Times oracle.pipeline.run (as it stands) on the event of config `name` (or on a smaller event of the same generator and
+    architecture when n_particles is given); returns per-stage seconds, unit counts and the wall time."""
+    from oracle import pipeline as opipe
+    from synth.configs import make_events
+    cfg, calib, ev, model = build_workload(name)
+    if n_particles is not None:
+        ev = make_events(cfg, n_particles=n_particles)
+    timing = {}
+    t0 = time.perf_counter()
+    out = opipe.run(cfg, model, calib, ev["hits"], ev["event_offsets"], timing=timing)
+    wall = time.perf_counter() - t0
+    units = dict(n=len(ev["hits"]), e_c=len(out["cand_src"]), e_k=len(out["src"]), e_t=int(np.sum(out["gnn_score"] > cfg["gnn_cut"])))
+    return timing, units, wall
+
+
+def reference_units(cfg, calib, ev, model, k):
+    """The oracle's pass over ONE event cut into exactly k consecutive pieces of work (the reference arm's steps): S1, S2,
+    then S3 in k-4 equal slices of the candidate edges (the filter MLP is row-wise, so slices give the same values as one
+    call), S4, S5.  Every piece calls the oracle's own stage function; together they are one full event."""
+    from oracle import s1_embed, s2_frnn, s3_filter, s4_gnn, s5_cc
+    from oracle.mlp import sigmoid
+    st = {}
+    hits, off = ev["hits"], ev["event_offsets"]
+
+    def u_s1():
+        st["emb"] = s1_embed.embed_f32(hits, model["embed"])
+
+    def u_s2():
+        st["src"], st["dst"], _ = s2_frnn.frnn(st["emb"], hits, off, calib["frnn_radius"], cfg["frnn_k"])
+        st["fs"] = np.empty(len(st["src"]), np.float32)
+
+    def u_s3(i, parts):
+        e = len(st["src"])
+        lo, hi = e * i // parts, e * (i + 1) // parts
+        feat = st["emb"] if cfg["filter_input"] == "emb" else hits
+        st["fs"][lo:hi] = s3_filter.filter_scores(feat, st["src"][lo:hi], st["dst"][lo:hi], model["filter"]).astype(np.float32)
+        if i == parts - 1:
+            keep = s3_filter.keep_mask(st["fs"], calib["filter_cut"])
+            st["ks"], st["kd"] = st["src"][keep], st["dst"][keep]
+
+    def u_s4():
+        st["score"] = sigmoid(s4_gnn.gnn_forward(hits, st["ks"], st["kd"], model, cfg["gnn_iters"])).astype(np.float32)
+
+    def u_s5():
+        st["labels"] = s5_cc.connected_components(len(hits), st["ks"], st["kd"], st["score"], cfg["gnn_cut"])
+
+    parts = max(1, k - 4)
+    units = [("s1_embed", u_s1), ("s2_frnn", u_s2)] + [("s3_filter", (lambda i=i: u_s3(i, parts))) for i in range(parts)] + \
+            [("s4_gnn", u_s4), ("s5_cc", u_s5)]
+    # fewer than 5 steps asked for: consecutive pieces are merged so that the number of steps is exactly k
+    while len(units) > max(1, k):
+        (n0, f0), (n1, f1) = units[-2], units[-1]
+        units[-2:] = [(n0 + "+" + n1, (lambda f0=f0, f1=f1: (f0(), f1())))]
+    return units, st
+
+
 def run_reference(args):
+    """The reference arm: the oracle as it stands on the host cores, on the headline event itself.  K full passes of the
+    pileup-200 event would take K x ~100 s, so the K timed steps are the K consecutive pieces of ONE pass (reference_units):
+    value = 1 event / (sum of the K step times), ms_per_step = their mean.  Warm-up steps run the whole pipeline on a small
+    event of the same generator (BLAS pool start-up, imports)."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    from synth.configs import load_calibration
-    cal = load_calibration("pileup200")
-    target = dict(n=cal["n_hits"], e_c=cal["n_cand_edges"], e_k=cal["n_kept_edges"])
-    npart = args.ref_particles
     for _ in range(args.warmup):
-        oracle_sample(npart)
-    vals, walls = [], []
-    for _ in range(args.steps):
-        timing, units, wall = oracle_sample(npart)
-        v, _ = extrapolate_events_per_s(timing, units, target)
-        vals.append(v); walls.append(wall)
-    value = float(np.mean(vals))
-    sample = (f"oracle (fp64 NumPy) on a {npart}-particle event of the same generator and architecture "
-              f"({units['n']} hits, {units['e_c']} candidate, {units['e_k']} kept edges), per-stage times scaled by unit counts "
-              f"to the pileup-200 event ({target['n']} hits, {target['e_c']}, {target['e_k']})")
-    line = {"impl": "reference", "metric": "events/s (pileup-200 event)", "value": value, "unit": "events/s", "n_gpus": args.gpus,
-            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1000.0 * float(np.mean(walls)), "higher_is_better": True,
+        oracle_full_event("pileup50", n_particles=100)
+    cfg, calib, ev, model = build_workload(args.config)
+    units, st = reference_units(cfg, calib, ev, model, args.steps)
+    walls, stage_s = [], {}
+    for name, fn in units:
+        t0 = time.perf_counter()
+        fn()
+        dt = time.perf_counter() - t0
+        walls.append(dt)
+        for part in name.split("+"):
+            stage_s[part] = stage_s.get(part, 0.0) + dt / len(name.split("+"))
+    total = float(np.sum(walls))
+    n = len(ev["hits"])
+    n_events = len(ev["event_offsets"]) - 1
+    value = n_events / total
+    sample = (f"oracle (fp64 NumPy) on the {args.config} event itself ({n} hits, {len(st['src'])} candidate, {len(st['ks'])} kept edges): "
+              f"ONE full pass cut into {len(units)} consecutive steps (S1, S2, S3 in {max(1, args.steps - 4)} edge slices, S4, S5), "
+              f"{total:.1f} s in total")
+    line = {"impl": "reference", "metric": f"events/s ({args.config} event)", "value": value, "unit": "events/s", "n_gpus": args.gpus,
+            "steps": len(units), "warmup": args.warmup, "ms_per_step": 1000.0 * total / len(units), "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": "pileup200", "hits": target["n"], "parallelism": "host cores"},
-            "cpu_baseline": {"value": value, "unit": "events/s", "cores": cpu_threads(), "kind": "oracle", "sample": sample},
+            "config": {"workload": args.config, "hits": n, "events_per_step": n_events / len(units), "cand_edges": len(st["src"]),
+                       "kept_edges": len(st["ks"]), "parallelism": "host cores",
+                       "step": "one of the consecutive pieces of one full oracle pass over the event (see cpu_baseline.sample)"},
+            "hits_per_s": value * n / n_events,
+            "cpu_baseline": {"value": value, "unit": "events/s", "cores": blas_threads(), "kind": "oracle", "sample": sample,
+                             "stage_s": {k: round(v, 3) for k, v in stage_s.items()}, "stage_threads": stage_threads(),
+                             "event_s": total},
             "e2e": {"value": value, "unit": "events/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line))
@@ -245,6 +295,76 @@ def run_concurrency_scan(args):
     print(json.dumps(res))
 
 
+def make_trk(cfg, calib, ev, model, device):
+    from paper_2501_05520_b200 import trk_from_config
+    n = len(ev["hits"])
+    n_events = len(ev["event_offsets"]) - 1
+    # capacities: N*K can never overflow S2 (SURVEY 8b); kept edges sized from the calibrated count with head-room
+    max_cand = n * cfg["frnn_k"]
+    per_event = calib["n_kept_edges"] * max(1.0, (n / n_events) / calib["n_hits"])
+    max_kept = int(min(max_cand, per_event * n_events * 1.5 + 4096))
+    return trk_from_config(cfg, model, calib, max_hits=n, max_events=n_events, max_cand_edges=max_cand, max_kept_edges=max_kept,
+                           device=device)
+
+
+def timed_steps(trk, hits, off, out, flush, steps, profiled=False):
+    """`steps` trk_infer calls, each between its own CUDA-event pair on the launch stream, the L2 flushed (256 MB written) before
+    each pair.  profiled: also reads the library's per-stage / per-launch event times after every step (a second pass: the
+    headline value is timed with profiling off)."""
+    import torch
+    starts = [torch.cuda.Event(enable_timing=True) for _ in range(steps)]
+    ends = [torch.cuda.Event(enable_timing=True) for _ in range(steps)]
+    stage_ms, kernel_ms = [], []
+    for i in range(steps):
+        flush.zero_()
+        starts[i].record()
+        trk.infer(hits, off, out=out)
+        ends[i].record()
+        if profiled:
+            stage_ms.append(trk.stage_ms())
+            kernel_ms.append(trk.kernel_ms())
+    torch.cuda.synchronize()
+    return [s.elapsed_time(e) for s, e in zip(starts, ends)], stage_ms, kernel_ms
+
+
+def bench_other_config(name, dev, flush, steps=5, warmup=3):
+    """One of the non-headline configs through the same call (GPU arm only): events/s, hits/s, stage times."""
+    import torch
+    cfg, calib, ev, model = build_workload(name)
+    trk = make_trk(cfg, calib, ev, model, dev.index)
+    hits = torch.from_numpy(ev["hits"]).to(dev)
+    off = ev["event_offsets"]
+    n, n_events = len(ev["hits"]), len(off) - 1
+    out = trk.infer(hits, off)
+    for _ in range(warmup):
+        trk.infer(hits, off, out=out)
+    torch.cuda.synchronize()
+    ms, _, _ = timed_steps(trk, hits, off, out, flush, steps)
+    trk.profile(True)
+    _, st, _ = timed_steps(trk, hits, off, out, flush, 3, profiled=True)
+    counts = out["counts"].cpu().numpy().tolist()
+    res = {"precision": cfg["precision"], "hits": n, "events_per_call": n_events, "cand_edges": counts[0], "kept_edges": counts[1],
+           "gnn_pass_edges": counts[2], "overflow": counts[3], "steps": steps, "ms_per_call": float(np.mean(ms)),
+           "events_per_s": n_events * steps / (float(np.sum(ms)) * 1e-3), "hits_per_s": n * steps / (float(np.sum(ms)) * 1e-3),
+           "stage_ms": {k: round(float(np.mean([x[k] for x in st])), 4) for k in st[0]}, "workspace_gb": round(trk.workspace_bytes / 2 ** 30, 3),
+           "gpu_launches_per_call": trk.last_launch_count}
+    trk.close()
+    del hits, out
+    torch.cuda.empty_cache()
+    return res
+
+
+def dominant_kernel_traffic():
+    """dram__bytes_read.sum + dram__bytes_write.sum of one full-chunk launch of the dominant kernel, from the tracked ncu summary
+    (profiles/dominant_kernel_traffic.json names the capture and the commit it was taken at); None if the file is missing."""
+    p = os.path.join(ROOT, "profiles", "dominant_kernel_traffic.json")
+    try:
+        with open(p) as f:
+            return json.load(f)
+    except Exception:
+        return None
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -252,10 +372,11 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="pileup200")
-    ap.add_argument("--ref-particles", type=int, default=500)
-    ap.add_argument("--cpu-baseline-particles", type=int, default=2500)
+    ap.add_argument("--cpu-baseline-particles", type=int, default=0,
+                    help="opt-out: time the oracle on a smaller event of this many particles instead of the headline event itself")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-all-configs", action="store_true", help="skip the short runs of the other configs (all_configs)")
     ap.add_argument("--scan", action="store_true", help="concurrency scan (model instances x streams, packed batch, CUDA graph)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
@@ -266,8 +387,8 @@ def main():
 
     import torch
     import torch.distributed as dist
-    from paper_2501_05520_b200 import gemm_bf16, trk_from_config
-    from paper_2501_05520_b200.replicas import max_over_ranks
+    from paper_2501_05520_b200 import gemm_bf16
+    from paper_2501_05520_b200.replicas import max_over_ranks, sum_over_ranks
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -278,16 +399,15 @@ def main():
     dev = torch.device("cuda", local)
     warmup = max(args.warmup, 3)
 
-    cfg, calib, ev, model = build_workload(args.config)
+    # replicas only: every rank serves its OWN event of the headline config (seed = rank), no collective
+    # on the data path; rank 0's event is the literal headline event
+    cfg, calib, ev, model = build_workload(args.config, seed_offset=rank)
     n = len(ev["hits"])
     n_events = len(ev["event_offsets"]) - 1
-    # capacities: N*K can never overflow S2 (SURVEY 8b); kept edges sized from the calibrated count with head-room
-    max_cand = n * cfg["frnn_k"]
-    max_kept = int(min(max_cand, calib["n_kept_edges"] * (n / calib["n_hits"]) * 1.5 + 4096))
-    trk = trk_from_config(cfg, model, calib, max_hits=n, max_events=n_events, max_cand_edges=max_cand, max_kept_edges=max_kept,
-                          device=local)
+    trk = make_trk(cfg, calib, ev, model, local)
     hits = torch.from_numpy(ev["hits"]).to(dev)
-    out = trk.infer(hits, ev["event_offsets"])          # allocates outputs once
+    off = ev["event_offsets"]
+    out = trk.infer(hits, off)          # allocates outputs once
     torch.cuda.synchronize()
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # > 126 MB L2
 
@@ -296,30 +416,27 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    trk.profile(True)
     for _ in range(warmup):
         flush.zero_()
-        trk.infer(hits, ev["event_offsets"], out=out)
+        trk.infer(hits, off, out=out)
     barrier()
+    # ---- the headline: K steps, profiling OFF
     sampler = ClockSampler(local) if rank == 0 else None
-    starts = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
-    ends = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
-    stage_ms, kernel_ms = [], []
-    for i in range(args.steps):
-        flush.zero_()
-        starts[i].record()
-        trk.infer(hits, ev["event_offsets"], out=out)
-        ends[i].record()
-        stage_ms.append(trk.stage_ms())                 # waits for this step (the next flush is outside the timed pair anyway)
-        kernel_ms.append(trk.kernel_ms())
+    step_ms, _, _ = timed_steps(trk, hits, off, out, flush, args.steps)
     barrier()
     clocks = sampler.stop() if sampler else None
-    step_ms = [s.elapsed_time(e) for s, e in zip(starts, ends)]
-    total_ms = float(np.sum(step_ms))
     launches = trk.last_launch_count * args.steps
     counts = out["counts"].cpu().numpy().tolist()
-    total_ms = max_over_ranks(total_ms, dev)            # replicas: the slowest rank's device time (no data-path collective)
+    total_ms = max_over_ranks(float(np.sum(step_ms)), dev)            # replicas: the slowest rank's device time
+    hits_all = sum_over_ranks(float(n), dev)
     events_per_s = world * n_events * args.steps / (total_ms / 1000.0)
+    hits_per_s = hits_all * args.steps / (total_ms / 1000.0)
+
+    # ---- second pass, profiling ON: per-stage times and the per-launch times of the dominant kernel
+    trk.profile(True)
+    prof_steps = min(max(args.steps, 3), 10)
+    prof_ms, stage_ms, kernel_ms = timed_steps(trk, hits, off, out, flush, prof_steps, profiled=True)
+    trk.profile(False)
 
     # ---- end to end through the host API: pinned host buffers, H2D + D2H inside the timed region
     e2e = None
@@ -328,11 +445,11 @@ def main():
         lh = torch.empty(n, dtype=torch.int32).pin_memory()
         ch = torch.zeros(4, dtype=torch.int32).pin_memory()
         for _ in range(2):
-            trk.infer_host(hh, ev["event_offsets"], lh, ch)
+            trk.infer_host(hh, off, lh, ch)
         barrier()
         t0 = time.perf_counter()
         for _ in range(args.steps):
-            trk.infer_host(hh, ev["event_offsets"], lh, ch)
+            trk.infer_host(hh, off, lh, ch)
         torch.cuda.synchronize()
         dt = time.perf_counter() - t0
         dt = max_over_ranks(dt, dev)
@@ -340,6 +457,7 @@ def main():
                "d2h_bytes_per_step": n * 4 + 16, "api": "trk_infer_host (pinned host hits in, host labels out, sync inside)"}
 
     if rank != 0:
+        trk.close()
         if world > 1:
             dist.destroy_process_group()
         return
@@ -350,7 +468,7 @@ def main():
     st = {k: float(np.mean([s[k] for s in stage_ms])) for k in stage_ms[0]}
     s3_flops = e_c * FILTER_FLOP_PER_EDGE
     s3_tflops = s3_flops / (st["s3_filter"] * 1e-3) / 1e12
-    # the dominant kernel inside the timed steps: CUDA-event pairs around every hidden-layer GEMM launch of S3
+    # the dominant kernel inside the profiled steps: CUDA-event pairs around every hidden-layer GEMM launch of S3
     # (trk_profile_kernel_ms); chunk c of launch i = c // 2 holds rows [c*chunk, (c+1)*chunk) clipped to E_c
     width = cfg["filter_dims"][1]
     k_flops, k_ms, k_n = 0.0, 0.0, 0
@@ -380,6 +498,7 @@ def main():
     torch.cuda.synchronize()
     iso_ms = float(np.mean([s.elapsed_time(e) for s, e in evs]))
     iso_tflops = 2.0 * m_chunk * 1024 * 1024 / (iso_ms * 1e-3) / 1e12
+    del a, w, b
     hbm = peaks["hbm_gbs"]
     stage_roofline = {
         "s1_embed": {"bound": "tensor", "achieved_tflops": n * EMBED_FLOP_PER_HIT / (st["s1_embed"] * 1e-3) / 1e12},
@@ -391,8 +510,8 @@ def main():
     s4 = stage_roofline["s4_gnn"]
     s4["hbm_view"] = {"achieved_gbs": gnn_bytes(n, e_k, cfg["gnn_hidden"], cfg["gnn_iters"]) / (st["s4_gnn"] * 1e-3) / 1e9}
     s4["hbm_view"]["frac_of_measured"] = s4["hbm_view"]["achieved_gbs"] / hbm
-    stage_roofline["s2_frnn"]["note"] = ("nominally HBM; really instruction-issue bound (tables live in L2/L1, no DRAM traffic): "
-                                         "ncu issue 63 %, profiles/r1_full_v4.md")
+    stage_roofline["s2_frnn"]["note"] = ("nominally HBM; really instruction-issue bound (tables live in L2/L1, no DRAM traffic), "
+                                         "see profiles/")
     stage_roofline["s5_cc"]["note"] = "nominally HBM; really bound by the latency of atomics on the L2-resident parent array"
     s4["note"] = "on the tensor/HBM ridge: the flop count is the split-first-layer minimum, the byte count the bf16-state minimum"
     for k, v in stage_roofline.items():
@@ -403,9 +522,9 @@ def main():
         else:
             v["frac_of_measured"] = v["achieved_gbs"] / hbm
             v["frac_of_nominal_8000"] = v["achieved_gbs"] / 8000.0
-    # peak: the launches are 0.4 ms kernels inside 14 ms steps of a ~0.2 s timed region, far from the 4 s back-to-back run that
-    # defines the "sustained" cuBLAS figure (SM clocks settle near 1.33 GHz there; here they stay near the burst clocks, see
-    # `clocks`), so the burst figure is the denominator; the fraction of the sustained figure is given beside it.
+    # peak: the launches are ~1.2 ms kernels inside ~12 ms steps of a ~0.2 s timed region, far from the 4 s back-to-back run
+    # that defines the "sustained" cuBLAS figure, so the burst figure is the denominator; the sustained one is given beside it.
+    traffic = dominant_kernel_traffic()
     roofline = {"bound": "tensor",
                 "kernel": "tc::gemm_tc2_kernel<256,*> (tcgen05.mma.cta_group::2, the 1024x1024 hidden layers of the S3 filter MLP; "
                           f"one launch = one layer of one {chunk_rows}-edge chunk)",
@@ -414,41 +533,60 @@ def main():
                 "frac_of_sustained_peak": kern_tflops / peaks["bf16_sustained"], "sustained_peak": peaks["bf16_sustained"],
                 "launches_timed": k_n, "avg_launch_ms": k_ms / max(1, k_n), "flop_per_full_launch": 2.0 * chunk_rows * width * width,
                 "how": "algorithmic flops of the non-empty launches (2 x rows x 1024 x 1024 each) / their summed durations, CUDA-event pairs "
-                       "around each launch on the launch stream inside the timed steps (trk_profile_kernel_ms)",
-                # ncu --set full, profiles/r1_full_v6.md: dram__bytes_read.sum + dram__bytes_write.sum of one full-chunk launch
-                "traffic": NCU_TRAFFIC_BYTES["bias_act"], "traffic_unit": "bytes per full-chunk launch (EpiBiasActBf16 variant)",
-                "traffic_detail": dict(NCU_TRAFFIC_BYTES, algorithmic_bias_act=2 * chunk_rows * width * 2 + width * width * 2,
-                                       algorithmic_relu_dot=chunk_rows * width * 2 + width * width * 2 + chunk_rows * 16,
-                                       source="profiles/r1_full_v6.md"),
+                       f"around each launch on the launch stream (trk_profile_kernel_ms) in {prof_steps} profiled steps run right after the "
+                       "timed steps",
+                "traffic": traffic["bytes_per_full_launch"]["bias_act"] if traffic else None,
+                "traffic_unit": "bytes per full-chunk launch (EpiBiasActBf16 variant), ncu dram__bytes_read.sum + dram__bytes_write.sum",
+                "traffic_detail": dict(traffic or {}, algorithmic_bias_act=2 * chunk_rows * width * 2 + width * width * 2,
+                                       algorithmic_relu_dot=chunk_rows * width * 2 + width * width * 2 + chunk_rows * 16),
                 "whole_stage": {"achieved": s3_tflops, "frac": s3_tflops / peaks["bf16_sustained"],
                                 "how": "algorithmic flops of S3 (E_c x 4 245 504) / S3 stage time (gather, 3 GEMMs, finish, compaction)"},
                 "isolated_launch": {"shape": [m_chunk, 1024, 1024], "ms": iso_ms, "achieved": iso_tflops,
                                     "frac_of_burst_peak": iso_tflops / peaks["bf16_tflops"]}}
 
+    # ---- the other configs (BASELINE.json configs[0,1,3,4], the size-matched pileup-200 and the paper-scale event): a few steps each
+    all_configs = None
+    if world == 1 and not args.no_all_configs:
+        trk.close()
+        trk = None
+        del hits, out
+        torch.cuda.empty_cache()
+        all_configs = {}
+        for name in ("toy", "pileup50", "pileup200_nominal", "batch16", "pileup300", "paper350k"):
+            if name != args.config:
+                all_configs[name] = bench_other_config(name, dev, flush)
+
     cpu_baseline = None
     if world == 1 and not args.no_cpu_baseline:
-        timing, units, wall = oracle_sample(args.cpu_baseline_particles)
-        from synth.configs import load_calibration
-        cal = load_calibration("pileup200")
-        target = dict(n=cal["n_hits"], e_c=cal["n_cand_edges"], e_k=cal["n_kept_edges"])
-        v, t_est = extrapolate_events_per_s(timing, units, target)
-        cpu_baseline = {"value": v, "unit": "events/s", "cores": cpu_threads(), "kind": "oracle",
-                        "sample": (f"oracle (fp64 NumPy) on the {args.cpu_baseline_particles}-particle pileup-50 event (same architecture; "
-                                   f"{units['n']} hits, {units['e_c']} candidate, {units['e_k']} kept edges; {wall:.1f} s wall), per-stage "
-                                   f"times scaled by unit counts to the pileup-200 event => {t_est:.0f} s/event"),
-                        "stage_s": {k: round(v_, 3) for k, v_ in timing.items()}}
+        npart = args.cpu_baseline_particles if args.cpu_baseline_particles > 0 else None
+        timing, units, wall = oracle_full_event(args.config, n_particles=npart)
+        what = (f"the {args.config} event itself" if npart is None else
+                f"a {npart}-particle event of the same generator and architecture (opt-out sample, NOT the headline event)")
+        cpu_baseline = {"value": (len(off) - 1) / wall if npart is None else None, "unit": "events/s", "cores": blas_threads(), "kind": "oracle",
+                        "sample": (f"oracle.pipeline.run (fp64 NumPy, as it stands) on {what}: {units['n']} hits, {units['e_c']} candidate, "
+                                   f"{units['e_k']} kept edges, {units['e_t']} edges above the GNN cut; {wall:.1f} s wall, measured once"),
+                        "event_s": wall, "hits_per_s": units["n"] / wall,
+                        "stage_s": {k: round(v_, 3) for k, v_ in timing.items()}, "stage_threads": stage_threads()}
+        if npart is not None:
+            cpu_baseline["value"] = 1.0 / wall
+            cpu_baseline["unit"] = "sample events/s"
 
-    line = {"metric": "events/s (pileup-200 event)", "value": events_per_s, "unit": "events/s", "n_gpus": world, "steps": args.steps,
+    line = {"metric": f"events/s ({args.config} event)", "value": events_per_s, "unit": "events/s", "n_gpus": world, "steps": args.steps,
             "warmup": warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "bf16", "data": "synthetic",
             "config": {"workload": args.config, "hits": n, "events_per_step": n_events, "cand_edges": e_c, "kept_edges": e_k,
-                       "gnn_pass_edges": counts[2], "overflow": counts[3], "parallelism": f"replicas x{world}",
+                       "gnn_pass_edges": counts[2], "overflow": counts[3],
+                       "parallelism": f"replicas x{world}" + (" (rank r serves its own event, seed r; no collective on the data path)" if world > 1 else ""),
                        "l2": "256 MB buffer written between timed steps (L2 flush)", "precision": "bf16 operands, fp32 accumulate",
-                       "workspace_gb": trk.workspace_bytes / 2 ** 30},
-            "hits_per_s": events_per_s * n / n_events, "stage_ms": st, "stage_roofline": stage_roofline,
-            "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu_baseline}
+                       "workspace_gb": (trk.workspace_bytes if trk else 0) / 2 ** 30 or None,
+                       "timing": "value: CUDA-event pair per step, profiling off; stage_ms / roofline: a second, profiled pass"},
+            "hits_per_s": hits_per_s, "stage_ms": st, "profiled_pass_ms_per_step": float(np.mean(prof_ms)),
+            "stage_roofline": stage_roofline,
+            "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu_baseline,
+            "all_configs": all_configs}
     print(json.dumps(line))
-    trk.close()
+    if trk:
+        trk.close()
     if world > 1:
         dist.destroy_process_group()
 

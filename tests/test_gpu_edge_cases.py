@@ -314,3 +314,32 @@ def test_infer_host_equals_infer():
         assert np.array_equal(lab, ref["labels"].cpu().numpy()) and np.array_equal(cnt, ref["counts"].cpu().numpy())
     finally:
         trk.close()
+
+
+def test_dispatcher_two_replicas_serve_four_different_events():
+    """SURVEY.md section 8(f) NEXT-4 on one GPU: two model instances on device 0 behind the Dispatcher serve four DIFFERENT
+    events concurrently (one host thread per replica) and return, in request order, exactly what one context returns."""
+    from paper_2501_05520_b200.replicas import Dispatcher
+    cfg = G.get_config("pileup50")
+    calib = G.load_calibration("pileup50")
+    model = G.centred_model(cfg, calib)
+    events = []
+    for seed in (3, 4, 5, 6):
+        ev = G.make_events(dict(cfg, seeds=[seed]), n_particles=300 + 50 * seed)
+        events.append((ev["hits"], ev["event_offsets"]))
+    max_hits = max(len(h) for h, _ in events)
+    disp = Dispatcher.from_devices(cfg, model, calib, max_hits=max_hits, devices=[0], instances_per_device=2)
+    from paper_2501_05520_b200 import trk_from_config
+    single = trk_from_config(cfg, model, calib, max_hits=max_hits)
+    try:
+        assert disp.assignment(4) == [[0, 2], [1, 3]]
+        res = disp.serve(events)
+        assert len(res) == 4
+        for (hits, off), (labels, counts) in zip(events, res):
+            want_labels, want_counts = single.infer_host(hits, off)
+            assert np.array_equal(labels, want_labels) and np.array_equal(counts, want_counts)
+            assert counts[3] == 0 and counts[0] > counts[1] > 0 and len(np.unique(labels)) < len(hits)
+        assert len({len(r[0]) for r in res}) == 4                     # four different events indeed
+    finally:
+        disp.close()
+        single.close()
