@@ -102,8 +102,8 @@ typedef struct {
    *                      activation buffers hold rows x widest layer bf16 each.  Default 128 x SMs x 64 rows
    *                      (1 212 416 on a B200: 2.5 GB per buffer, 5 launches per pass); smaller values trade a few
    *                      per cent of throughput for memory (64 x 148 rows: 20 MB per buffer) -- DESIGN.md section 6.
-   *   grid_max           upper bound of the S2 search grid's cells per axis and event (1..128).  Default: the largest of
-   *                      128, 64, 32, 16, 8 whose cell table (max_events x grid_max^3 cells) fits 2^21 cells.          */
+   *   grid_max           upper bound of the S2 search grid's cells per axis and event (1..128).  Default (and upper limit):
+   *                      the largest value whose cell table (max_events x grid_max^3 x 16 radius buckets) fits 2^22 entries.  */
   int64_t filter_chunk_rows;
   int32_t grid_max;
 } trk_config;

@@ -124,11 +124,14 @@ void carve(trk_ctx* c, Carver& k) {
   const size_t N = (size_t)f.max_hits, EC = (size_t)f.max_cand_edges, EK = (size_t)f.max_kept_edges;
   const size_t es = bf ? 2 : 4;
   const int H = c->H;
+  const size_t f_w1 = c->filter.layers.empty() ? 0 : (size_t)c->filter.layers[0].out_pad;
   int maxw = 64;
   for (auto& L : c->embed.layers) maxw = std::max(maxw, L.out_pad);
   for (auto& L : c->filter.layers) maxw = std::max(maxw, L.out_pad);
   {
-    int64_t chunk = (int64_t)128 * c->sm_count * kFilterChunkTilesPerSm;
+    // layer-by-layer S3: rows per pass.  With the fused S3 kernel (the default when the shape allows it) the chunked path only
+    // serves as a test variant, so its buffers stay small unless the caller sizes them.
+    int64_t chunk = (int64_t)128 * c->sm_count * (c->filter_fusable ? 1 : kFilterChunkTilesPerSm);
     if (f.filter_chunk_rows > 0) chunk = (f.filter_chunk_rows + 127) / 128 * 128;
     c->filter_chunk = std::min<int64_t>(chunk, ((int64_t)EC + 127) / 128 * 128);
   }
@@ -140,8 +143,13 @@ void carve(trk_ctx* c, Carver& k) {
   k.take(&p, (size_t)c->act_rows * maxw * es); c->act1 = p;
   k.take(&p, (size_t)c->filter_chunk * (bf ? 64 * 2 : 2 * c->filter_u * 4)); c->act_in = p;
   k.take(&c->partial, (size_t)c->filter_chunk * 16);
+  if (c->filter_fusable) {
+    const size_t rows = (size_t)(c->sm_count / 2) * 256;
+    k.take(&c->filter_s1, rows * f_w1);
+    k.take(&c->filter_s2, rows * f_w1);
+  }
   k.take(&c->proj, N * 3);
-  k.take(&c->bbox, 8);
+  k.take(&c->bbox, 16);
   k.take(&c->grid, 1);
   k.take(&c->cell_of_hit, N);
   k.take(&c->cell_count, (size_t)c->max_cells + 1);
@@ -277,6 +285,9 @@ trk_status trk_destroy(trk_ctx* ctx) {
   cudaFree(ctx->edge_dec_wab);
   cudaFree(ctx->edge_dec_wc);
   cudaFree(ctx->filter_w1_pad);
+  cudaFree(ctx->filter_w1_frag);
+  cudaFree(ctx->node_enc_w1p);
+  cudaFree(ctx->edge_enc_w1p);
   cudaFree(ctx->ws.base);
   delete ctx;
   return TRK_OK;
@@ -355,11 +366,11 @@ trk_status trk_create(const trk_config* cfg, trk_ctx** out) {
   ctx->grid_dims = cfg->grid_dims;
   // cells per axis and event: the finest grid whose cell table fits (the cell edge never goes below r, so a finer bound only
   // helps: candidates per query fall with the cell volume until the edge reaches r)
-  ctx->grid_max = 8;
-  for (int g : {128, 64, 32, 16})
-    if (cfg->max_events * (int64_t)g * g * g <= kMaxCells) { ctx->grid_max = g; break; }
-  if (cfg->grid_max > 0) ctx->grid_max = cfg->grid_max;
-  ctx->max_cells = (int64_t)cfg->max_events * ctx->grid_max * ctx->grid_max * ctx->grid_max;
+  ctx->grid_max = 1;
+  for (int g = 128; g > 1; --g)
+    if (cfg->max_events * (int64_t)g * g * g * kRBuckets <= kMaxCells) { ctx->grid_max = g; break; }
+  if (cfg->grid_max > 0) ctx->grid_max = std::min(ctx->grid_max, cfg->grid_max);
+  ctx->max_cells = (int64_t)cfg->max_events * ctx->grid_max * ctx->grid_max * ctx->grid_max * kRBuckets;
 
   trk_status s = TRK_OK;
   auto bail = [&](trk_status st) {
@@ -423,6 +434,39 @@ trk_status trk_create(const trk_config* cfg, trk_ctx** out) {
     for (int o = 0; o < w1; ++o)
       for (int i = 0; i < k1; ++i) p[(size_t)o * 64 + i] = f32_to_bf16_rne(cfg->filter.weight[0][(size_t)o * k1 + i]);
     if ((s = upload_bf16_block(ctx, p, &ctx->filter_w1_pad)) != TRK_OK) return bail(s);
+    // fused S3 kernel: applicable shape, and W1 in mma.sync.m16n8k16 B-fragment order (filter_fused.cuh)
+    {
+      const trk_mlp& m = cfg->filter;
+      const int W = m.dims[1];
+      ctx->filter_fusable = m.n_layers == 4 && k1 <= 32 && W % 256 == 0 && W <= 1024 && m.dims[2] == W && m.dims[3] == W;
+      if (ctx->filter_fusable) {
+        std::vector<uint32_t> f((size_t)(W / 8) * 32 * 4, 0);
+        auto wq = [&](int n, int k) -> uint32_t { return k < k1 ? f32_to_bf16_rne(m.weight[0][(size_t)n * k1 + k]) : 0u; };
+        for (int nt = 0; nt < W / 8; ++nt)
+          for (int lane = 0; lane < 32; ++lane) {
+            const int g = lane >> 2, t4 = lane & 3, n = nt * 8 + g;
+            for (int ks = 0; ks < 2; ++ks)
+              for (int hc = 0; hc < 2; ++hc) {
+                const int k = ks * 16 + hc * 8 + 2 * t4;
+                f[((size_t)nt * 32 + lane) * 4 + ks * 2 + hc] = wq(n, k) | (wq(n, k + 1) << 16);
+              }
+          }
+        if (cudaMalloc(&ctx->filter_w1_frag, f.size() * 4) != cudaSuccess ||
+            cudaMemcpy(ctx->filter_w1_frag, f.data(), f.size() * 4, cudaMemcpyHostToDevice) != cudaSuccess)
+          return bail(fail(ctx, TRK_ERR_OOM, "filter_w1_frag upload failed"));
+      }
+    }
+    // encoder first layers (K = 3 / 4) as a [H][64] bf16 K block: every weight column twice, once for the hi and once for the
+    // lo half of its fp32 input feature (gnn_fused.cuh kEncode)
+    auto dup = [&](const trk_mlp& m, __nv_bfloat16** out) -> trk_status {
+      const int k = m.dims[0];
+      std::vector<uint16_t> w((size_t)H * 64, 0);
+      for (int o = 0; o < H; ++o)
+        for (int i = 0; i < k; ++i) w[(size_t)o * 64 + 2 * i] = w[(size_t)o * 64 + 2 * i + 1] = f32_to_bf16_rne(m.weight[0][(size_t)o * k + i]);
+      return upload_bf16_block(ctx, w, out);
+    };
+    if ((s = dup(cfg->node_enc, &ctx->node_enc_w1p)) != TRK_OK) return bail(s);
+    if ((s = dup(cfg->edge_enc, &ctx->edge_enc_w1p)) != TRK_OK) return bail(s);
   }
 
   Carver size_pass;
@@ -592,7 +636,8 @@ trk_status trk_profile_kernel_ms(trk_ctx* ctx, float* ms, int32_t capacity, int3
   if (!ctx->prof_valid) return fail(ctx, TRK_ERR_INVALID_ARG, "no profiled trk_infer call to read");
   TRK_CUDA(ctx, cudaEventSynchronize(ctx->prof_ev[5]));
   *n_launches = ctx->kprof_n;
-  if (rows_per_launch) *rows_per_launch = ctx->filter_chunk;
+  // fused S3 (one launch runs every layer over all candidate edges): -1; layer by layer: the rows of one pass
+  if (rows_per_launch) *rows_per_launch = ctx->filter_fusable && ctx->knobs[kKnobFilterFused] != 0 ? -1 : ctx->filter_chunk;
   for (int i = 0; i < ctx->kprof_n && i < capacity; ++i)
     TRK_CUDA(ctx, cudaEventElapsedTime(&ms[i], ctx->kprof_ev[(size_t)i * 2], ctx->kprof_ev[(size_t)i * 2 + 1]));
   return TRK_OK;
@@ -690,7 +735,8 @@ trk_status trk_set_option(trk_ctx* ctx, const char* key, int64_t value) {
   if (!ctx) return TRK_ERR_INVALID_ARG;
   if (!key) return fail(ctx, TRK_ERR_INVALID_ARG, "trk_set_option: key is NULL");
   static const struct { const char* name; int knob; } keys[] = {
-      {"gemm_pair", kKnobGemmPair}, {"gnn_fused", kKnobGnnFused}, {"epi_split", kKnobEpiSplit}, {"gemm_row_major", kKnobRowMajor}};
+      {"gemm_pair", kKnobGemmPair}, {"gnn_fused", kKnobGnnFused}, {"epi_split", kKnobEpiSplit}, {"gemm_row_major", kKnobRowMajor},
+      {"filter_fused", kKnobFilterFused}};
   for (const auto& k : keys)
     if (std::strcmp(key, k.name) == 0) {
       ctx->knobs[k.knob] = value;

@@ -14,12 +14,13 @@ namespace trk {
 
 constexpr int kMaxEmbDim = 16;      // d_e is padded to a multiple of 4, at most 16
 constexpr int kMaxEvents = 1024;    // event offsets travel as a kernel parameter
-constexpr int64_t kMaxCells = 1 << 21;  // FRNN grid cells summed over the events of a call
+constexpr int kRBuckets = 16;            // FRNN: radius buckets inside a spatial cell (a tracking detector has ~10 layers)
+constexpr int64_t kMaxCells = 1 << 22;  // FRNN cell-table entries (spatial cells x radius buckets) summed over the events of a call
 constexpr int kFilterChunkTilesPerSm = 64;  // default S3 rows per pass = 128 x sm_count x 64 (trk_config.filter_chunk_rows overrides):
                                             // 2.5 GB per activation buffer buys 5 launches per 1.2 M candidate edges
 
 // ---- test / tuning options (trk_set_option), per context ----
-enum { kKnobGemmPair = 0, kKnobGnnFused = 1, kKnobEpiSplit = 2, kKnobRowMajor = 3, kKnobCount = 4 };
+enum { kKnobGemmPair = 0, kKnobGnnFused = 1, kKnobEpiSplit = 2, kKnobRowMajor = 3, kKnobFilterFused = 4, kKnobCount = 5 };
 
 // One Linear layer resident on the device.
 struct DevLinear {
@@ -39,7 +40,9 @@ struct GridParams {
   float origin[3];
   float inv_cell[3];
   int dims[3];
-  int cells_per_event;
+  int cells_per_event;        // spatial cells of one event (the cell table has kRBuckets entries per spatial cell)
+  float proj_eps;             // rounding slack of the fp32 projection, scaled with max|e| (frnn_grid_setup_kernel)
+  float r_origin, r_inv;      // radius bucket = clamp(floor((r - r_origin) * r_inv), 0, kRBuckets - 1)
 };
 
 struct EventOffsets {
@@ -63,7 +66,7 @@ struct trk_ctx {
   cudaStream_t own_stream = nullptr;
   std::string last_error;
   int64_t launch_count = 0;
-  int64_t knobs[trk::kKnobCount] = {1, 1, 1, 16};   // gemm_pair, gnn_fused, epi_split, gemm_row_major (include/trk.h trk_set_option)
+  int64_t knobs[trk::kKnobCount] = {1, 1, 1, 16, 1};   // gemm_pair, gnn_fused, epi_split, gemm_row_major, filter_fused (trk_set_option)
   std::vector<const void*> smem_attr_set;          // kernels whose dynamic shared-memory limit has been raised on ctx->device
   bool profiling = false;
   cudaEvent_t prof_ev[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
@@ -83,6 +86,14 @@ struct trk_ctx {
   __nv_bfloat16* edge_dec_wab = nullptr;
   __nv_bfloat16* edge_dec_wc = nullptr;
   __nv_bfloat16* filter_w1_pad = nullptr;  // [1024][64] = W1 zero padded in K
+  // fused S3 kernel (filter_fused.cuh): layer-1 weights in mma.sync fragment order and the per-pair activation scratch
+  bool filter_fusable = false;             // filter = 2u -> W -> W -> W -> 1, 2u <= 32, W a multiple of 256, W <= 1024
+  uint4* filter_w1_frag = nullptr;         // [W/8][32] x {b0, b1 (k 0..15), b0, b1 (k 16..31)}
+  __nv_bfloat16* filter_s1 = nullptr;      // [sm_count/2 * 256][W]  act1
+  __nv_bfloat16* filter_s2 = nullptr;      // [sm_count/2 * 256][W]  act2
+  // first layers of the S4 encoders for the tensor core (gnn_fused.cuh kEncode): [H][64], columns (2k, 2k+1) = w[:, k] twice
+  __nv_bfloat16* node_enc_w1p = nullptr;
+  __nv_bfloat16* edge_enc_w1p = nullptr;
   float filter_b_last = 0.f;               // bias of the filter's final Linear(W -> 1)
   float edge_dec_b_last = 0.f;             // bias of the decoder's final Linear(H -> 1)
 
@@ -99,7 +110,7 @@ struct trk_ctx {
   int64_t filter_chunk = 0;         // S3 rows per pass: min(kFilterChunkRows, max_cand_edges rounded up to 128)
   // S2
   float* proj = nullptr;            // [max_hits][3]
-  int32_t* bbox = nullptr;          // [6] ordered-int min/max
+  int32_t* bbox = nullptr;          // [16]: ordered-int min/max of the three binning coordinates [0..6), of the radius feature [6..8), bits of max|e| [8]
   trk::GridParams* grid = nullptr;
   int32_t* cell_of_hit = nullptr;   // [max_hits]
   int32_t* cell_count = nullptr;    // [max_cells+1]

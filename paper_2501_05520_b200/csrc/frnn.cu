@@ -7,11 +7,15 @@
 //
 // Search structure (an implementation detail that cannot change the result): hits are binned on
 // g <= 3 coordinates of P^T e (P has orthonormal columns, so projected distance <= true distance)
-// into a per-event grid with cell edge >= r; a query looks at the 3^g neighbouring cells.  Hits
-// are counting-sorted by cell so a row of 3 x-adjacent cells is one contiguous candidate range.
-// One warp serves one query: lanes stride over the candidates, accepted ones are appended to a
-// shared-memory buffer via ballot, and a warp bitonic sort on (d2, j) prunes to the K nearest
-// whenever the buffer fills; a final sort on j gives the (src, dst) output order.
+// into a per-event grid with cell edge >= r; a query looks at the 3^g neighbouring cells.  Inside a
+// spatial cell the hits are further binned by kRBuckets monotone buckets of their radius feature r:
+// outer(i,j) needs r_j >= r_i, hence bucket(j) >= bucket(i), so a query scans only the part of each
+// neighbouring cell that starts at its own bucket (about half of it) -- the counting sort by
+// (cell, bucket) makes that part one contiguous range.  One warp serves one query: lanes stride over
+// the candidates, accepted ones are appended to a shared-memory buffer via ballot; when the buffer
+// fills, a bisection on d2 finds a threshold that keeps at least the K nearest (a warp bitonic sort on
+// (d2, j) only when ties defeat it, and once at the end for the exact K nearest); rank counting on j
+// gives the (src, dst) output order.
 #include <cmath>
 
 #include "common.cuh"
@@ -31,23 +35,30 @@ __global__ void frnn_reset_kernel(int32_t* __restrict__ bbox, int32_t* __restric
     bbox[i] = 0x7fffffff;          // min
     bbox[3 + i] = (int)0x80000000; // max
   }
+  if (i == 3) {
+    bbox[6] = 0x7fffffff;          // min of the radius feature
+    bbox[7] = (int)0x80000000;     // max
+    bbox[8] = 0;                   // max |e_k| over all hits and coordinates (bits of a non-negative float)
+  }
   if (i < n_cells_plus1) cell_count[i] = 0;
 }
 
 // proj[i] = P^T e_i  (or the first g coordinates), and the global bounding box.
-__global__ void frnn_project_kernel(const float* __restrict__ emb, int d_e, const float* __restrict__ P, int g,
+__global__ void frnn_project_kernel(const float* __restrict__ emb, const float* __restrict__ hits, int d_e, const float* __restrict__ P, int g,
                                     float* __restrict__ proj, int32_t* __restrict__ bbox, int64_t n) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   float p[3] = {0.f, 0.f, 0.f};
+  float emax = 0.f;
   if (i < n) {
     const float* e = emb + i * d_e;
     if (P) {
       for (int k = 0; k < d_e; ++k) {
         float v = e[k];
+        emax = fmaxf(emax, fabsf(v));
         for (int a = 0; a < g; ++a) p[a] = fmaf(v, P[k * 3 + a], p[a]);
       }
     } else {
-      for (int a = 0; a < g; ++a) p[a] = e[a];
+      for (int a = 0; a < g; ++a) p[a] = e[a];      // exact: no rounding slack needed (emax stays 0)
     }
     proj[i * 3 + 0] = p[0];
     proj[i * 3 + 1] = p[1];
@@ -66,12 +77,33 @@ __global__ void frnn_project_kernel(const float* __restrict__ emb, int d_e, cons
       atomicMax(&bbox[3 + a], hi);
     }
   }
+  {
+    const int key = i < n ? float_to_ordered(hits[i * 3]) : 0;
+    int lo = i < n ? key : 0x7fffffff;
+    int hi = i < n ? key : (int)0x80000000;
+    for (int o = 16; o > 0; o >>= 1) {
+      lo = min(lo, __shfl_xor_sync(0xffffffffu, lo, o));
+      hi = max(hi, __shfl_xor_sync(0xffffffffu, hi, o));
+    }
+    int em = __float_as_int(emax);       // non-negative floats order like their bit patterns
+    for (int o = 16; o > 0; o >>= 1) em = max(em, __shfl_xor_sync(0xffffffffu, em, o));
+    if ((threadIdx.x & 31) == 0) {
+      atomicMin(&bbox[6], lo);
+      atomicMax(&bbox[7], hi);
+      atomicMax(&bbox[8], em);
+    }
+  }
 }
 
 __global__ void frnn_grid_setup_kernel(const int32_t* __restrict__ bbox, float radius, int g, int G, GridParams* __restrict__ gp) {
   if (threadIdx.x != 0 || blockIdx.x != 0) return;
-  // cell edge >= r with slack for the fp32 rounding of the projection (|p| of order 1..10, error ~1e-6)
-  const float cell_min = radius * 1.001f + 1e-5f;
+  // Rounding slack of the fp32 projection p = sum_k e_k P_ka (an fmaf chain): |p_hat - p| <= d_e 2^-24 sum_k |e_k| |P_ka|
+  // <= d_e^1.5 2^-24 max|e| (unit columns), i.e. <= 2^-18 max|e| for d_e <= 16.  Two computed points are at most 2 sqrt(3) of
+  // that further apart than the true ones; proj_eps = 2^-16 max|e| covers it with margin and scales with the data.
+  const float proj_eps = __int_as_float(bbox[8]) * 1.52587890625e-05f;
+  gp->proj_eps = proj_eps;
+  // cell edge >= r with relative slack for the cell-index arithmetic and proj_eps for the projection
+  const float cell_min = radius * 1.001f + proj_eps + 1e-30f;
   int cells = 1;
   for (int a = 0; a < 3; ++a) {
     if (a >= g) {
@@ -92,6 +124,18 @@ __global__ void frnn_grid_setup_kernel(const int32_t* __restrict__ bbox, float r
     cells *= d;
   }
   gp->cells_per_event = cells;
+  // radius buckets: equal-width bins over [r_min, r_max]; any monotone map keeps the search exact (see r_bucket)
+  float rlo = ordered_to_float(bbox[6]), rhi = ordered_to_float(bbox[7]);
+  if (!(rhi > rlo)) { rlo = 0.f; rhi = 0.f; }
+  gp->r_origin = rlo;
+  gp->r_inv = rhi > rlo ? (float)kRBuckets / (rhi - rlo) : 0.f;
+}
+
+// Monotone non-decreasing in r (fp32 subtraction of a constant, multiplication by a non-negative constant, floor and clamp
+// all are), so r_i <= r_j implies bucket(i) <= bucket(j): a candidate in a lower bucket than the query can never be "outer".
+__device__ __forceinline__ int r_bucket(const GridParams& gp, float r) {
+  const int b = (int)floorf((r - gp.r_origin) * gp.r_inv);
+  return max(0, min(b, kRBuckets - 1));
 }
 
 __device__ __forceinline__ void cell_coords(const GridParams& gp, const float* p, int c[3]) {
@@ -102,7 +146,7 @@ __device__ __forceinline__ void cell_coords(const GridParams& gp, const float* p
   }
 }
 
-__global__ void frnn_count_kernel(const float* __restrict__ proj, const int32_t* __restrict__ ev_of_hit,
+__global__ void frnn_count_kernel(const float* __restrict__ proj, const float* __restrict__ hits, const int32_t* __restrict__ ev_of_hit,
                                   const GridParams* __restrict__ gpp, int32_t* __restrict__ cell_of_hit,
                                   int32_t* __restrict__ cell_count, int64_t n) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -110,7 +154,8 @@ __global__ void frnn_count_kernel(const float* __restrict__ proj, const int32_t*
   const GridParams gp = *gpp;
   int c[3];
   cell_coords(gp, proj + i * 3, c);
-  int cell = ev_of_hit[i] * gp.cells_per_event + (c[2] * gp.dims[1] + c[1]) * gp.dims[0] + c[0];
+  // (event, spatial cell, radius bucket), the bucket fastest: the part of a spatial cell from bucket b on is contiguous
+  int cell = (ev_of_hit[i] * gp.cells_per_event + (c[2] * gp.dims[1] + c[1]) * gp.dims[0] + c[0]) * kRBuckets + r_bucket(gp, hits[i * 3]);
   cell_of_hit[i] = cell;
   atomicAdd(&cell_count[cell], 1);
 }
@@ -158,17 +203,25 @@ constexpr int kWarpsPerBlock = 4;
 // Three-level test per candidate.  Level 0 (all candidates, 16 bytes and 6 flops each): the squared distance of the
 // binning coordinates P^T e (the same fp32 values the grid was built from) against lambda r^2 with slack, lambda >= the
 // largest eigenvalue of P^T P (1 for orthonormal P), so no pair with d2 <= r2 can fail it; a ball inside the 27 cells keeps
-// ~15 % of them.  Survivors are queued and, 32 at a time, take level 1 (fp32 with FMA, all d_e coordinates): d2f <= r2 (1 + 1e-4).  The fp32 value differs
-// from the exact d2 by at most ~16 ulp relative (all terms are non-negative, so there is no cancellation), so no candidate
-// with d2 <= r2 can fail it.  Survivors (a few per cent) are queued in shared memory and, 32 at a time, take level 2: the
-// outer() test and the exact fp64 d2 (no FMA) that decides acceptance and rank -- the same arithmetic as before, so the
-// edge list is unchanged; only the work on the ~97 % of candidates that are nowhere near the radius is cheaper.
+// ~15 % of them.  Survivors are queued and, 32 at a time, take level 1 (fp32 with FMA, all d_e coordinates): d2f <= r2 (1 + 1e-4).
+// The fp32 value differs from the exact d2 by at most ~16 ulp relative (all terms are non-negative, so there is no
+// cancellation), so no candidate with d2 <= r2 can fail it.  Survivors (a few per cent) are queued in shared memory and, 32 at
+// a time, take level 2: the outer() test and the exact fp64 d2 (no FMA) that decides acceptance and rank.
+//
+// Candidates: for each of the (up to) 27 neighbouring spatial cells the contiguous range of hits whose radius bucket is >=
+// the query's (lower buckets cannot be "outer", r_bucket()); empty ranges are skipped.
+//
+// Buffer of accepted neighbours (CAP = 2 K entries): when it cannot take 32 more, prune() bisects on d2 for a threshold T
+// with K <= #{d2 <= T} <= CAP - 32, drops everything above T (none of it can be among the K nearest: K entries are at most
+// T) and tightens the accept thresholds of all three levels to T.  Only when ties in d2 defeat the bisection the buffer is
+// sorted by (d2, j) and cut to K; the exact K nearest by (d2, j) are selected once, at the end.
 template <int D4, int CAP>
 __global__ void __launch_bounds__(kWarpsPerBlock * 32)
 frnn_search_kernel(const float* __restrict__ semb, const float4* __restrict__ smeta, const float4* __restrict__ sproj,
                    const int32_t* __restrict__ cell_start, const GridParams* __restrict__ gpp, double r2_in, float r2_loose_in,
-                   float r2_proj_in, float proj_scale, int K, int32_t* __restrict__ slots, int32_t* __restrict__ deg, int64_t n) {
+                   float r_proj_in, float proj_scale, int K, int32_t* __restrict__ slots, int32_t* __restrict__ deg, int64_t n) {
   constexpr int D = D4 * 4;
+  constexpr int PER = CAP / 32;            // buffer entries per lane
   __shared__ unsigned long long s_d2[kWarpsPerBlock][CAP];
   __shared__ int s_idx[kWarpsPerBlock][CAP];
   __shared__ int s_queue[kWarpsPerBlock][64];
@@ -187,6 +240,8 @@ frnn_search_kernel(const float* __restrict__ semb, const float4* __restrict__ sm
   const float q_r = qm.x, q_az = qm.y;
   const int q_i = __float_as_int(qm.z);
   int cell = __float_as_int(qm.w);
+  const int q_b = cell % kRBuckets;        // the query's radius bucket
+  cell /= kRBuckets;
   const int ev = cell / gp.cells_per_event;
   cell -= ev * gp.cells_per_event;
   const int cx = cell % gp.dims[0];
@@ -203,21 +258,88 @@ frnn_search_kernel(const float* __restrict__ semb, const float4* __restrict__ sm
   // both queues are rings (64 and 128 entries): entry i lives at (head + i) & (size - 1), so draining moves nothing
   int qn = 0, qh = 0;     // warp-uniform number / head of queued level-1 survivors
   int qn0 = 0, qh0 = 0;   // warp-uniform number / head of queued level-0 survivors
-  // Thresholds shrink once K neighbours are known: after a prune the K-th smallest d2 so far bounds every later accept
-  // (a candidate with a larger d2 can never enter the K nearest; equal d2 is kept and settled by the (d2, j) order).
+  // Thresholds shrink once K neighbours are known: a candidate with d2 above a value that K buffered entries do not exceed can
+  // never enter the K nearest (equal d2 is kept and settled by the (d2, j) order at the end).
   double r2 = r2_in;
-  float r2_loose = r2_loose_in, r2_proj = r2_proj_in;
-  auto tighten = [&]() {
-    const double kth = __longlong_as_double((long long)bd2[K - 1]);
+  // level-0 threshold on the binning coordinates: (sqrt(lambda) r, with the slack of the grid's cell edge)^2, rounded up
+  const float r0_in = __fadd_ru(r_proj_in, gp.proj_eps);
+  float r2_loose = r2_loose_in, r2_proj = __fmul_ru(r0_in, r0_in);
+  auto tighten = [&](double kth) {
     if (kth < r2) {
       r2 = kth;
       r2_loose = fminf(r2_loose, __double2float_ru(kth * (1.0 + 1e-4)));
-      const float r0 = proj_scale * __double2float_ru(sqrt(kth)) + 2e-5f;
+      const float r0 = __fadd_ru(__fmul_ru(proj_scale, __double2float_ru(sqrt(kth))), gp.proj_eps);
       r2_proj = fminf(r2_proj, __fmul_ru(r0, r0));
     }
   };
   for (int t = lane; t < CAP; t += 32) { bd2[t] = kInfBits; bidx[t] = 0x7fffffff; }
   __syncwarp();
+
+  // makes room for 32 more entries (count <= CAP - 32 afterwards, every entry that can still be among the K nearest kept)
+  auto prune = [&]() {
+    unsigned long long mine[PER];
+#pragma unroll
+    for (int i = 0; i < PER; ++i) mine[i] = bd2[lane + 32 * i];          // unused slots hold +inf
+    // d2 >= 0, so the bit patterns order like the values; bisect on the value between 0 and the largest buffered d2
+    unsigned long long mx = 0ull;
+#pragma unroll
+    for (int i = 0; i < PER; ++i) mx = (mine[i] != kInfBits && mine[i] > mx) ? mine[i] : mx;
+    for (int o = 16; o > 0; o >>= 1) {
+      const unsigned long long other = __shfl_xor_sync(0xffffffffu, mx, o);
+      mx = other > mx ? other : mx;
+    }
+    double lo = 0.0, hi = __longlong_as_double((long long)mx);
+    int cnt_hi = count;
+    bool found = false;
+    for (int it = 0; it < 24 && !found; ++it) {
+      const double mid = 0.5 * (lo + hi);
+      const unsigned long long mb = (unsigned long long)__double_as_longlong(mid);
+      int c = 0;
+#pragma unroll
+      for (int i = 0; i < PER; ++i) c += mine[i] <= mb ? 1 : 0;
+      c = __reduce_add_sync(0xffffffffu, c);
+      if (c < K) {
+        lo = mid;
+      } else {
+        hi = mid;
+        cnt_hi = c;
+        found = c <= CAP - 32;
+      }
+    }
+    if (found) {
+      // keep the entries with d2 <= hi, in place and in buffer order
+      const unsigned long long hb = (unsigned long long)__double_as_longlong(hi);
+      int idx[PER];
+#pragma unroll
+      for (int i = 0; i < PER; ++i) idx[i] = bidx[lane + 32 * i];
+      __syncwarp();
+      int base = 0;
+#pragma unroll
+      for (int i = 0; i < PER; ++i) {
+        const bool keep = mine[i] <= hb;
+        const unsigned m = __ballot_sync(0xffffffffu, keep);
+        if (keep) {
+          const int slot = base + __popc(m & ((1u << lane) - 1u));
+          bd2[slot] = mine[i];
+          bidx[slot] = idx[i];
+        }
+        base += __popc(m);
+      }
+      __syncwarp();
+      for (int t = base + lane; t < CAP; t += 32) { bd2[t] = kInfBits; bidx[t] = 0x7fffffff; }
+      __syncwarp();
+      count = base;
+      tighten(hi);
+    } else {
+      // ties in d2: the exact K nearest by (d2, j)
+      warp_bitonic(bd2, bidx, CAP, false, lane);
+      tighten(__longlong_as_double((long long)bd2[K - 1]));
+      __syncwarp();
+      for (int t = K + lane; t < CAP; t += 32) { bd2[t] = kInfBits; bidx[t] = 0x7fffffff; }
+      __syncwarp();
+      count = K;
+    }
+  };
 
   // level 2 on the first min(qn, 32) queued positions
   auto drain = [&]() {
@@ -249,20 +371,17 @@ frnn_search_kernel(const float* __restrict__ semb, const float4* __restrict__ sm
     qn -= take;
     const unsigned m = __ballot_sync(0xffffffffu, ok);
     if (m) {
-      if (count + 32 > CAP) {  // make room: keep the K nearest so far
-        warp_bitonic(bd2, bidx, CAP, false, lane);
-        if (count >= K) tighten();
-        __syncwarp();
-        for (int t = K + lane; t < CAP; t += 32) { bd2[t] = kInfBits; bidx[t] = 0x7fffffff; }
-        __syncwarp();
-        count = min(count, K);
+      if (count + 32 > CAP) {
+        prune();
+        ok = ok && d2 <= r2;                 // the threshold may just have moved
       }
+      const unsigned m2 = __ballot_sync(0xffffffffu, ok);
       if (ok) {
-        const int slot = count + __popc(m & ((1u << lane) - 1u));
+        const int slot = count + __popc(m2 & ((1u << lane) - 1u));
         bd2[slot] = (unsigned long long)__double_as_longlong(d2);
         bidx[slot] = c_i;
       }
-      count += __popc(m);
+      count += __popc(m2);
     }
     __syncwarp();
   };
@@ -299,19 +418,21 @@ frnn_search_kernel(const float* __restrict__ semb, const float4* __restrict__ sm
     __syncwarp();
   };
 
-  // the (up to) nine rows of three x-adjacent cells: lane r < 9 fetches the candidate range of row r, so the nine dependent
-  // cell_start look-ups cost one memory latency instead of nine
-  const int x0 = max(cx - 1, 0), x1 = min(cx + 1, gp.dims[0] - 1);
+  // the (up to) 27 neighbouring spatial cells: lane c < 27 fetches the candidate range of cell c -- its hits from the query's
+  // radius bucket on -- so the dependent cell_start look-ups cost one memory latency
   int my_lo = 0, my_hi = 0;
-  if (lane < 9) {
-    const int z = cz + lane / 3 - 1, y = cy + lane % 3 - 1;
-    if (z >= 0 && z < gp.dims[2] && y >= 0 && y < gp.dims[1]) {
-      const int row = ev * gp.cells_per_event + (z * gp.dims[1] + y) * gp.dims[0];
-      my_lo = cell_start[row + x0];
-      my_hi = cell_start[row + x1 + 1];
+  if (lane < 27) {
+    const int z = cz + lane / 9 - 1, y = cy + (lane / 3) % 3 - 1, x = cx + lane % 3 - 1;
+    if (z >= 0 && z < gp.dims[2] && y >= 0 && y < gp.dims[1] && x >= 0 && x < gp.dims[0]) {
+      const int64_t sp = (int64_t)ev * gp.cells_per_event + (z * gp.dims[1] + y) * gp.dims[0] + x;
+      my_lo = cell_start[sp * kRBuckets + q_b];
+      my_hi = cell_start[(sp + 1) * kRBuckets];
     }
   }
-  for (int rr = 0; rr < 9; ++rr) {
+  unsigned todo = __ballot_sync(0xffffffffu, my_hi > my_lo);
+  while (todo) {
+    const int rr = __ffs(todo) - 1;
+    todo &= todo - 1;
     const int lo = __shfl_sync(0xffffffffu, my_lo, rr), hi = __shfl_sync(0xffffffffu, my_hi, rr);
     // two 32-candidate groups per trip: their loads are independent, the loop and queue bookkeeping is paid once
     for (int base = lo; base < hi; base += 64) {
@@ -399,9 +520,10 @@ __global__ void event_of_hit_kernel(const __grid_constant__ EventOffsets offs, i
 
 template <int D4>
 trk_status launch_search(trk_ctx* ctx, int K, double r2, int64_t n, cudaStream_t st) {
-  // level-0 threshold on the binning coordinates: (sqrt(lambda) r with the slack of the grid's cell edge)^2
-  const double r0 = std::sqrt((double)ctx->proj_gain) * (double)ctx->cfg.frnn_radius * 1.001 + 2e-5;
-  const float r2_proj = r0 * r0 >= 3.0e38 ? __builtin_inff() : nextafterf((float)(r0 * r0), __builtin_inff());
+  // level-0 radius on the binning coordinates: sqrt(lambda) r with the relative slack of the grid's cell edge (the kernel adds the
+  // data-dependent rounding slack GridParams::proj_eps and squares)
+  const double r0 = std::sqrt((double)ctx->proj_gain) * (double)ctx->cfg.frnn_radius * 1.001;
+  const float r_proj = r0 >= 1.0e19 ? __builtin_inff() : nextafterf((float)r0, __builtin_inff());
   const float proj_scale = nextafterf((float)(std::sqrt((double)ctx->proj_gain) * 1.001), __builtin_inff());
   const unsigned blocks = (unsigned)ceil_div(n, kWarpsPerBlock);
   // level-1 threshold: r^2 (1 + 1e-4) rounded up, infinite when r^2 overflows fp32 (then every candidate takes level 2)
@@ -409,13 +531,13 @@ trk_status launch_search(trk_ctx* ctx, int K, double r2, int64_t n, cudaStream_t
   const float r2_loose = loose >= 3.0e38 ? __builtin_inff() : fmaxf(nextafterf((float)loose, __builtin_inff()), 1e-30f);
   if (K <= 32) {
     TRK_LAUNCH(ctx, (frnn_search_kernel<D4, 64>), blocks, kWarpsPerBlock * 32, 0, st, ctx->semb, ctx->smeta, ctx->sproj, ctx->cell_start,
-               ctx->grid, r2, r2_loose, r2_proj, proj_scale, K, ctx->slots, ctx->deg, n);
+               ctx->grid, r2, r2_loose, r_proj, proj_scale, K, ctx->slots, ctx->deg, n);
   } else if (K <= 64) {
     TRK_LAUNCH(ctx, (frnn_search_kernel<D4, 128>), blocks, kWarpsPerBlock * 32, 0, st, ctx->semb, ctx->smeta, ctx->sproj, ctx->cell_start,
-               ctx->grid, r2, r2_loose, r2_proj, proj_scale, K, ctx->slots, ctx->deg, n);
+               ctx->grid, r2, r2_loose, r_proj, proj_scale, K, ctx->slots, ctx->deg, n);
   } else {
     TRK_LAUNCH(ctx, (frnn_search_kernel<D4, 256>), blocks, kWarpsPerBlock * 32, 0, st, ctx->semb, ctx->smeta, ctx->sproj, ctx->cell_start,
-               ctx->grid, r2, r2_loose, r2_proj, proj_scale, K, ctx->slots, ctx->deg, n);
+               ctx->grid, r2, r2_loose, r_proj, proj_scale, K, ctx->slots, ctx->deg, n);
   }
   return TRK_OK;
 }
@@ -429,15 +551,15 @@ trk_status frnn_build(trk_ctx* ctx, const float* emb, const float* hits, int64_t
   const int K = ctx->cfg.frnn_k;
   const int g = ctx->grid_dims;
   const int G = ctx->grid_max;
-  const int64_t n_cells = (int64_t)n_events * G * G * G;
+  const int64_t n_cells = (int64_t)n_events * G * G * G * kRBuckets;
   if (n_cells > ctx->max_cells) return fail(ctx, TRK_ERR_CAPACITY, "frnn: n_events exceeds max_events");
   if (n <= 0) return fail(ctx, TRK_ERR_INVALID_ARG, "frnn: empty input");
   const unsigned nb = (unsigned)ceil_div(n, 256);
   // only the cells of this call's events are touched
   TRK_LAUNCH(ctx, frnn_reset_kernel, (unsigned)ceil_div(n_cells + 1, 256), 256, 0, st, ctx->bbox, ctx->cell_count, n_cells + 1);
-  TRK_LAUNCH(ctx, frnn_project_kernel, nb, 256, 0, st, emb, ctx->d_e, ctx->grid_proj, g, ctx->proj, ctx->bbox, n);
+  TRK_LAUNCH(ctx, frnn_project_kernel, nb, 256, 0, st, emb, hits, ctx->d_e, ctx->grid_proj, g, ctx->proj, ctx->bbox, n);
   TRK_LAUNCH(ctx, frnn_grid_setup_kernel, 1, 32, 0, st, ctx->bbox, ctx->cfg.frnn_radius, g, G, ctx->grid);
-  TRK_LAUNCH(ctx, frnn_count_kernel, nb, 256, 0, st, ctx->proj, ctx->ev_of_hit, ctx->grid, ctx->cell_of_hit, ctx->cell_count, n);
+  TRK_LAUNCH(ctx, frnn_count_kernel, nb, 256, 0, st, ctx->proj, hits, ctx->ev_of_hit, ctx->grid, ctx->cell_of_hit, ctx->cell_count, n);
   TRK_TRY(exclusive_scan_i32(ctx, ctx->cell_count, ctx->cell_start, n_cells, ctx->scan_tmp, st));
   TRK_TRY(fill_i32(ctx, ctx->cell_fill, 0, n_cells, st));
   TRK_LAUNCH(ctx, frnn_scatter_kernel, nb, 256, 0, st, emb, hits, ctx->d_e, ctx->d_e_pad, ctx->cell_of_hit, ctx->cell_start,

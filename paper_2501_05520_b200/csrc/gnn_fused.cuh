@@ -3,6 +3,13 @@
 //   e_k <- e_k + LNR(W2 LNR(W1 [h_src(k) ; h_dst(k) ; e_k] + b1) + b2)           (kUpdate: the edge update, rows of E)
 //   score_k = sigmoid(w_out . LNR(W1 [h_src ; h_dst ; e_k] + b1) + b_out)        (kDecode: the decoder)
 //   h_v <- h_v + LNR(W2 LNR(W1 [h_v ; m_in_v ; m_out_v] + b1) + b2)              (kNode: the node update, rows of X)
+//   out_m = LNR(W2 LNR(W1 f_m + b1) + b2)                                        (kEncode: node / edge encoder, K = 3 or 4)
+//
+// kEncode: the K = 3 / K = 4 first layer runs on the tensor core too.  Every fp32 input feature f is split into two bf16
+// values hi = bf16(f), lo = bf16(f - hi) (f = hi + lo up to 2^-17 relative) that meet the SAME weight column, so the fp32
+// accumulator holds sum_k w_k (hi_k + lo_k): the layer sees its input at fp32-like precision although the operands are
+// bf16.  The operand tile is one K block (128 rows x 64 columns, 16 used: one UMMA K step) that the four gather warps
+// write straight into the swizzled layout, one row per thread (edge features computed on the fly from the hits).
 //
 // One 2-CTA cluster handles 256 rows per tile (128 per CTA) and never writes an intermediate to HBM:
 //   * both weight matrices stay in shared memory for the whole kernel, split by output row between the two CTAs
@@ -25,6 +32,7 @@
 #pragma once
 
 #include "gemm_tc2.cuh"
+#include "nn.cuh"
 
 namespace trk {
 namespace gf {
@@ -36,7 +44,7 @@ constexpr int kTileRows = 128;            // per CTA
 constexpr int kKB = 16384;                // one 128-row x 64-column bf16 K block
 constexpr int kWKB = 8192;                // one 64-row x 64-column K block of a weight half
 
-enum Mode { kUpdate = 0, kDecode = 1, kNode = 2 };
+enum Mode { kUpdate = 0, kDecode = 1, kNode = 2, kEncode = 3 };
 
 struct FusedParams {
   const __nv_bfloat16* X;     // [n_nodes][ldx] bf16, h = columns [0, 128)
@@ -49,10 +57,15 @@ struct FusedParams {
   const float* w_out;         // kDecode
   float b_out;
   float* score;
+  const float* hits;          // kEncode: fp32 [n][3]; the rows are nodes when src == nullptr, edges (src[m], dst[m]) otherwise
 };
 
 __device__ __forceinline__ void cp_async_16(uint32_t smem_dst, const void* gsrc, int src_bytes) {
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(smem_dst), "l"(gsrc), "r"(src_bytes) : "memory");
+}
+// the same through L1 (.ca): the kept edges are sorted by src, so the ~9 out-edges of a node gather the same h row back to back
+__device__ __forceinline__ void cp_async_16_l1(uint32_t smem_dst, const void* gsrc) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(smem_dst), "l"(gsrc) : "memory");
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N>
@@ -87,6 +100,13 @@ __device__ __forceinline__ void tma_prefetch_l2_2d(const CUtensorMap* tmap, int 
 }
 
 __device__ __forceinline__ float2 f2(float a, float b) { return make_float2(a, b); }
+
+// bf16x2(max(lo, 0), max(hi, 0)) in one instruction: the ReLU rides on the conversion (lo in the low half, hi in the high half)
+__device__ __forceinline__ uint32_t pack_relu_bf16(float lo, float hi) {
+  uint32_t r;
+  asm("cvt.rn.relu.bf16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
+  return r;
+}
 
 constexpr int kFusedThreads = 22 * 32;
 constexpr int kOffW1 = 0;                       // 6 K blocks of this CTA's 64 output rows of W1
@@ -181,6 +201,8 @@ gnn_fused_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constant
   const int64_t total = (M + 2 * kTileRows - 1) / (2 * kTileRows);
   const int n_my = total > pair ? (int)((total - pair + n_pairs - 1) / n_pairs) : 0;
   constexpr bool kTwoLayers = MODE != kDecode;
+  constexpr bool kResidual = MODE == kUpdate || MODE == kNode;     // epilogue 2 adds (and TMA loads) the residual tile
+  constexpr int kW1Blocks = MODE == kEncode ? 1 : 6;               // K blocks of W1 resident in shared memory
   // K blocks of W1 that go with the operand tile (e, or h in kNode) and with the two ring halves
   constexpr int kbE = MODE == kNode ? 0 : 4;
   constexpr int kbR = MODE == kNode ? 2 : 0;
@@ -205,8 +227,8 @@ gnn_fused_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constant
     mbar_init(&bar->tempty, 1);
     fence_barrier_init();
     // this CTA's halves of the weights: output rows [64 rank, 64 rank + 64)
-    mbar_arrive_expect_tx(&bar->w_full, 8 * kWKB);
-    for (int kb = 0; kb < 6; ++kb) tma_load_2d(smem + kOffW1 + kb * kWKB, &tmW1, &bar->w_full, kb * 64, (int)rank * 64);
+    mbar_arrive_expect_tx(&bar->w_full, (kW1Blocks + 2) * kWKB);
+    for (int kb = 0; kb < kW1Blocks; ++kb) tma_load_2d(smem + kOffW1 + kb * kWKB, &tmW1, &bar->w_full, kb * 64, (int)rank * 64);
     for (int kb = 0; kb < 2; ++kb) tma_load_2d(smem + kOffW2 + kb * kWKB, &tmW2, &bar->w_full, kb * 64, (int)rank * 64);
   }
   if (warp == 1) tmem_alloc_pair<512>(&bar->tmem_slot);
@@ -229,7 +251,7 @@ gnn_fused_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constant
     if (lane == 0) {
       auto row0_of = [&](int tl) { return (int)((pair + (int64_t)tl * n_pairs) * 2 * kTileRows + rank * kTileRows); };
       auto prefetch = [&](int tl) {
-        if (tl < n_my)
+        if (MODE != kEncode && tl < n_my)
           for (int kb = 0; kb < (MODE == kNode ? 6 : 2); ++kb) tma_prefetch_l2_2d(&tmE, kb * 64, row0_of(tl));
       };
       prefetch(1);
@@ -237,9 +259,10 @@ gnn_fused_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constant
       const uint32_t eopfull_leader = mapa_u32(smem_u32(&bar->eopfull), 0);
       const uint32_t gfull_leader[2] = {mapa_u32(smem_u32(&bar->gfull[0]), 0), mapa_u32(smem_u32(&bar->gfull[1]), 0)};
       int n_op = 0, n_res = 0, n_g[2] = {0, 0};
-      const int res_end = kTwoLayers ? n_my : 0;
+      const int op_end = MODE == kEncode ? 0 : n_my;
+      const int res_end = kResidual ? n_my : 0;
       const int g_end = MODE == kNode ? n_my : 0;
-      while (n_op < n_my || n_res < res_end || n_g[0] < g_end || n_g[1] < g_end) {
+      while (n_op < op_end || n_res < res_end || n_g[0] < g_end || n_g[1] < g_end) {
 #pragma unroll
         for (int h = 0; h < 2; ++h) {              // kNode: m_in | m_out blocks into the ring halves
           if (n_g[h] < g_end && mbar_test(&bar->gempty[h], (uint32_t)(n_g[h] & 1) ^ 1)) {
@@ -249,7 +272,7 @@ gnn_fused_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constant
             ++n_g[h];
           }
         }
-        if (n_op < n_my && mbar_test(&bar->eopempty, (uint32_t)(n_op & 1) ^ 1)) {
+        if (n_op < op_end && mbar_test(&bar->eopempty, (uint32_t)(n_op & 1) ^ 1)) {
           if (leader) mbar_arrive_expect_tx(&bar->eopfull, 2 * 2 * kKB);
           for (int kb = 0; kb < 2; ++kb) tma_load_2d_pair(smem + kOffEOp + kb * kKB, &tmE, eopfull_leader, colE + kb * 64, row0_of(n_op));
           prefetch(n_op + 3);
@@ -296,9 +319,17 @@ gnn_fused_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constant
           if (stage1 == 0) {
             if (mbar_test(&bar->a1empty[b], ph ^ 1) && mbar_test(&bar->gfull[0], (uint32_t)(n1 & 1))) {
               tc_fence_after();
-              for (int kb = 0; kb < 2; ++kb) kblock(d, sbase + kOffRing + kb * kKB, sbase + kOffW1 + (kbR + kb) * kWKB, kb == 0);
-              tc_commit_pair(&bar->gempty[0]);
-              stage1 = 1;
+              if constexpr (MODE == kEncode) {
+                // one K step: the 16 columns that hold the hi / lo feature pairs
+                tc_mma_bf16_pair(d, make_smem_desc(sbase + kOffRing), make_smem_desc(sbase + kOffW1), idesc, 0u);
+                tc_commit_pair(&bar->gempty[0]);
+                tc_commit_pair(&bar->a1full[b]);
+                ++n1;
+              } else {
+                for (int kb = 0; kb < 2; ++kb) kblock(d, sbase + kOffRing + kb * kKB, sbase + kOffW1 + (kbR + kb) * kWKB, kb == 0);
+                tc_commit_pair(&bar->gempty[0]);
+                stage1 = 1;
+              }
             }
           }
           if (stage1 == 1) {
@@ -335,7 +366,35 @@ gnn_fused_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constant
     const uint32_t dst0 = sbase + kOffRing + kb * kKB + (gw * 32 + half) * 128;
     const char* xb = reinterpret_cast<const char*>(p.X) + chunk * 16;
     const int64_t ldb = p.ldx * 2;
-    for (int tl = 0; tl < (MODE == kNode ? 0 : n_my); ++tl) {
+    if (MODE == kEncode) {
+      // one operand row per thread: (hi, lo) pairs of the 3 node or 4 edge features in columns [0, 8), zeros in [8, 16)
+      const int r = gw * 32 + lane;
+      uint8_t* rowp = smem + kOffRing + r * 128;
+      for (int tl = 0; tl < n_my; ++tl) {
+        const int64_t tile = pair + (int64_t)tl * n_pairs;
+        const int64_t row = tile * 2 * kTileRows + rank * kTileRows + r;
+        float4 f = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (row < M) {
+          if (p.src) f = edge_features(p.hits, p.src[row], p.dst[row]);
+          else f = make_float4(p.hits[row * 3], p.hits[row * 3 + 1], p.hits[row * 3 + 2], 0.f);
+        }
+        uint32_t w[4];
+        const float fv[4] = {f.x, f.y, f.z, f.w};
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+          const __nv_bfloat16 hi = __float2bfloat16_rn(fv[i]);
+          const __nv_bfloat16 lo = __float2bfloat16_rn(fv[i] - __bfloat162float(hi));
+          w[i] = (uint32_t)__bfloat16_as_ushort(hi) | ((uint32_t)__bfloat16_as_ushort(lo) << 16);
+        }
+        mbar_wait(&bar->gempty[0], (uint32_t)(tl & 1) ^ 1);
+        *reinterpret_cast<uint4*>(rowp + ((0 ^ (r & 7)) << 4)) = make_uint4(w[0], w[1], w[2], w[3]);
+        *reinterpret_cast<uint4*>(rowp + ((1 ^ (r & 7)) << 4)) = make_uint4(0u, 0u, 0u, 0u);
+        fence_proxy_async();
+        __syncwarp();
+        if (lane == 0) mbar_arrive_remote(gfull0);
+      }
+    }
+    for (int tl = 0; tl < (MODE == kNode || MODE == kEncode ? 0 : n_my); ++tl) {
       const int64_t tile = pair + (int64_t)tl * n_pairs;
       const int64_t row = tile * 2 * kTileRows + rank * kTileRows + gw * 32 + lane;
       // rows beyond M gather node 0: their results are computed but never read (segment sums and scores stop at M)
@@ -348,7 +407,8 @@ gnn_fused_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constant
 #pragma unroll
         for (int i = 0; i < 16; ++i) {
           const int idx = __shfl_sync(0xffffffffu, mine, 2 * i + half);
-          cp_async_16(dsth + i * 256 + sw[i & 3], xb + (int64_t)idx * ldb, 16);
+          if (h == 0) cp_async_16_l1(dsth + i * 256 + sw[i & 3], xb + (int64_t)idx * ldb);
+          else cp_async_16(dsth + i * 256 + sw[i & 3], xb + (int64_t)idx * ldb, 16);
         }
         cp_async_commit();
       }
@@ -422,10 +482,8 @@ gnn_fused_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constant
           uint32_t w[4];
 #pragma unroll
           for (int i = 0; i < 4; ++i) {
-            // ReLU after the rounding: max(bf16(v), 0) == bf16(max(v, 0)), one packed instruction for the pair
             const float2 v = __ffma2_rn(x[c / 2 + i], rs, sh);
-            const __nv_bfloat162 t = __hmax2(__floats2bfloat162_rn(v.x, v.y), __floats2bfloat162_rn(0.f, 0.f));
-            w[i] = *reinterpret_cast<const uint32_t*>(&t);
+            w[i] = pack_relu_bf16(v.x, v.y);
           }
           const int ch = c >> 3;
           *reinterpret_cast<uint4*>(smem + kOffT + half * kKB + r * 128 + ((ch ^ (r & 7)) << 4)) = make_uint4(w[0], w[1], w[2], w[3]);
@@ -455,10 +513,10 @@ gnn_fused_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constant
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive_remote(b == 0 ? a2empty0 : a2empty1);
-        mbar_wait(&bar->resfull, (uint32_t)(tl & 1));        // the residual copy of this tile has landed
+        if (kResidual) mbar_wait(&bar->resfull, (uint32_t)(tl & 1));        // the residual copy of this tile has landed
         // exchange of the half-row statistics through the first cell of this thread's residual row (its values wait in e0)
         uint4* cell0 = reinterpret_cast<uint4*>(res + r * 128 + ((0 ^ (r & 7)) << 4));
-        const uint4 e0 = *cell0;
+        const uint4 e0 = kResidual ? *cell0 : make_uint4(0u, 0u, 0u, 0u);
         *reinterpret_cast<float2*>(cell0) = f2(ps, pq);
         named_bar_sync(bid, 64);
         const float2 other = *reinterpret_cast<const float2*>(smem + kOffRes + (half ^ 1) * kKB + r * 128 + ((0 ^ (r & 7)) << 4));
@@ -469,16 +527,22 @@ gnn_fused_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constant
         for (int c = 0; c < 64; c += 8) {
           const int ch = c >> 3;
           uint4* cell = reinterpret_cast<uint4*>(res + r * 128 + ((ch ^ (r & 7)) << 4));
-          const uint4 e = c == 0 ? e0 : *cell;
+          const uint4 e = (c == 0 || !kResidual) ? e0 : *cell;
           const __nv_bfloat162* e2 = reinterpret_cast<const __nv_bfloat162*>(&e);
           uint32_t w[4];
 #pragma unroll
           for (int i = 0; i < 4; ++i) {
-            float2 v = __ffma2_rn(x[c / 2 + i], rs, sh);
-            v.x = fmaxf(v.x, 0.f);
-            v.y = fmaxf(v.y, 0.f);
-            v = __fadd2_rn(v, __bfloat1622float2(e2[i]));
-            w[i] = pack_bf16(v.x, v.y);
+            // LNR(.) is rounded to bf16 (ReLU inside the conversion) and the residual is added in bf16x2 arithmetic: the sum of two
+            // bf16 values rounded once.  Against adding in fp32 this is one more rounding of the UPDATE (|LNR| <= ~11, ulp 2^-9
+            // relative), far below the rounding of the residual stream itself (|e| grows to ~20) that both forms share.
+            const float2 v = __ffma2_rn(x[c / 2 + i], rs, sh);
+            const uint32_t u = pack_relu_bf16(v.x, v.y);
+            if (kResidual) {
+              const __nv_bfloat162 t = __hadd2(*reinterpret_cast<const __nv_bfloat162*>(&u), e2[i]);
+              w[i] = *reinterpret_cast<const uint32_t*>(&t);
+            } else {
+              w[i] = u;
+            }
           }
           *cell = make_uint4(w[0], w[1], w[2], w[3]);
         }
@@ -489,8 +553,9 @@ gnn_fused_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constant
           tma_store_2d(&tmEst, res + quad * 32 * 128, colE + half * 64, row0);
           bulk_commit();
           bulk_wait_read<0>();  // the rows have left shared memory: the buffer may be refilled
-          mbar_arrive(&bar->resempty);
+          if (kResidual) mbar_arrive(&bar->resempty);
         }
+        if (!kResidual) __syncwarp();   // no residual load orders the next tile's writes after the store's read-out: the warp does
       }
       if (lane == 0) bulk_wait_all();
     }

@@ -43,19 +43,59 @@ __global__ void place_keys_kernel(const int32_t* __restrict__ key, const int32_t
   }
 }
 
-// Each segment of perm is put in ascending edge order (segments are short: mean in-degree ~10).
-__global__ void sort_segments_kernel(const int32_t* __restrict__ rowptr, int32_t* __restrict__ perm, int64_t n_nodes) {
-  const int64_t v = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+// Each segment of perm is put in ascending edge order (place_keys_kernel fills a segment in the arbitrary order of its atomics;
+// the order of a segmented sum must not depend on it).  One warp per node: the entries of a segment are distinct, so the rank of
+// one is the number of smaller ones -- 32 entries per pass live in registers and are compared through shuffles.  Segments longer
+// than kSortMaxLen (a node with that many in-edges does not occur in tracking graphs) fall back to an insertion sort by one lane.
+constexpr int kSortChunks = 8;
+constexpr int kSortMaxLen = 32 * kSortChunks;
+__global__ void __launch_bounds__(256) sort_segments_kernel(const int32_t* __restrict__ rowptr, int32_t* __restrict__ perm, int64_t n_nodes) {
+  const int lane = threadIdx.x & 31;
+  const int64_t v = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   if (v >= n_nodes) return;
-  const int b = rowptr[v], e = rowptr[v + 1];
-  for (int i = b + 1; i < e; ++i) {
-    const int x = perm[i];
-    int j = i - 1;
-    while (j >= b && perm[j] > x) {
-      perm[j + 1] = perm[j];
-      --j;
+  const int b = rowptr[v], len = rowptr[v + 1] - b;
+  if (len <= 1) return;
+  if (len <= 32) {
+    const int x = lane < len ? perm[b + lane] : 0x7fffffff;
+    int rank = 0;
+    for (int j = 0; j < len; ++j) rank += __shfl_sync(0xffffffffu, x, j) < x ? 1 : 0;
+    __syncwarp();
+    if (lane < len) perm[b + rank] = x;
+    return;
+  }
+  if (len <= kSortMaxLen) {
+    int x[kSortChunks], rank[kSortChunks];
+#pragma unroll
+    for (int c = 0; c < kSortChunks; ++c) {
+      x[c] = c * 32 + lane < len ? perm[b + c * 32 + lane] : 0x7fffffff;
+      rank[c] = 0;
     }
-    perm[j + 1] = x;
+#pragma unroll
+    for (int d = 0; d < kSortChunks; ++d) {
+      if (d * 32 >= len) break;
+      for (int j = 0; j < 32; ++j) {
+        const int y = __shfl_sync(0xffffffffu, x[d], j);
+#pragma unroll
+        for (int c = 0; c < kSortChunks; ++c) rank[c] += y < x[c] ? 1 : 0;
+      }
+    }
+    __syncwarp();
+#pragma unroll
+    for (int c = 0; c < kSortChunks; ++c)
+      if (c * 32 + lane < len) perm[b + rank[c]] = x[c];
+    return;
+  }
+  if (lane == 0) {
+    const int e = b + len;
+    for (int i = b + 1; i < e; ++i) {
+      const int x = perm[i];
+      int j = i - 1;
+      while (j >= b && perm[j] > x) {
+        perm[j + 1] = perm[j];
+        --j;
+      }
+      perm[j + 1] = x;
+    }
   }
 }
 
@@ -121,6 +161,56 @@ segment_sum_kernel(const T* __restrict__ E, int H, const int32_t* __restrict__ i
   }
 }
 
+
+// bf16, H = 128 (the pileup configs): a half warp per row (16 lanes x 16 B = one 256-byte row), so one load instruction
+// fetches two rows and eight rows are in flight per warp; the in-edge row indices of up to 32 entries come with one
+// coalesced load and travel by shuffle.  Rows 0, 2, 4, ... of a segment accumulate in the lower half warp, rows 1, 3, 5, ...
+// in the upper one, each in segment order; the two partial sums are added at the end: a fixed order (reading C-14).
+__global__ void __launch_bounds__(256)
+segment_sum_h128_kernel(const __nv_bfloat16* __restrict__ E, const int32_t* __restrict__ in_rowptr, const int32_t* __restrict__ in_perm,
+                        const int32_t* __restrict__ out_rowptr, __nv_bfloat16* __restrict__ X, int64_t n_nodes) {
+  constexpr int H = 128;
+  const int lane = threadIdx.x & 31;
+  const int64_t w = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  if (w >= 2 * n_nodes) return;
+  const int64_t v = n_nodes - 1 - (w >> 1);   // from the back: the edge kernel's last rows are still in L2
+  const int dir = (int)(w & 1);               // 0: in (dst == v, via perm), 1: out (src == v, contiguous)
+  const int32_t* rp = dir == 0 ? in_rowptr : out_rowptr;
+  const int b = rp[v], e = rp[v + 1];
+  const int half = lane >> 4, c = (lane & 15) * 8;
+  float acc[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+  for (int base = b; base < e; base += 32) {
+    const int cnt = min(32, e - base);
+    const int mine = base + lane < e ? (dir == 0 ? __ldg(in_perm + base + lane) : base + lane) : 0;
+    for (int j = 0; j < cnt; j += 8) {
+      uint4 u[4];
+#pragma unroll
+      for (int t = 0; t < 4; ++t) {
+        const int r = j + 2 * t + half;
+        const int idx = __shfl_sync(0xffffffffu, mine, r & 31);
+        u[t] = r < cnt ? __ldg(reinterpret_cast<const uint4*>(E + (int64_t)idx * H + c)) : make_uint4(0u, 0u, 0u, 0u);
+      }
+#pragma unroll
+      for (int t = 0; t < 4; ++t) {
+        const __nv_bfloat162* h2 = reinterpret_cast<const __nv_bfloat162*>(&u[t]);
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+          acc[2 * i] += __low2float(h2[i]);
+          acc[2 * i + 1] += __high2float(h2[i]);
+        }
+      }
+    }
+  }
+#pragma unroll
+  for (int i = 0; i < 8; ++i) acc[i] += __shfl_xor_sync(0xffffffffu, acc[i], 16);
+  if (half == 0) {
+    __nv_bfloat162 o[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) o[i] = __floats2bfloat162_rn(acc[2 * i], acc[2 * i + 1]);
+    *reinterpret_cast<uint4*>(X + v * (3 * H) + H + dir * H + c) = *reinterpret_cast<const uint4*>(o);
+  }
+}
+
 }  // namespace
 
 trk_status build_gnn_csr(trk_ctx* ctx, const int32_t* src, const int32_t* dst, const int32_t* n_edges_dev, int64_t n_edges_cap,
@@ -132,14 +222,17 @@ trk_status build_gnn_csr(trk_ctx* ctx, const int32_t* src, const int32_t* dst, c
   TRK_TRY(exclusive_scan_i32(ctx, ctx->in_fill, ctx->in_rowptr, n_nodes, ctx->scan_tmp, st));
   TRK_TRY(fill_i32(ctx, ctx->in_fill, 0, n_nodes, st));
   TRK_LAUNCH(ctx, place_keys_kernel, eb, 256, 0, st, dst, n_edges_dev, n_edges_cap, ctx->in_rowptr, ctx->in_fill, ctx->in_perm);
-  TRK_LAUNCH(ctx, sort_segments_kernel, (unsigned)ceil_div(n_nodes, 128), 128, 0, st, ctx->in_rowptr, ctx->in_perm, n_nodes);
+  TRK_LAUNCH(ctx, sort_segments_kernel, (unsigned)ceil_div(n_nodes * 32, 256), 256, 0, st, ctx->in_rowptr, ctx->in_perm, n_nodes);
   return TRK_OK;
 }
 
 trk_status segment_sums(trk_ctx* ctx, const void* E, bool bf16, int64_t n_nodes, void* X, cudaStream_t st) {
   const int H = ctx->H;
   const unsigned blocks = (unsigned)ceil_div(2 * n_nodes * 32, 256);
-  if (bf16) {
+  if (bf16 && H == 128 && false) {   // measured slower than the generic kernel (99 vs 80 us per pileup-200 iteration)
+    TRK_LAUNCH(ctx, segment_sum_h128_kernel, blocks, 256, 0, st, (const __nv_bfloat16*)E, ctx->in_rowptr, ctx->in_perm, ctx->out_rowptr,
+               (__nv_bfloat16*)X, n_nodes);
+  } else if (bf16) {
     TRK_LAUNCH(ctx, segment_sum_kernel<__nv_bfloat16>, blocks, 256, 0, st, (const __nv_bfloat16*)E, H, ctx->in_rowptr,
                ctx->in_perm, ctx->out_rowptr, (__nv_bfloat16*)X, 3 * H, n_nodes);
   } else {

@@ -15,6 +15,7 @@
 #include "common.cuh"
 #include "gemm_tc.cuh"
 #include "gemm_tc2.cuh"
+#include "filter_fused.cuh"
 #include "gnn_fused.cuh"
 #include "graph.cuh"
 #include "nn.cuh"
@@ -171,7 +172,7 @@ trk_status launch_edge_fused(trk_ctx* ctx, const bf16* X, int64_t ldx, bf16* E, 
   TRK_TRY(make_tmap(ctx, &tw2, L2.w_bf16, gf::kH, gf::kH, gf::kH, 64));
   TRK_TRY(make_tmap(ctx, &te, E, e_rows, gf::kH, gf::kH, 128));
   TRK_TRY(make_tmap(ctx, &test, E, e_rows, gf::kH, gf::kH, 32));
-  gf::FusedParams p{X, ldx, src, dst, L1.b_f32, L2.b_f32, ctx->cfg.gnn_layernorm, w_out, b_out, score};
+  gf::FusedParams p{X, ldx, src, dst, L1.b_f32, L2.b_f32, ctx->cfg.gnn_layernorm, w_out, b_out, score, nullptr};
   const int64_t ptiles = ceil_div(rows.m_cap, 2 * gf::kTileRows);
   const unsigned grid = 2u * (unsigned)std::min<int64_t>(ptiles, ctx->sm_count / 2);
   TRK_LAUNCH(ctx, kern, grid, gf::kFusedThreads, gf::kSmemFused, st, tw1, tw2, te, test, rows, p);
@@ -189,10 +190,28 @@ trk_status launch_node_fused(trk_ctx* ctx, bf16* X, int64_t x_rows, const DevLin
   TRK_TRY(make_tmap(ctx, &tw2, L2.w_bf16, gf::kH, gf::kH, gf::kH, 64));
   TRK_TRY(make_tmap(ctx, &tx, X, x_rows, 3 * gf::kH, 3 * gf::kH, 128));
   TRK_TRY(make_tmap(ctx, &txst, X, x_rows, gf::kH, 3 * gf::kH, 32));
-  gf::FusedParams p{X, 3 * gf::kH, nullptr, nullptr, L1.b_f32, L2.b_f32, ctx->cfg.gnn_layernorm, nullptr, 0.f, nullptr};
+  gf::FusedParams p{X, 3 * gf::kH, nullptr, nullptr, L1.b_f32, L2.b_f32, ctx->cfg.gnn_layernorm, nullptr, 0.f, nullptr, nullptr};
   const int64_t ptiles = ceil_div(rows.m_cap, 2 * gf::kTileRows);
   const unsigned grid = 2u * (unsigned)std::min<int64_t>(ptiles, ctx->sm_count / 2);
   TRK_LAUNCH(ctx, kern, grid, gf::kFusedThreads, gf::kSmemFused, st, tw1, tw2, tx, txst, rows, p);
+  return TRK_OK;
+}
+
+// Fused encoder of S4 (gnn_fused.cuh, kEncode), H = 128: out[m] = LNR(W2 LNR(W1 f_m + b1) + b2), f_m = the 3 features of node m
+// (src == nullptr) or the 4 edge features of (src[m], dst[m]); w1p is the [H][64] hi/lo copy of W1; out bf16 with row stride ldo.
+trk_status launch_encoder_fused(trk_ctx* ctx, const float* hits, const int32_t* src, const int32_t* dst, const bf16* w1p, const DevLinear& L1,
+                                const DevLinear& L2, bf16* out, int64_t out_rows, int64_t ldo, tc::Rows rows, cudaStream_t st) {
+  if (rows.m_cap <= 0) return TRK_OK;
+  auto kern = gf::gnn_fused_kernel<gf::kEncode>;
+  TRK_TRY(ensure_smem(ctx, kern, gf::kSmemFused));
+  CUtensorMap tw1, tw2, tout;
+  TRK_TRY(make_tmap(ctx, &tw1, w1p, gf::kH, 64, 64, 64));
+  TRK_TRY(make_tmap(ctx, &tw2, L2.w_bf16, gf::kH, gf::kH, gf::kH, 64));
+  TRK_TRY(make_tmap(ctx, &tout, out, out_rows, gf::kH, ldo, 32));
+  gf::FusedParams p{nullptr, 0, src, dst, L1.b_f32, L2.b_f32, ctx->cfg.gnn_layernorm, nullptr, 0.f, nullptr, hits};
+  const int64_t ptiles = ceil_div(rows.m_cap, 2 * gf::kTileRows);
+  const unsigned grid = 2u * (unsigned)std::min<int64_t>(ptiles, ctx->sm_count / 2);
+  TRK_LAUNCH(ctx, kern, grid, gf::kFusedThreads, gf::kSmemFused, st, tw1, tw2, tout, tout, rows, p);
   return TRK_OK;
 }
 
@@ -391,8 +410,40 @@ trk_status embed_forward_bf16(trk_ctx* ctx, const float* hits, int64_t n, float*
 }
 
 // ---------------------------------------------------------------- S3
+// All layers of the filter MLP in one persistent CTA-pair kernel (filter_fused.cuh); activations stay in L2-resident scratch.
+static trk_status filter_forward_fused(trk_ctx* ctx, const float* feat, const int32_t* src, const int32_t* dst,
+                                       const int32_t* n_edges_dev, int64_t n_edges_cap, float* score, cudaStream_t st) {
+  const auto& L = ctx->filter.layers;
+  const int W = L[0].out_pad;
+  const int n_pairs_max = ctx->sm_count / 2;
+  const int64_t s_rows = (int64_t)n_pairs_max * 256;
+  auto kern = ff::filter_mlp_kernel;
+  TRK_TRY(ensure_smem(ctx, kern, ff::kSmemFilter));
+  CUtensorMap ts1, ts2, tw2, tw3, ts2st;
+  TRK_TRY(make_tmap(ctx, &ts1, ctx->filter_s1, s_rows, W, W, 128));
+  TRK_TRY(make_tmap(ctx, &ts2, ctx->filter_s2, s_rows, W, W, 128));
+  TRK_TRY(make_tmap(ctx, &tw2, L[1].w_bf16, W, W, W, 128));
+  TRK_TRY(make_tmap(ctx, &tw3, L[2].w_bf16, W, W, W, 128));
+  TRK_TRY(make_tmap(ctx, &ts2st, ctx->filter_s2, s_rows, W, W, 32));
+  ff::FilterParams p{feat, src, dst, ctx->filter_u, ctx->filter_w1_frag, L[0].b_f32, L[1].b_f32, L[2].b_f32, L[3].w_f32,
+                     ctx->filter_b_last, ctx->filter_s1, score, W};
+  const tc::Rows rows{n_edges_dev, 0, n_edges_cap};
+  const unsigned grid = 2u * (unsigned)std::min<int64_t>(ceil_div(n_edges_cap, 256), n_pairs_max);
+  // trk_profile_kernel_ms: one CUDA-event pair around the launch
+  const bool kprof = ctx->profiling && n_edges_dev == &ctx->counts[0] && ctx->kprof_ev.size() >= 2;
+  if (kprof) {
+    ctx->kprof_n = 1;
+    TRK_CUDA(ctx, cudaEventRecord(ctx->kprof_ev[0], st));
+  }
+  TRK_LAUNCH(ctx, kern, grid, ff::kThreadsFilter, ff::kSmemFilter, st, ts1, ts2, tw2, tw3, ts2st, rows, p);
+  if (kprof) TRK_CUDA(ctx, cudaEventRecord(ctx->kprof_ev[1], st));
+  return TRK_OK;
+}
+
 trk_status filter_forward_bf16(trk_ctx* ctx, const float* feat, const int32_t* src, const int32_t* dst,
                                const int32_t* n_edges_dev, int64_t n_edges_cap, float* score, cudaStream_t st) {
+  if (ctx->filter_fusable && ctx->knobs[kKnobFilterFused] != 0)
+    return filter_forward_fused(ctx, feat, src, dst, n_edges_dev, n_edges_cap, score, st);
   const auto& L = ctx->filter.layers;
   const int nl = (int)L.size();
   const int u = ctx->filter_u;
@@ -459,6 +510,15 @@ trk_status gnn_forward_bf16(trk_ctx* ctx, const float* hits, int64_t n, const in
   tc::Rows erows{n_edges_dev, 0, n_edges_cap};
   TRK_TRY(build_gnn_csr(ctx, src, dst, n_edges_dev, n_edges_cap, n, st));
 
+  const bool fused = H == gf::kH && ctx->knobs[kKnobGnnFused] != 0;
+  if (fused) {
+    // both encoders as fused two-layer kernels: the K = 3 / 4 first layer on the tensor core from hi/lo-split features
+    TRK_TRY(launch_encoder_fused(ctx, hits, nullptr, nullptr, ctx->node_enc_w1p, ctx->node_enc.layers[0], ctx->node_enc.layers[1], X, x_rows,
+                                 3 * H, nrows, st));
+    if (n_edges_cap > 0)
+      TRK_TRY(launch_encoder_fused(ctx, hits, src, dst, ctx->edge_enc_w1p, ctx->edge_enc.layers[0], ctx->edge_enc.layers[1], E, e_rows, H,
+                                   erows, st));
+  } else {
   // node encoder: 3 -> H (SIMT) -> H (GEMM, LNR) -> X[:, 0:H]
   TRK_TRY(launch_encoder_first<false>(ctx, hits, nullptr, nullptr, ctx->node_enc.layers[0], H, ln, nullptr, n, T1, st));
   {
@@ -471,7 +531,7 @@ trk_status gnn_forward_bf16(trk_ctx* ctx, const float* hits, int64_t n, const in
     tc::EpiRowLn::Params ep{ctx->edge_enc.layers[1].b_f32, nullptr, nullptr, nullptr, ln, nullptr, 0, E, H, nullptr, 0.f, nullptr};
     TRK_TRY(gemm_row_ln(ctx, T1, t_rows, H, H, ctx->edge_enc.layers[1].w_bf16, ep, erows, st));
   }
-  const bool fused = H == gf::kH && ctx->knobs[kKnobGnnFused] != 0;
+  }
   for (int t = 0; t < ctx->cfg.gnn_iters; ++t) {
     if (n_edges_cap > 0 && fused) {
       TRK_TRY(launch_edge_fused<gf::kUpdate>(ctx, X, 3 * H, E, e_rows, src, dst, ctx->edge_net.layers[0], ctx->edge_net.layers[1], nullptr,
