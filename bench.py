@@ -472,18 +472,23 @@ def main():
     # (trk_profile_kernel_ms); chunk c of launch i = c // 2 holds rows [c*chunk, (c+1)*chunk) clipped to E_c
     width = cfg["filter_dims"][1]
     k_flops, k_ms, k_n = 0.0, 0.0, 0
-    for ms_list, chunk_rows in kernel_ms:
+    chunk_rows = kernel_ms[0][1]
+    fused_filter = chunk_rows < 0        # one launch = every layer of the filter MLP over all candidate edges (filter_fused.cuh)
+    for ms_list, _ in kernel_ms:
         per_chunk = max(1, len(cfg["filter_dims"]) - 3)
         for i, ms in enumerate(ms_list):
-            rows = min(max(e_c - (i // per_chunk) * chunk_rows, 0), chunk_rows)
+            if fused_filter:
+                rows, flops = e_c, float(e_c) * FILTER_FLOP_PER_EDGE
+            else:
+                rows = min(max(e_c - (i // per_chunk) * chunk_rows, 0), chunk_rows)
+                flops = 2.0 * rows * width * width
             if rows > 0:
-                k_flops += 2.0 * rows * width * width
+                k_flops += flops
                 k_ms += ms
                 k_n += 1
     kern_tflops = k_flops / (k_ms * 1e-3) / 1e12 if k_ms > 0 else 0.0
-    chunk_rows = kernel_ms[0][1]
-    # ... and in isolation, at the per-launch shape of the pipeline (one full chunk, one hidden layer)
-    m_chunk = chunk_rows
+    # ... and a plain 1024 x 1024 layer in isolation on the GEMM kernel (1 212 416 rows: the chunk of the layer-by-layer path)
+    m_chunk = 128 * 148 * 64
     a = torch.randn(m_chunk, 1024, device=dev).to(torch.bfloat16)
     w = (torch.randn(1024, 1024, device=dev) / 32).to(torch.bfloat16)
     b = torch.zeros(1024, device=dev)
@@ -525,20 +530,25 @@ def main():
     # peak: the launches are ~1.2 ms kernels inside ~12 ms steps of a ~0.2 s timed region, far from the 4 s back-to-back run
     # that defines the "sustained" cuBLAS figure, so the burst figure is the denominator; the sustained one is given beside it.
     traffic = dominant_kernel_traffic()
+    kernel_name = ("ff::filter_mlp_kernel (the whole S3 filter MLP in one persistent CTA-pair kernel: layer 1 on mma.sync, the two 1024x1024 "
+                   "hidden layers on tcgen05.mma.cta_group::2 with L2-resident activations, the output layer in the epilogue; one launch = "
+                   "all candidate edges of the event)" if fused_filter else
+                   "tc::gemm_tc2_kernel<256,*> (tcgen05.mma.cta_group::2, the 1024x1024 hidden layers of the S3 filter MLP; "
+                   f"one launch = one layer of one {chunk_rows}-edge chunk)")
     roofline = {"bound": "tensor",
-                "kernel": "tc::gemm_tc2_kernel<256,*> (tcgen05.mma.cta_group::2, the 1024x1024 hidden layers of the S3 filter MLP; "
-                          f"one launch = one layer of one {chunk_rows}-edge chunk)",
+                "kernel": kernel_name,
                 "achieved": kern_tflops, "peak": peaks["bf16_tflops"], "unit": "TFLOP/s", "frac": kern_tflops / peaks["bf16_tflops"],
                 "peak_source": peaks["source"] + ", burst bf16 (short launches at burst clocks)",
                 "frac_of_sustained_peak": kern_tflops / peaks["bf16_sustained"], "sustained_peak": peaks["bf16_sustained"],
-                "launches_timed": k_n, "avg_launch_ms": k_ms / max(1, k_n), "flop_per_full_launch": 2.0 * chunk_rows * width * width,
-                "how": "algorithmic flops of the non-empty launches (2 x rows x 1024 x 1024 each) / their summed durations, CUDA-event pairs "
-                       f"around each launch on the launch stream (trk_profile_kernel_ms) in {prof_steps} profiled steps run right after the "
+                "launches_timed": k_n, "avg_launch_ms": k_ms / max(1, k_n),
+                "flop_per_launch": float(e_c) * FILTER_FLOP_PER_EDGE if fused_filter else 2.0 * chunk_rows * width * width,
+                "how": ("algorithmic flops of S3 (E_c x 4 245 504: all four layers) / the launch's duration, a CUDA-event pair " if fused_filter else
+                        "algorithmic flops of the non-empty launches (2 x rows x 1024 x 1024 each) / their summed durations, CUDA-event pairs ")
+                       + f"around each launch on the launch stream (trk_profile_kernel_ms) in {prof_steps} profiled steps run right after the "
                        "timed steps",
-                "traffic": traffic["bytes_per_full_launch"]["bias_act"] if traffic else None,
-                "traffic_unit": "bytes per full-chunk launch (EpiBiasActBf16 variant), ncu dram__bytes_read.sum + dram__bytes_write.sum",
-                "traffic_detail": dict(traffic or {}, algorithmic_bias_act=2 * chunk_rows * width * 2 + width * width * 2,
-                                       algorithmic_relu_dot=chunk_rows * width * 2 + width * width * 2 + chunk_rows * 16),
+                "traffic": traffic.get("bytes_per_launch") if traffic else None,
+                "traffic_unit": "bytes per launch, ncu dram__bytes_read.sum + dram__bytes_write.sum",
+                "traffic_detail": dict(traffic or {}, algorithmic_bytes_s3=e_c * 108),
                 "whole_stage": {"achieved": s3_tflops, "frac": s3_tflops / peaks["bf16_sustained"],
                                 "how": "algorithmic flops of S3 (E_c x 4 245 504) / S3 stage time (gather, 3 GEMMs, finish, compaction)"},
                 "isolated_launch": {"shape": [m_chunk, 1024, 1024], "ms": iso_ms, "achieved": iso_tflops,

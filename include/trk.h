@@ -98,10 +98,11 @@ typedef struct {
    * the paper states no minimum, reading C-23).  Used only when track outputs are wanted. */
   int32_t min_track_hits;
   /* Workspace / search-structure sizing, 0 = default (neither changes any result):
-   *   filter_chunk_rows  S3 processes the candidate edges in passes of this many rows (rounded up to 128); its two
-   *                      activation buffers hold rows x widest layer bf16 each.  Default 128 x SMs x 64 rows
-   *                      (1 212 416 on a B200: 2.5 GB per buffer, 5 launches per pass); smaller values trade a few
-   *                      per cent of throughput for memory (64 x 148 rows: 20 MB per buffer) -- DESIGN.md section 6.
+   *   filter_chunk_rows  the layer-by-layer S3 (used when the fused S3 kernel does not apply to the filter's shape, or with
+   *                      trk_set_option "filter_fused" = 0) processes the candidate edges in passes of this many rows
+   *                      (rounded up to 128); its two activation buffers hold rows x widest layer bf16 each.  Default:
+   *                      128 x SMs rows when the fused kernel applies (the chunked path is then only a test variant), else
+   *                      128 x SMs x 64 rows (1 212 416 on a B200: 2.5 GB per buffer) -- DESIGN.md section 6.
    *   grid_max           upper bound of the S2 search grid's cells per axis and event (1..128).  Default (and upper limit):
    *                      the largest value whose cell table (max_events x grid_max^3 x 16 radius buckets) fits 2^22 entries.  */
   int64_t filter_chunk_rows;
@@ -170,11 +171,13 @@ int64_t trk_last_launch_count(const trk_ctx* ctx);
  * waits for the last one and writes the HOST array ms[5] = {S1, S2, S3 (incl. compaction), S4, S5}. */
 trk_status trk_profile_enable(trk_ctx* ctx, int32_t on);
 trk_status trk_profile_stage_ms(trk_ctx* ctx, float* ms);
-/* Per-launch device time of the dominant kernel of the path, the hidden-layer GEMMs (K >= 256) of the S3 filter MLP
- * (DESIGN.md section 6), from CUDA-event pairs recorded around each such launch of the last profiled trk_infer.
- * Writes HOST ms[min(capacity, *n_launches)] in launch order: chunk 0 layer 2, chunk 0 layer 3, chunk 1 layer 2, ...;
- * chunk c covers candidate edges [c * *rows_per_launch, (c+1) * *rows_per_launch) clipped to counts[0], so launches of
- * chunks beyond the candidate count are empty.  Flops of a launch = 2 * rows * K * N with K = N = the hidden width. */
+/* Per-launch device time of the dominant kernel of the path, from CUDA-event pairs recorded around each
+ * such launch of the last profiled trk_infer.  With the fused S3 kernel (the default) there is ONE launch that runs every
+ * layer of the filter MLP over all counts[0] candidate edges and *rows_per_launch is -1.  With the layer-by-layer S3
+ * ("filter_fused" = 0) the launches are the hidden-layer GEMMs (K >= 256) in launch order: chunk 0 layer 2, chunk 0 layer 3,
+ * chunk 1 layer 2, ...; chunk c covers candidate edges [c * *rows_per_launch, (c+1) * *rows_per_launch) clipped to counts[0]
+ * (launches of chunks beyond the candidate count are empty) and a launch does 2 * rows * K * N flop with K = N = the hidden
+ * width.  Writes HOST ms[min(capacity, *n_launches)]. */
 trk_status trk_profile_kernel_ms(trk_ctx* ctx, float* ms, int32_t capacity, int32_t* n_launches, int64_t* rows_per_launch);
 
 /* Stage hooks: run ONE stage on caller-supplied DEVICE inputs (BASELINE.json north_star: "each
@@ -223,7 +226,10 @@ trk_status trk_gemm_bf16(const void* a, const void* w, const float* bias, void* 
  *   "gnn_fused"       1 (default): with gnn_hidden == 128 the S4 encoders, edge update, node update and decoder run as
  *                     fused two-layer CTA-pair kernels (gnn_fused.cuh); 0: layer-by-layer GEMM launches with the exact
  *                     split first layer.
- *   "epi_split"       1 (default): bf16-output layers with 256-column tiles and a single 64-wide K block (the first layer
+ *   "filter_fused"    1 (default): when the filter MLP is 2u -> W -> W -> W -> 1 with 2u <= 32 and W a multiple of 256 (<= 1024) S3
+ *                     runs as ONE persistent CTA-pair kernel with L2-resident activations (filter_fused.cuh); 0: layer by layer,
+ *                     one GEMM launch per layer over passes of trk_config.filter_chunk_rows edges.
+ *   "epi_split"       (layer-by-layer S3 only) 1 (default): bf16-output layers with 256-column tiles and a single 64-wide K block (the first layer
  *                     of the S3 filter MLP) run their epilogue on eight warps (two per TMEM lane quadrant); 2: in addition
  *                     that layer's input rows [e_src ; e_dst] are gathered inside the GEMM kernel instead of by a separate
  *                     launch (measured slower on the pileup-200 event, so not the default); 0: four warps.

@@ -285,7 +285,6 @@ trk_status trk_destroy(trk_ctx* ctx) {
   cudaFree(ctx->edge_dec_wab);
   cudaFree(ctx->edge_dec_wc);
   cudaFree(ctx->filter_w1_pad);
-  cudaFree(ctx->filter_w1_frag);
   cudaFree(ctx->node_enc_w1p);
   cudaFree(ctx->edge_enc_w1p);
   cudaFree(ctx->ws.base);
@@ -434,27 +433,11 @@ trk_status trk_create(const trk_config* cfg, trk_ctx** out) {
     for (int o = 0; o < w1; ++o)
       for (int i = 0; i < k1; ++i) p[(size_t)o * 64 + i] = f32_to_bf16_rne(cfg->filter.weight[0][(size_t)o * k1 + i]);
     if ((s = upload_bf16_block(ctx, p, &ctx->filter_w1_pad)) != TRK_OK) return bail(s);
-    // fused S3 kernel: applicable shape, and W1 in mma.sync.m16n8k16 B-fragment order (filter_fused.cuh)
+    // fused S3 kernel (filter_fused.cuh): applicable shape
     {
       const trk_mlp& m = cfg->filter;
       const int W = m.dims[1];
       ctx->filter_fusable = m.n_layers == 4 && k1 <= 32 && W % 256 == 0 && W <= 1024 && m.dims[2] == W && m.dims[3] == W;
-      if (ctx->filter_fusable) {
-        std::vector<uint32_t> f((size_t)(W / 8) * 32 * 4, 0);
-        auto wq = [&](int n, int k) -> uint32_t { return k < k1 ? f32_to_bf16_rne(m.weight[0][(size_t)n * k1 + k]) : 0u; };
-        for (int nt = 0; nt < W / 8; ++nt)
-          for (int lane = 0; lane < 32; ++lane) {
-            const int g = lane >> 2, t4 = lane & 3, n = nt * 8 + g;
-            for (int ks = 0; ks < 2; ++ks)
-              for (int hc = 0; hc < 2; ++hc) {
-                const int k = ks * 16 + hc * 8 + 2 * t4;
-                f[((size_t)nt * 32 + lane) * 4 + ks * 2 + hc] = wq(n, k) | (wq(n, k + 1) << 16);
-              }
-          }
-        if (cudaMalloc(&ctx->filter_w1_frag, f.size() * 4) != cudaSuccess ||
-            cudaMemcpy(ctx->filter_w1_frag, f.data(), f.size() * 4, cudaMemcpyHostToDevice) != cudaSuccess)
-          return bail(fail(ctx, TRK_ERR_OOM, "filter_w1_frag upload failed"));
-      }
     }
     // encoder first layers (K = 3 / 4) as a [H][64] bf16 K block: every weight column twice, once for the hi and once for the
     // lo half of its fp32 input feature (gnn_fused.cuh kEncode)

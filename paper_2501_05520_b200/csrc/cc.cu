@@ -12,13 +12,23 @@ __global__ void cc_init_kernel(int32_t* __restrict__ parent, int64_t n, int32_t*
   if (i == 0 && pass_count) *pass_count = 0;
 }
 
+// A parent pointer only ever changes to another ancestor of its node (path halving) or, at a root, to a smaller root (the
+// hook below), so a STALE value is still an ancestor: the walk may read through the SM's L1 (ld.global.ca, ~10x shorter
+// latency than the L2 round trip of a volatile load), it just may take a step more.  A stale "root" is caught by the hook:
+// atomicMin acts on the true value and the caller retries from what it returns.
+__device__ __forceinline__ int32_t load_parent(const int32_t* p) {
+  int32_t v;
+  asm volatile("ld.global.ca.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+
 __device__ __forceinline__ int32_t find_root(int32_t* parent, int32_t x) {
   // path halving with plain stores: every value ever stored is an ancestor of x (links are only ever added at roots and
   // point to smaller indices), hence valid whatever the interleaving; only the hook below needs an atomic
-  int32_t p = ((volatile int32_t*)parent)[x];
+  int32_t p = load_parent(parent + x);
   while (p != x) {
-    int32_t gp = ((volatile int32_t*)parent)[p];
-    if (gp != p) ((volatile int32_t*)parent)[x] = gp;
+    const int32_t gp = load_parent(parent + p);
+    if (gp != p) parent[x] = gp;
     x = p;
     p = gp;
   }

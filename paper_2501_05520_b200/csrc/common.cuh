@@ -86,9 +86,8 @@ struct trk_ctx {
   __nv_bfloat16* edge_dec_wab = nullptr;
   __nv_bfloat16* edge_dec_wc = nullptr;
   __nv_bfloat16* filter_w1_pad = nullptr;  // [1024][64] = W1 zero padded in K
-  // fused S3 kernel (filter_fused.cuh): layer-1 weights in mma.sync fragment order and the per-pair activation scratch
+  // fused S3 kernel (filter_fused.cuh): the per-pair activation scratch
   bool filter_fusable = false;             // filter = 2u -> W -> W -> W -> 1, 2u <= 32, W a multiple of 256, W <= 1024
-  uint4* filter_w1_frag = nullptr;         // [W/8][32] x {b0, b1 (k 0..15), b0, b1 (k 16..31)}
   __nv_bfloat16* filter_s1 = nullptr;      // [sm_count/2 * 256][W]  act1
   __nv_bfloat16* filter_s2 = nullptr;      // [sm_count/2 * 256][W]  act2
   // first layers of the S4 encoders for the tensor core (gnn_fused.cuh kEncode): [H][64], columns (2k, 2k+1) = w[:, k] twice

@@ -2,26 +2,27 @@
 // MLP = 2u -> W -> W -> W -> 1 with ReLU, W a multiple of 256 (1024 in BASELINE.json's pileup configs).
 //
 // A CTA pair owns 256-row blocks of candidate edges (row block rb = pair, pair + n_pairs, ...) and runs ALL layers of a row
-// block itself, so no activation of one pair is ever read by another and nothing needs a grid-wide synchronisation:
-//   layer 1 (K = 2u <= 32)  four "side" warps per CTA: the gathered, bf16-rounded rows [u_src ; u_dst] live in mma.sync
-//                           A fragments in registers, W1 streams from L2 in fragment order; bias + ReLU -> bf16 -> act1;
-//   layer 2 (K = W)         tcgen05.mma.cta_group::2, 256 x 256 tiles, A = act1 by TMA, epilogue bias + ReLU -> bf16 -> act2
-//                           by TMA store;
-//   layer 3 (K = W)         same MMAs with A = act2; the epilogue folds the final Linear(W -> 1) in: every thread keeps the
-//                           running dot of its row over the column tiles and writes sigmoid(dot + b) after the last one.
+// block itself, so no activation of one pair is ever read by another and nothing needs a grid-wide synchronisation.  Per row
+// block the tensor core walks 3 x W/256 tiles of 256 x 256 (tcgen05.mma.cta_group::2, accumulators double-buffered in TMEM):
+//   layer 1 (K = 2u <= 32)  A = the gathered rows [u_src ; u_dst] rounded to bf16, written by four gather warps straight into a
+//                           swizzled operand tile (one K block, only ceil(2u/16) K steps are issued); epilogue bias + ReLU ->
+//                           bf16 -> act1 by TMA store;
+//   layer 2 (K = W)         A = act1 by TMA; epilogue bias + ReLU -> bf16 -> act2 by TMA store;
+//   layer 3 (K = W)         A = act2; the epilogue folds the final Linear(W -> 1) in: every thread keeps the running dot of its row
+//                           over the column tiles and writes sigmoid(dot + b) after the last one.
 // act1 / act2 are per-pair scratch of 256 x W bf16 each in global memory (n_pairs x 2 x 512 KB = 74 MB for W = 1024 on 148
-// SMs): they are rewritten for every row block and stay in the 126 MB L2, so the only HBM traffic of the stage is the gather,
-// the indices and the scores -- against one HBM round trip of the 2 KB activation row per layer before.
+// SMs): they are rewritten for every row block and are always read back from the 126 MB L2, so the stage reads from HBM only
+// the gather, the indices and the weights once -- against one HBM round trip of the 2 KB activation row per layer before.
 //
-// Dependencies inside a pair (all mbarriers; the side warps and the TMA producer of a CTA only ever touch their own CTA's 128
-// rows of the scratch, so every one of them is CTA-local):
-//   act1_ready     side warps -> TMA producer: layer-1 rows of the NEXT row block are in global memory
-//   l2_done        MMA issuer (commit after the last layer-2 tile) -> side warps: act1 may be overwritten
-//   act2_ready[s]  epilogue warps (after their TMA stores of column slab s completed) -> TMA producer: layer 3 may load the
-//                  K blocks of slab s.  Layer 3's first K blocks come from the slabs stored first, so the tensor pipe does not
-//                  wait for the last layer-2 epilogue.
-// Writes by TMA store and reads by TMA load of the same CTA are ordered by cp.async.bulk.wait_group (completion, not .read);
-// the side warps' st.global are made visible to the TMA loads by fence.proxy.async + the mbarrier.
+// Dependencies inside a pair (mbarriers; a CTA's epilogue warps and TMA producer only ever touch their own CTA's 128 rows of the
+// scratch, so the slab barriers are CTA-local):
+//   xfull / xempty      gather warps <-> MMA issuer: the layer-1 operand tile of the next row block (single buffer: it is free
+//                       again as soon as the W/256 short layer-1 MMAs of the current row block have been issued and completed)
+//   act1_ready[s], act2_ready[s]   epilogue warps (after their TMA stores of column slab s have COMPLETED) -> TMA producer: the
+//                       next layer may load the K blocks of slab s.  A layer's first K blocks come from the slabs stored first,
+//                       so the tensor pipe does not wait for the last epilogue of the layer before.
+// Writes by TMA store and reads by TMA load of the same CTA are ordered by cp.async.bulk.wait_group (completion, not .read)
+// followed by the mbarrier.
 #pragma once
 
 #include "gemm_tc2.cuh"
@@ -31,26 +32,28 @@ namespace ff {
 
 using namespace tc;
 
-constexpr int kSideWarps = 4;
-constexpr int kThreadsFilter = kThreads + 32 * kSideWarps;   // 0 TMA, 1 MMA, 2-5 epilogue, 6-9 layer 1
+constexpr int kGatherWarpsF = 4;
+constexpr int kThreadsFilter = kThreads + 32 * kGatherWarpsF;   // 0 TMA, 1 MMA, 2-5 epilogue, 6-9 gather
 constexpr int kBN = 256;
-constexpr int kStages = num_stages_pair(kBN);
-constexpr int kStage = stage_bytes_pair(kBN);
-constexpr int kSmemFilter = kStages * kStage + kEpiWarps * kStoreStage + 1024 /*alignment*/ + 512 /*barriers*/;
-constexpr int kMaxSlabs = 4;                                  // W <= 1024
+constexpr int kStages = 5;
+constexpr int kStage = stage_bytes_pair(kBN);                  // A 16 KB + this CTA's half of W 16 KB
+constexpr int kXBytes = BM * BK * 2;                           // layer-1 operand tile of one CTA
+constexpr int kMaxSlabs = 4;                                   // W <= 1024
+constexpr int kMaxW = kMaxSlabs * kBN;
+constexpr int kVecBytes = 4 * kMaxW * 4;                       // b1, b2, b3, w4 in shared memory
+constexpr int kSmemFilter = kStages * kStage + kXBytes + kEpiWarps * kStoreStage + kVecBytes + 1024 /*alignment*/ + 512 /*barriers*/;
+static_assert(kSmemFilter <= 232448, "shared memory budget of one CTA");
 
 struct FilterParams {
   const float* feat;          // fp32 [n][u]: the embedding (or the raw hits)
   const int32_t* src;         // candidate edges
   const int32_t* dst;
   int u;                      // 2 u <= 32
-  const uint4* w1_frag;       // layer 1 weights in mma.sync B-fragment order: [W / 8][32 lanes] x {b0, b1 (k 0..15), b0, b1 (k 16..31)}
   const float* b1;            // [W]
   const float* b2;            // [W]
   const float* b3;            // [W]
   const float* w4;            // [W] final Linear(W -> 1)
   float b4;
-  __nv_bfloat16* act1;        // scratch [n_pairs * 256][W]
   float* score;               // [rows]
   int W;
 };
@@ -60,37 +63,56 @@ struct FilterBars {
   uint64_t empty[8];
   uint64_t tfull[2];
   uint64_t tempty[2];
-  uint64_t act1_ready;        // 4 arrivals (side warps)
-  uint64_t l2_done;           // multicast commit
-  uint64_t act2_ready[kMaxSlabs];   // 4 arrivals each (epilogue warps)
+  uint64_t xfull;                   // L  8 arrivals (4 gather warps x 2 CTAs)
+  uint64_t xempty;                  //    own, multicast commit
+  uint64_t act1_ready[kMaxSlabs];   //    own, 4 arrivals each (epilogue warps)
+  uint64_t act2_ready[kMaxSlabs];
   uint32_t tmem_slot;
 };
 static_assert(sizeof(FilterBars) <= 512, "barrier block");
-
-__device__ __forceinline__ void fence_proxy_async_global() { asm volatile("fence.proxy.async.global;" ::: "memory"); }
-
-__device__ __forceinline__ void mma_bf16_16816(float (&c)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1) {
-  asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0, %1, %2, %3}, {%4, %5, %6, %7}, {%8, %9}, {%0, %1, %2, %3};"
-               : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
-               : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
-}
 
 __device__ __forceinline__ uint32_t pack_relu_bf16x2(float lo, float hi) {
   uint32_t r;
   asm("cvt.rn.relu.bf16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
   return r;
 }
+// L2 eviction priority for the activation scratch: it is rewritten every row block and should not leave the L2 in between
+__device__ __forceinline__ uint64_t l2_policy_evict_last() {
+  uint64_t pol;
+  asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+  return pol;
+}
+__device__ __forceinline__ void tma_store_2d_hint(const CUtensorMap* tmap, const void* smem_src, int c0, int c1, uint64_t pol) {
+  asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group.L2::cache_hint [%0, {%2, %3}], [%1], %4;" ::"l"(
+                   reinterpret_cast<uint64_t>(tmap)),
+               "r"(smem_u32(smem_src)), "r"(c0), "r"(c1), "l"(pol)
+               : "memory");
+}
+__device__ __forceinline__ void tma_load_2d_pair_hint(void* smem_dst, const CUtensorMap* tmap, uint32_t bar_cluster_addr, int c0, int c1,
+                                                      uint64_t pol) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%3, %4}], [%2], %5;" ::"r"(
+          smem_u32(smem_dst)),
+      "l"(reinterpret_cast<uint64_t>(tmap)), "r"(bar_cluster_addr), "r"(c0), "r"(c1), "l"(pol)
+      : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_remote_cta(uint32_t cluster_addr) {
+  asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
+}
 
-// tmS1 / tmS2: the act1 / act2 scratch as A operands (box 64 x 128); tmW2 / tmW3: weights (box 64 x 128 = this CTA's half of a
-// 256-column tile); tmS2st: act2 for the TMA stores of the layer-2 epilogue (box 64 x 32).
+// tmS1 / tmS2: the act1 / act2 scratch as A operands (box 64 x 128); tmW1 (K padded to 64) / tmW2 / tmW3: weights (box 64 x 128 =
+// this CTA's half of a 256-column tile); tmS1st / tmS2st: the scratch for the TMA stores of the epilogues (box 64 x 32).
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsFilter, 1)
-filter_mlp_kernel(const __grid_constant__ CUtensorMap tmS1, const __grid_constant__ CUtensorMap tmS2, const __grid_constant__ CUtensorMap tmW2,
-                  const __grid_constant__ CUtensorMap tmW3, const __grid_constant__ CUtensorMap tmS2st, Rows rows, FilterParams p) {
+filter_mlp_kernel(const __grid_constant__ CUtensorMap tmS1, const __grid_constant__ CUtensorMap tmS2, const __grid_constant__ CUtensorMap tmW1,
+                  const __grid_constant__ CUtensorMap tmW2, const __grid_constant__ CUtensorMap tmW3, const __grid_constant__ CUtensorMap tmS1st,
+                  const __grid_constant__ CUtensorMap tmS2st, Rows rows, FilterParams p) {
   constexpr int A_BYTES = BM * BK * 2;
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
-  uint8_t* store_stage = smem + kStages * kStage;
-  FilterBars* bar = reinterpret_cast<FilterBars*>(store_stage + kEpiWarps * kStoreStage);
+  uint8_t* xbuf = smem + kStages * kStage;
+  uint8_t* store_stage = xbuf + kXBytes;
+  float* svec = reinterpret_cast<float*>(store_stage + kEpiWarps * kStoreStage);   // [4][kMaxW]: b1, b2, b3, w4
+  FilterBars* bar = reinterpret_cast<FilterBars*>(reinterpret_cast<uint8_t*>(svec) + kVecBytes);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const uint32_t rank = cluster_ctarank();
@@ -102,10 +124,12 @@ filter_mlp_kernel(const __grid_constant__ CUtensorMap tmS1, const __grid_constan
   const int n_tiles = p.W / kBN;          // column tiles (= slabs) per layer
   const int k_blocks = p.W / BK;
   const int kb_per_slab = kBN / BK;
-  const int scratch_row0 = pair * kPairBM + (int)rank * BM;   // this CTA's rows of the scratch
+  const int k1_steps = (2 * p.u + UMMA_K - 1) / UMMA_K;      // K steps of layer 1 that hold data
+  const int scratch_row0 = pair * kPairBM + (int)rank * BM;  // this CTA's rows of the scratch
 
   if (warp == 0 && lane == 0) {
-    prefetch_tmap(&tmS1); prefetch_tmap(&tmS2); prefetch_tmap(&tmW2); prefetch_tmap(&tmW3); prefetch_tmap(&tmS2st);
+    prefetch_tmap(&tmS1); prefetch_tmap(&tmS2); prefetch_tmap(&tmW1); prefetch_tmap(&tmW2); prefetch_tmap(&tmW3);
+    prefetch_tmap(&tmS1st); prefetch_tmap(&tmS2st);
     for (int s = 0; s < kStages; ++s) {
       mbar_init(&bar->full[s], 1);
       mbar_init(&bar->empty[s], 1);
@@ -114,12 +138,22 @@ filter_mlp_kernel(const __grid_constant__ CUtensorMap tmS1, const __grid_constan
       mbar_init(&bar->tfull[s], 1);
       mbar_init(&bar->tempty[s], 2 * kEpiWarps);
     }
-    mbar_init(&bar->act1_ready, kSideWarps);
-    mbar_init(&bar->l2_done, 1);
-    for (int s = 0; s < kMaxSlabs; ++s) mbar_init(&bar->act2_ready[s], kEpiWarps);
+    mbar_init(&bar->xfull, 2 * kGatherWarpsF);
+    mbar_init(&bar->xempty, 1);
+    for (int s = 0; s < kMaxSlabs; ++s) {
+      mbar_init(&bar->act1_ready[s], kEpiWarps);
+      mbar_init(&bar->act2_ready[s], kEpiWarps);
+    }
     fence_barrier_init();
   }
   if (warp == 1) tmem_alloc_pair<512>(&bar->tmem_slot);
+  for (int c = threadIdx.x; c < p.W; c += blockDim.x) {
+    svec[c] = p.b1[c];
+    svec[kMaxW + c] = p.b2[c];
+    svec[2 * kMaxW + c] = p.b3[c];
+    svec[3 * kMaxW + c] = p.w4[c];
+  }
+  __syncthreads();
   tc_fence_before();
   cluster_sync_all();
   tc_fence_after();
@@ -130,23 +164,32 @@ filter_mlp_kernel(const __grid_constant__ CUtensorMap tmS1, const __grid_constan
     if (lane == 0) {
       int stage = 0;
       uint32_t phase = 0;
+      const uint64_t keep = l2_policy_evict_last();
+      auto next_stage = [&]() { if (++stage == kStages) { stage = 0; phase ^= 1; } };
       for (int i = 0; i < n_rb; ++i) {
+        // layer 1: only this CTA's half of the W1 tile travels through the ring (the A operand is the gathered tile)
+        for (int nb = 0; nb < n_tiles; ++nb) {
+          mbar_wait(&bar->empty[stage], phase ^ 1);
+          if (leader) mbar_arrive_expect_tx(&bar->full[stage], 2 * (kStage - A_BYTES));
+          const uint32_t full_leader = mapa_u32(smem_u32(&bar->full[stage]), 0);
+          tma_load_2d_pair(smem + stage * kStage + A_BYTES, &tmW1, full_leader, 0, nb * kBN + (int)rank * (kBN / 2));
+          next_stage();
+        }
         for (int layer = 2; layer <= 3; ++layer) {
           const CUtensorMap* tmA = layer == 2 ? &tmS1 : &tmS2;
           const CUtensorMap* tmB = layer == 2 ? &tmW2 : &tmW3;
+          uint64_t* ready = layer == 2 ? bar->act1_ready : bar->act2_ready;
           for (int nb = 0; nb < n_tiles; ++nb) {
             for (int kb = 0; kb < k_blocks; ++kb) {
-              if (nb == 0) {   // the first column tile of a layer is the first reader of its operand
-                if (layer == 2 && kb == 0) mbar_wait(&bar->act1_ready, (uint32_t)(i & 1));
-                if (layer == 3 && kb % kb_per_slab == 0) mbar_wait(&bar->act2_ready[kb / kb_per_slab], (uint32_t)(i & 1));
-              }
+              // the first column tile of a layer is the first reader of its operand: slab by slab as the stores complete
+              if (nb == 0 && kb % kb_per_slab == 0) mbar_wait(&ready[kb / kb_per_slab], (uint32_t)(i & 1));
               mbar_wait(&bar->empty[stage], phase ^ 1);
               if (leader) mbar_arrive_expect_tx(&bar->full[stage], 2 * kStage);
               const uint32_t full_leader = mapa_u32(smem_u32(&bar->full[stage]), 0);
               uint8_t* sa = smem + stage * kStage;
-              tma_load_2d_pair(sa, tmA, full_leader, kb * BK, scratch_row0);
+              tma_load_2d_pair_hint(sa, tmA, full_leader, kb * BK, scratch_row0, keep);
               tma_load_2d_pair(sa + A_BYTES, tmB, full_leader, kb * BK, nb * kBN + (int)rank * (kBN / 2));
-              if (++stage == kStages) { stage = 0; phase ^= 1; }
+              next_stage();
             }
           }
         }
@@ -160,8 +203,26 @@ filter_mlp_kernel(const __grid_constant__ CUtensorMap tmS1, const __grid_constan
       uint32_t phase = 0;
       int as = 0;
       uint32_t aphase = 0;
+      auto next_stage = [&]() { if (++stage == kStages) { stage = 0; phase ^= 1; } };
+      auto next_acc = [&]() { if (++as == 2) { as = 0; aphase ^= 1; } };
+      const uint64_t xdesc = make_smem_desc(smem_u32(xbuf));
       for (int i = 0; i < n_rb; ++i) {
-        for (int t = 0; t < 2 * n_tiles; ++t) {
+        mbar_wait_cluster(&bar->xfull, (uint32_t)(i & 1));          // both CTAs' gathered rows are in shared memory
+        for (int nb = 0; nb < n_tiles; ++nb) {                      // layer 1: one short MMA group per column tile
+          mbar_wait_cluster(&bar->tempty[as], aphase ^ 1);
+          mbar_wait(&bar->full[stage], phase);
+          tc_fence_after();
+          const uint32_t d_tmem = tmem_base + (uint32_t)(as * kBN);
+          const uint64_t bdesc = make_smem_desc(smem_u32(smem + stage * kStage) + A_BYTES);
+          for (int k = 0; k < k1_steps; ++k)
+            tc_mma_bf16_pair(d_tmem, xdesc + (uint64_t)(k * 2), bdesc + (uint64_t)(k * 2), idesc, k != 0 ? 1u : 0u);
+          tc_commit_pair(&bar->empty[stage]);
+          tc_commit_pair(&bar->tfull[as]);
+          next_stage();
+          next_acc();
+        }
+        tc_commit_pair(&bar->xempty);                               // the gathered tile may be overwritten
+        for (int t = 0; t < 2 * n_tiles; ++t) {                     // layers 2 and 3
           mbar_wait_cluster(&bar->tempty[as], aphase ^ 1);
           tc_fence_after();
           const uint32_t d_tmem = tmem_base + (uint32_t)(as * kBN);
@@ -175,11 +236,10 @@ filter_mlp_kernel(const __grid_constant__ CUtensorMap tmS1, const __grid_constan
             for (int k = 0; k < BK / UMMA_K; ++k)
               tc_mma_bf16_pair(d_tmem, adesc + (uint64_t)(k * 2), bdesc + (uint64_t)(k * 2), idesc, (kb | k) != 0 ? 1u : 0u);
             tc_commit_pair(&bar->empty[stage]);
-            if (++stage == kStages) { stage = 0; phase ^= 1; }
+            next_stage();
           }
           tc_commit_pair(&bar->tfull[as]);
-          if (t == n_tiles - 1) tc_commit_pair(&bar->l2_done);   // every layer-2 MMA of this row block has read act1
-          if (++as == 2) { as = 0; aphase ^= 1; }
+          next_acc();
         }
       }
     }
@@ -189,22 +249,36 @@ filter_mlp_kernel(const __grid_constant__ CUtensorMap tmS1, const __grid_constan
     int as = 0;
     uint32_t aphase = 0;
     uint8_t* stage_buf = store_stage + (warp - 2) * kStoreStage;
-    uint32_t chunk = 0;
+    const uint64_t keep = l2_policy_evict_last();
     const uint32_t tempty_leader0 = mapa_u32(smem_u32(&bar->tempty[0]), 0);
     const uint32_t tempty_leader1 = mapa_u32(smem_u32(&bar->tempty[1]), 0);
+    // The TMA stores of a tile are only ASKED about at the start of the next tile's epilogue (a whole tile of MMAs later they
+    // have long completed), so the epilogue never sits in the store latency; the last tile of a layer asks at once, because the
+    // next epilogue cannot start before the next layer has consumed that very slab.
+    uint64_t* pending = nullptr;
     for (int i = 0; i < n_rb; ++i) {
       const int64_t rb = pair + (int64_t)i * n_pairs;
       const int64_t row = rb * kPairBM + (int64_t)rank * BM + quad * 32 + lane;
       float dot = 0.f;
-      for (int t = 0; t < 2 * n_tiles; ++t) {
-        const int layer = t < n_tiles ? 2 : 3;
-        const int nb = t < n_tiles ? t : t - n_tiles;
+      for (int t = 0; t < 3 * n_tiles; ++t) {
+        const int layer = 1 + t / n_tiles;
+        const int nb = t % n_tiles;
         mbar_wait(&bar->tfull[as], aphase);
         tc_fence_after();
+        if (pending) {
+          if (lane == 0) {
+            bulk_wait_all();
+            mbar_arrive(pending);
+          }
+          pending = nullptr;
+        }
         const uint32_t taddr = tmem_base + ((uint32_t)(quad * 32) << 16) + (uint32_t)(as * kBN);
         const uint32_t rel = as == 0 ? tempty_leader0 : tempty_leader1;
-        if (layer == 2) {
-          // bias + ReLU -> bf16 -> act2 (this warp's 32 rows x 256 columns, 64 columns per TMA store box)
+        if (layer < 3) {
+          // bias + ReLU -> bf16 -> act1 / act2 (this warp's 32 rows x 256 columns, 64 columns per TMA store box)
+          const float* bias = svec + (layer == 1 ? 0 : kMaxW) + nb * kBN;
+          const CUtensorMap* tmC = layer == 1 ? &tmS1st : &tmS2st;
+          uint32_t chunk = 0;
 #pragma unroll 1
           for (int c = 0; c < kBN; c += 64) {
             uint32_t ra[32], rb2[32];
@@ -215,19 +289,22 @@ filter_mlp_kernel(const __grid_constant__ CUtensorMap tmS1, const __grid_constan
               if (lane == 0) bulk_wait_read<1>();
               __syncwarp();
             }
+            const float4* b4 = reinterpret_cast<const float4*>(bias + c);
+            float4 bb[16];
+#pragma unroll
+            for (int j = 0; j < 16; ++j) bb[j] = b4[j];
             tmem_ld_wait();
             if (c + 64 >= kBN) {
               tc_fence_before();
               __syncwarp();
               if (lane == 0) mbar_arrive_cluster(rel);
             }
-            const float4* b4 = reinterpret_cast<const float4*>(p.b2 + nb * kBN + c);
 #pragma unroll
             for (int q = 0; q < 8; ++q) {
               uint32_t w[4];
 #pragma unroll
               for (int h = 0; h < 2; ++h) {
-                const float4 b = __ldg(b4 + q * 2 + h);
+                const float4 b = bb[q * 2 + h];
                 const uint32_t* r = (q < 4 ? ra : rb2) + (q & 3) * 8 + h * 4;
                 w[h * 2 + 0] = pack_relu_bf16x2(__uint_as_float(r[0]) + b.x, __uint_as_float(r[1]) + b.y);
                 w[h * 2 + 1] = pack_relu_bf16x2(__uint_as_float(r[2]) + b.z, __uint_as_float(r[3]) + b.w);
@@ -237,39 +314,45 @@ filter_mlp_kernel(const __grid_constant__ CUtensorMap tmS1, const __grid_constan
             fence_proxy_async();
             __syncwarp();
             if (lane == 0) {
-              tma_store_2d(&tmS2st, buf, nb * kBN + c, scratch_row0 + quad * 32);
+              tma_store_2d_hint(tmC, buf, nb * kBN + c, scratch_row0 + quad * 32, keep);
               bulk_commit();
             }
             ++chunk;
           }
-          // slab nb of act2 is complete for this warp's rows once its stores have landed
-          if (lane == 0) {
-            bulk_wait_all();
-            mbar_arrive(&bar->act2_ready[nb]);
+          // slab nb is complete for this warp's rows once its stores have landed
+          uint64_t* ready = layer == 1 ? &bar->act1_ready[nb] : &bar->act2_ready[nb];
+          if (nb == n_tiles - 1) {
+            if (lane == 0) {
+              bulk_wait_all();
+              mbar_arrive(ready);
+            }
+          } else {
+            pending = ready;
           }
           __syncwarp();
-          chunk = 0;   // nothing of this warp is in flight any more
         } else {
           // ReLU(acc + b3) . w4 over this tile's columns, accumulated over the column tiles in the thread's register
 #pragma unroll 1
           for (int c = 0; c < kBN; c += 32) {
             uint32_t r[32];
             tmem_ld32(taddr + c, r);
+            const float4* b4 = reinterpret_cast<const float4*>(svec + 2 * kMaxW + nb * kBN + c);
+            const float4* w4 = reinterpret_cast<const float4*>(svec + 3 * kMaxW + nb * kBN + c);
+            float4 bb[8], ww[8];
+#pragma unroll
+            for (int q = 0; q < 8; ++q) { bb[q] = b4[q]; ww[q] = w4[q]; }
             tmem_ld_wait();
             if (c + 32 >= kBN) {
               tc_fence_before();
               __syncwarp();
               if (lane == 0) mbar_arrive_cluster(rel);
             }
-            const float4* b4 = reinterpret_cast<const float4*>(p.b3 + nb * kBN + c);
-            const float4* w4 = reinterpret_cast<const float4*>(p.w4 + nb * kBN + c);
 #pragma unroll
             for (int q = 0; q < 8; ++q) {
-              const float4 b = __ldg(b4 + q), w = __ldg(w4 + q);
-              dot = fmaf(fmaxf(__uint_as_float(r[q * 4 + 0]) + b.x, 0.f), w.x, dot);
-              dot = fmaf(fmaxf(__uint_as_float(r[q * 4 + 1]) + b.y, 0.f), w.y, dot);
-              dot = fmaf(fmaxf(__uint_as_float(r[q * 4 + 2]) + b.z, 0.f), w.z, dot);
-              dot = fmaf(fmaxf(__uint_as_float(r[q * 4 + 3]) + b.w, 0.f), w.w, dot);
+              dot = fmaf(fmaxf(__uint_as_float(r[q * 4 + 0]) + bb[q].x, 0.f), ww[q].x, dot);
+              dot = fmaf(fmaxf(__uint_as_float(r[q * 4 + 1]) + bb[q].y, 0.f), ww[q].y, dot);
+              dot = fmaf(fmaxf(__uint_as_float(r[q * 4 + 2]) + bb[q].z, 0.f), ww[q].z, dot);
+              dot = fmaf(fmaxf(__uint_as_float(r[q * 4 + 3]) + bb[q].w, 0.f), ww[q].w, dot);
             }
           }
           if (nb == n_tiles - 1 && row < M) p.score[rows.m_off + row] = fast_sigmoid(dot + p.b4);
@@ -278,60 +361,40 @@ filter_mlp_kernel(const __grid_constant__ CUtensorMap tmS1, const __grid_constan
       }
     }
   } else {
-    // ---------------------------------------------------------------- layer 1 on mma.sync: 32 rows per warp
-    const int sw = warp - (2 + kEpiWarps);
-    const int g = lane >> 2, t4 = lane & 3;
+    // ---------------------------------------------------------------- gather: one operand row per thread
+    const int r = (warp - (2 + kEpiWarps)) * 32 + lane;
     const int u = p.u;
-    __nv_bfloat16* out0 = p.act1 + (int64_t)(scratch_row0 + sw * 32) * p.W;
-    const int n8_tiles = p.W / 8;
+    const uint32_t xfull_leader = mapa_u32(smem_u32(&bar->xfull), 0);
+    uint8_t* rowp = xbuf + r * 128;
     for (int i = 0; i < n_rb; ++i) {
       const int64_t rb = pair + (int64_t)i * n_pairs;
-      const int64_t row0 = rb * kPairBM + (int64_t)rank * BM + sw * 32;
-      // A fragments: rows {g, g+8} of the two 16-row tiles, K = 32 columns = [u_src ; u_dst ; 0]
-      uint32_t a[2][2][4];
+      const int64_t row = rb * kPairBM + (int64_t)rank * BM + r;
+      float v[32];
 #pragma unroll
-      for (int mt = 0; mt < 2; ++mt) {
+      for (int c = 0; c < 32; ++c) v[c] = 0.f;
+      if (row < M) {
+        const int64_t si = p.src[rows.m_off + row], di = p.dst[rows.m_off + row];
+        const float* fs = p.feat + si * u;
+        const float* fd = p.feat + di * u;
 #pragma unroll
-        for (int hr = 0; hr < 2; ++hr) {
-          const int64_t row = row0 + mt * 16 + hr * 8 + g;
-          int64_t si = 0, di = 0;
-          const bool ok = row < M;
-          if (ok) { si = p.src[rows.m_off + row]; di = p.dst[rows.m_off + row]; }
+        for (int c = 0; c < 16; ++c)
+          if (c < u) v[c] = __ldg(fs + c);
 #pragma unroll
-          for (int ks = 0; ks < 2; ++ks) {
-#pragma unroll
-            for (int hc = 0; hc < 2; ++hc) {
-              const int c = ks * 16 + hc * 8 + 2 * t4;      // even column; (c, c+1) never straddles u when u is even
-              float v0 = 0.f, v1 = 0.f;
-              if (ok) {
-                if (c < u) v0 = __ldg(p.feat + si * u + c); else if (c < 2 * u) v0 = __ldg(p.feat + di * u + (c - u));
-                if (c + 1 < u) v1 = __ldg(p.feat + si * u + c + 1); else if (c + 1 < 2 * u) v1 = __ldg(p.feat + di * u + (c + 1 - u));
-              }
-              a[mt][ks][hc * 2 + hr] = pack_bf16(v0, v1);
-            }
-          }
-        }
+        for (int c = 0; c < 32; ++c)
+          if (c >= u && c < 2 * u) v[c] = __ldg(fd + (c - u));
       }
-      // act1 of the previous row block must have been read by all of its layer-2 MMAs
-      if (i > 0) mbar_wait(&bar->l2_done, (uint32_t)((i - 1) & 1));
-#pragma unroll 2
-      for (int nt = 0; nt < n8_tiles; ++nt) {
-        const uint4 b = __ldg(p.w1_frag + (int64_t)nt * 32 + lane);
-        const float2 bias = __ldg(reinterpret_cast<const float2*>(p.b1 + nt * 8 + 2 * t4));
+      uint32_t pk[16];
 #pragma unroll
-        for (int mt = 0; mt < 2; ++mt) {
-          float c[4] = {bias.x, bias.y, bias.x, bias.y};
-          mma_bf16_16816(c, a[mt][0], b.x, b.y);
-          mma_bf16_16816(c, a[mt][1], b.z, b.w);
-          __nv_bfloat16* o = out0 + (int64_t)(mt * 16 + g) * p.W + nt * 8 + 2 * t4;
-          *reinterpret_cast<uint32_t*>(o) = pack_relu_bf16x2(c[0], c[1]);
-          *reinterpret_cast<uint32_t*>(o + (int64_t)8 * p.W) = pack_relu_bf16x2(c[2], c[3]);
-        }
+      for (int c = 0; c < 16; ++c) pk[c] = pack_bf16(v[2 * c], v[2 * c + 1]);
+      if (i > 0) mbar_wait(&bar->xempty, (uint32_t)((i - 1) & 1));   // the layer-1 MMAs of the previous row block have read the tile
+#pragma unroll
+      for (int q = 0; q < 8; ++q) {
+        const uint4 val = q < 4 ? make_uint4(pk[q * 4], pk[q * 4 + 1], pk[q * 4 + 2], pk[q * 4 + 3]) : make_uint4(0u, 0u, 0u, 0u);
+        *reinterpret_cast<uint4*>(rowp + ((q ^ (r & 7)) << 4)) = val;
       }
-      __threadfence();
-      fence_proxy_async_global();
+      fence_proxy_async();
       __syncwarp();
-      if (lane == 0) mbar_arrive(&bar->act1_ready);
+      if (lane == 0) mbar_arrive_remote_cta(xfull_leader);
     }
   }
   if (warp >= 2 && warp < 2 + kEpiWarps && lane == 0) bulk_wait_all();

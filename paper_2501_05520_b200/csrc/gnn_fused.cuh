@@ -109,6 +109,7 @@ __device__ __forceinline__ uint32_t pack_relu_bf16(float lo, float hi) {
 }
 
 constexpr int kFusedThreads = 22 * 32;
+constexpr unsigned kPollSleepNs = 32;           // back-off of the polling TMA / MMA warps when none of their barriers is ready
 constexpr int kOffW1 = 0;                       // 6 K blocks of this CTA's 64 output rows of W1
 constexpr int kOffW2 = kOffW1 + 6 * kWKB;       // 2 K blocks of W2
 constexpr int kOffRing = kOffW2 + 2 * kWKB;     // 4 K blocks: h_src (2), h_dst (2)
@@ -263,9 +264,11 @@ gnn_fused_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constant
       const int res_end = kResidual ? n_my : 0;
       const int g_end = MODE == kNode ? n_my : 0;
       while (n_op < op_end || n_res < res_end || n_g[0] < g_end || n_g[1] < g_end) {
+        bool progressed = false;
 #pragma unroll
         for (int h = 0; h < 2; ++h) {              // kNode: m_in | m_out blocks into the ring halves
           if (n_g[h] < g_end && mbar_test(&bar->gempty[h], (uint32_t)(n_g[h] & 1) ^ 1)) {
+            progressed = true;
             if (leader) mbar_arrive_expect_tx(&bar->gfull[h], 2 * 2 * kKB);
             for (int kb = 0; kb < 2; ++kb)
               tma_load_2d_pair(smem + kOffRing + (h * 2 + kb) * kKB, &tmE, gfull_leader[h], kH + h * kH + kb * 64, row0_of(n_g[h]));
@@ -273,6 +276,7 @@ gnn_fused_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constant
           }
         }
         if (n_op < op_end && mbar_test(&bar->eopempty, (uint32_t)(n_op & 1) ^ 1)) {
+          progressed = true;
           if (leader) mbar_arrive_expect_tx(&bar->eopfull, 2 * 2 * kKB);
           for (int kb = 0; kb < 2; ++kb) tma_load_2d_pair(smem + kOffEOp + kb * kKB, &tmE, eopfull_leader, colE + kb * 64, row0_of(n_op));
           prefetch(n_op + 3);
@@ -280,10 +284,12 @@ gnn_fused_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constant
         }
         // the residual copy of tile t is asked for only after its operand copy, so it finds the rows in L2
         if (n_res < res_end && n_res < n_op && mbar_test(&bar->resempty, (uint32_t)(n_res & 1) ^ 1)) {
+          progressed = true;
           mbar_arrive_expect_tx(&bar->resfull, 2 * kKB);
           for (int kb = 0; kb < 2; ++kb) tma_load_2d(smem + kOffRes + kb * kKB, &tmE, &bar->resfull, colE + kb * 64, row0_of(n_res));
           ++n_res;
         }
+        if (!progressed) __nanosleep(kPollSleepNs);   // nothing was ready: leave the issue slots to the epilogue warps of this scheduler
       }
     }
   } else if (warp == 1) {
@@ -300,11 +306,13 @@ gnn_fused_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constant
       int stage1 = 0;          // 0: waiting for the accumulator and h_src, 1: for h_dst, 2: for the e operand tile
       const int n2_end = kTwoLayers ? n_my : 0;
       while (n1 < n_my || n2 < n2_end) {
+        bool progressed = false;
         if (n2 < n2_end && n2 < n1) {
           const int b = n2 & 1;
           const uint32_t ph = (n2 >> 1) & 1;
           if (mbar_test(&bar->tfull, (uint32_t)(n2 & 1)) && mbar_test(&bar->a2empty[b], ph ^ 1)) {
             tc_fence_after();
+            progressed = true;
             const uint32_t d = tmem_base + (uint32_t)(2 * kH + b * kH);
             for (int kb = 0; kb < 2; ++kb) kblock(d, sbase + kOffT + kb * kKB, sbase + kOffW2 + kb * kWKB, kb == 0);
             tc_commit_pair(&bar->tempty);
@@ -319,6 +327,7 @@ gnn_fused_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constant
           if (stage1 == 0) {
             if (mbar_test(&bar->a1empty[b], ph ^ 1) && mbar_test(&bar->gfull[0], (uint32_t)(n1 & 1))) {
               tc_fence_after();
+              progressed = true;
               if constexpr (MODE == kEncode) {
                 // one K step: the 16 columns that hold the hi / lo feature pairs
                 tc_mma_bf16_pair(d, make_smem_desc(sbase + kOffRing), make_smem_desc(sbase + kOffW1), idesc, 0u);
@@ -335,6 +344,7 @@ gnn_fused_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constant
           if (stage1 == 1) {
             if (mbar_test(&bar->gfull[1], (uint32_t)(n1 & 1))) {
               tc_fence_after();
+              progressed = true;
               for (int kb = 0; kb < 2; ++kb) kblock(d, sbase + kOffRing + (2 + kb) * kKB, sbase + kOffW1 + (kbR + 2 + kb) * kWKB, false);
               tc_commit_pair(&bar->gempty[1]);
               stage1 = 2;
@@ -343,6 +353,7 @@ gnn_fused_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constant
           if (stage1 == 2) {
             if (mbar_test(&bar->eopfull, (uint32_t)(n1 & 1))) {
               tc_fence_after();
+              progressed = true;
               for (int kb = 0; kb < 2; ++kb) kblock(d, sbase + kOffEOp + kb * kKB, sbase + kOffW1 + (kbE + kb) * kWKB, false);
               tc_commit_pair(&bar->eopempty);
               tc_commit_pair(&bar->a1full[b]);
@@ -351,6 +362,7 @@ gnn_fused_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constant
             }
           }
         }
+        if (!progressed) __nanosleep(kPollSleepNs);
       }
     }
   } else if (warp < 6) {

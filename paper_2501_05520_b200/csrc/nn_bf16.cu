@@ -419,14 +419,15 @@ static trk_status filter_forward_fused(trk_ctx* ctx, const float* feat, const in
   const int64_t s_rows = (int64_t)n_pairs_max * 256;
   auto kern = ff::filter_mlp_kernel;
   TRK_TRY(ensure_smem(ctx, kern, ff::kSmemFilter));
-  CUtensorMap ts1, ts2, tw2, tw3, ts2st;
+  CUtensorMap ts1, ts2, tw1, tw2, tw3, ts1st, ts2st;
   TRK_TRY(make_tmap(ctx, &ts1, ctx->filter_s1, s_rows, W, W, 128));
   TRK_TRY(make_tmap(ctx, &ts2, ctx->filter_s2, s_rows, W, W, 128));
+  TRK_TRY(make_tmap(ctx, &tw1, ctx->filter_w1_pad, W, 64, 64, 128));
   TRK_TRY(make_tmap(ctx, &tw2, L[1].w_bf16, W, W, W, 128));
   TRK_TRY(make_tmap(ctx, &tw3, L[2].w_bf16, W, W, W, 128));
+  TRK_TRY(make_tmap(ctx, &ts1st, ctx->filter_s1, s_rows, W, W, 32));
   TRK_TRY(make_tmap(ctx, &ts2st, ctx->filter_s2, s_rows, W, W, 32));
-  ff::FilterParams p{feat, src, dst, ctx->filter_u, ctx->filter_w1_frag, L[0].b_f32, L[1].b_f32, L[2].b_f32, L[3].w_f32,
-                     ctx->filter_b_last, ctx->filter_s1, score, W};
+  ff::FilterParams p{feat, src, dst, ctx->filter_u, L[0].b_f32, L[1].b_f32, L[2].b_f32, L[3].w_f32, ctx->filter_b_last, score, W};
   const tc::Rows rows{n_edges_dev, 0, n_edges_cap};
   const unsigned grid = 2u * (unsigned)std::min<int64_t>(ceil_div(n_edges_cap, 256), n_pairs_max);
   // trk_profile_kernel_ms: one CUDA-event pair around the launch
@@ -435,7 +436,7 @@ static trk_status filter_forward_fused(trk_ctx* ctx, const float* feat, const in
     ctx->kprof_n = 1;
     TRK_CUDA(ctx, cudaEventRecord(ctx->kprof_ev[0], st));
   }
-  TRK_LAUNCH(ctx, kern, grid, ff::kThreadsFilter, ff::kSmemFilter, st, ts1, ts2, tw2, tw3, ts2st, rows, p);
+  TRK_LAUNCH(ctx, kern, grid, ff::kThreadsFilter, ff::kSmemFilter, st, ts1, ts2, tw1, tw2, tw3, ts1st, ts2st, rows, p);
   if (kprof) TRK_CUDA(ctx, cudaEventRecord(ctx->kprof_ev[1], st));
   return TRK_OK;
 }

@@ -144,19 +144,25 @@ def test_s4_kernel_variants_agree_with_the_oracle(variant):
 
 
 def test_s3_first_layer_variants_are_bit_identical():
-    """trk_set_option 'epi_split': four or eight epilogue warps, gather inside the GEMM or before it -- the same arithmetic."""
+    """trk_set_option 'filter_fused' / 'epi_split': the fused S3 kernel against the layer-by-layer path, and the latter's variants
+    (four or eight epilogue warps, gather inside the GEMM or before it -- the same arithmetic)."""
     import torch
     run = G.oracle_run("pileup50", "bf16", True, 600)
     o = run["out"]
     trk = G.make_trk(run)
     try:
         feat, src, dst = _dev(o["emb"]), _dev(o["cand_src"]), _dev(o["cand_dst"])
+        fused = trk.stage_filter(feat, src, dst).clone()            # default: all layers in one persistent kernel
+        trk.set_option("filter_fused", 0)                           # layer by layer, chunked
         scores = []
         for v in (0, 1, 2):
             trk.set_option("epi_split", v)
             scores.append(trk.stage_filter(feat, src, dst).clone())
         torch.cuda.synchronize()
         assert torch.equal(scores[0], scores[1]) and torch.equal(scores[1], scores[2])
-        G.check_scores(scores[1].cpu().numpy(), o["filter_score"], "bf16", "filter score")
+        G.check_scores(scores[1].cpu().numpy(), o["filter_score"], "bf16", "filter score (layer by layer)")
+        G.check_scores(fused.cpu().numpy(), o["filter_score"], "bf16", "filter score (fused kernel)")
+        # the two implementations round the same quantities at the same places (bf16 activations, fp32 accumulation)
+        assert float((fused - scores[1]).abs().max()) < 2e-3
     finally:
         trk.close()
