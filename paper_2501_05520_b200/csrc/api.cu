@@ -79,6 +79,7 @@ trk_status upload_mlp(trk_ctx* ctx, const trk_mlp& m, DevMlp* out, bool bf16) {
     std::vector<float> b(L.out_pad, 0.f);
     std::memcpy(b.data(), m.bias[l], (size_t)L.out * 4);
     TRK_CUDA(ctx, cudaMemcpy(L.b_f32, b.data(), (size_t)L.out_pad * 4, cudaMemcpyHostToDevice));
+    L.b_host = b;
     if (bf16) {
       std::vector<uint16_t> w((size_t)L.in_pad * L.out_pad, 0);
       for (int o = 0; o < L.out; ++o)
@@ -136,7 +137,7 @@ void carve(trk_ctx* c, Carver& k) {
     c->filter_chunk = std::min<int64_t>(chunk, ((int64_t)EC + 127) / 128 * 128);
   }
   c->act_rows = (int64_t)std::max<size_t>(N, (size_t)c->filter_chunk);
-  char* p;
+  char* p = nullptr;
   k.take(&c->ev_of_hit, N);
   k.take(&c->emb, N * c->d_e);
   k.take(&p, (size_t)c->act_rows * maxw * es); c->act0 = p;

@@ -27,6 +27,7 @@ struct DevLinear {
   int in = 0, out = 0;
   float* w_f32 = nullptr;           // [out][in]
   float* b_f32 = nullptr;           // [out]
+  std::vector<float> b_host;        // the same on the host, zero padded to out_pad (small layers pass it as a kernel parameter)
   __nv_bfloat16* w_bf16 = nullptr;  // [out_pad][in_pad] K-major, zero padded (bf16 mode only)
   int in_pad = 0, out_pad = 0;
 };

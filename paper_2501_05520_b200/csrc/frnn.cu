@@ -275,8 +275,9 @@ frnn_search_kernel(const float* __restrict__ semb, const float4* __restrict__ sm
   for (int t = lane; t < CAP; t += 32) { bd2[t] = kInfBits; bidx[t] = 0x7fffffff; }
   __syncwarp();
 
-  // makes room for 32 more entries (count <= CAP - 32 afterwards, every entry that can still be among the K nearest kept)
-  auto prune = [&]() {
+  // keeps the entries with d2 <= T for a threshold T with K <= #{d2 <= T} <= max_keep (every entry that can still be among the K
+  // nearest stays); max_keep = CAP - 32 makes room for 32 more entries, max_keep = K is the final selection of the K nearest
+  auto prune = [&](int max_keep) {
     unsigned long long mine[PER];
 #pragma unroll
     for (int i = 0; i < PER; ++i) mine[i] = bd2[lane + 32 * i];          // unused slots hold +inf
@@ -291,7 +292,7 @@ frnn_search_kernel(const float* __restrict__ semb, const float4* __restrict__ sm
     double lo = 0.0, hi = __longlong_as_double((long long)mx);
     int cnt_hi = count;
     bool found = false;
-    for (int it = 0; it < 24 && !found; ++it) {
+    for (int it = 0; it < 48 && !found; ++it) {
       const double mid = 0.5 * (lo + hi);
       const unsigned long long mb = (unsigned long long)__double_as_longlong(mid);
       int c = 0;
@@ -303,7 +304,7 @@ frnn_search_kernel(const float* __restrict__ semb, const float4* __restrict__ sm
       } else {
         hi = mid;
         cnt_hi = c;
-        found = c <= CAP - 32;
+        found = c <= max_keep;
       }
     }
     if (found) {
@@ -372,7 +373,7 @@ frnn_search_kernel(const float* __restrict__ semb, const float4* __restrict__ sm
     const unsigned m = __ballot_sync(0xffffffffu, ok);
     if (m) {
       if (count + 32 > CAP) {
-        prune();
+        prune(CAP - 32);
         ok = ok && d2 <= r2;                 // the threshold may just have moved
       }
       const unsigned m2 = __ballot_sync(0xffffffffu, ok);
@@ -463,12 +464,7 @@ frnn_search_kernel(const float* __restrict__ semb, const float4* __restrict__ sm
   }
   while (qn0 > 0) drain0();
   while (qn > 0) drain();
-  if (count > K) {
-    warp_bitonic(bd2, bidx, CAP, false, lane);
-    for (int t = K + lane; t < CAP; t += 32) { bd2[t] = kInfBits; bidx[t] = 0x7fffffff; }
-    __syncwarp();
-    count = K;
-  }
+  if (count > K) prune(K);       // exactly the K nearest: a threshold between the K-th and the (K+1)-th d2, the sort only on ties
   // order the kept neighbours by index: the indices are distinct, so the rank of one is the number of smaller ones
   for (int t = lane; t < count; t += 32) {
     const int mine = bidx[t];

@@ -51,8 +51,10 @@ struct FusedParams {
   int64_t ldx;
   const int32_t* src;
   const int32_t* dst;
-  const float* b1;
-  const float* b2;
+  // the two bias vectors travel BY VALUE: kernel parameters live in the constant bank, so the epilogues read them with LDC
+  // (warp-uniform addresses) instead of competing with the tiles for the shared-memory / L1 data pipe
+  float b1[kH];
+  float b2[kH];
   int use_ln;
   const float* w_out;         // kDecode
   float b_out;
@@ -100,6 +102,14 @@ __device__ __forceinline__ void tma_prefetch_l2_2d(const CUtensorMap* tmap, int 
 }
 
 __device__ __forceinline__ float2 f2(float a, float b) { return make_float2(a, b); }
+
+// TMA store that ADDS the shared-memory box to the tensor in global memory (element type of the tensor map: bf16)
+__device__ __forceinline__ void tma_reduce_add_2d(const CUtensorMap* tmap, const void* smem_src, int c0, int c1) {
+  asm volatile("cp.reduce.async.bulk.tensor.2d.global.shared::cta.add.tile.bulk_group [%0, {%2, %3}], [%1];" ::"l"(
+                   reinterpret_cast<uint64_t>(tmap)),
+               "r"(smem_u32(smem_src)), "r"(c0), "r"(c1)
+               : "memory");
+}
 
 // bf16x2(max(lo, 0), max(hi, 0)) in one instruction: the ReLU rides on the conversion (lo in the low half, hi in the high half)
 __device__ __forceinline__ uint32_t pack_relu_bf16(float lo, float hi) {
@@ -187,13 +197,14 @@ __device__ __forceinline__ void ln_coeffs(float ps, float pq, float2 other, int 
 template <int MODE>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kFusedThreads, 1)
 gnn_fused_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constant__ CUtensorMap tmW2,
-                       const __grid_constant__ CUtensorMap tmE, const __grid_constant__ CUtensorMap tmEst, Rows rows, FusedParams p) {
+                       const __grid_constant__ CUtensorMap tmE, const __grid_constant__ CUtensorMap tmEst, Rows rows,
+                       const __grid_constant__ FusedParams p) {
   extern __shared__ __align__(1024) uint8_t smem[];
   if ((smem_u32(smem) & 1023u) != 0) __trap();   // the swizzled operand layout needs the 1024-byte alignment declared above
   Bars* bar = reinterpret_cast<Bars*>(smem + kOffBar);
-  float* sb1 = reinterpret_cast<float*>(smem + kOffVec);
-  float* sb2 = sb1 + kH;
-  float* swo = sb2 + kH;
+  const float* sb1 = p.b1;
+  const float* sb2 = p.b2;
+  float* swo = reinterpret_cast<float*>(smem + kOffVec) + 2 * kH;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const uint32_t rank = cluster_ctarank();
   const bool leader = rank == 0;
@@ -202,7 +213,11 @@ gnn_fused_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constant
   const int64_t total = (M + 2 * kTileRows - 1) / (2 * kTileRows);
   const int n_my = total > pair ? (int)((total - pair + n_pairs - 1) / n_pairs) : 0;
   constexpr bool kTwoLayers = MODE != kDecode;
-  constexpr bool kResidual = MODE == kUpdate || MODE == kNode;     // epilogue 2 adds (and TMA loads) the residual tile
+  // the residual: epilogue 2 stages only the UPDATE (bf16) and the TMA adds it to the rows in global memory
+  // (cp.reduce.async.bulk.tensor .add on bf16: e <- bf16(e + update), one rounding), so the residual tile is never loaded into
+  // shared memory again -- a quarter of the kernel's shared-memory traffic in the version that added it in registers
+  constexpr bool kAddStore = MODE == kUpdate || MODE == kNode;
+  constexpr bool kResidual = false;
   constexpr int kW1Blocks = MODE == kEncode ? 1 : 6;               // K blocks of W1 resident in shared memory
   // K blocks of W1 that go with the operand tile (e, or h in kNode) and with the two ring halves
   constexpr int kbE = MODE == kNode ? 0 : 4;
@@ -235,8 +250,6 @@ gnn_fused_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constant
   if (warp == 1) tmem_alloc_pair<512>(&bar->tmem_slot);
   if (threadIdx.x >= 128 && threadIdx.x < 128 + kH) {
     const int c = threadIdx.x - 128;
-    sb1[c] = p.b1[c];
-    sb2[c] = kTwoLayers ? p.b2[c] : 0.f;
     swo[c] = MODE == kDecode ? p.w_out[c] : 0.f;
   }
   __syncthreads();
@@ -562,7 +575,8 @@ gnn_fused_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constant
         __syncwarp();
         if (lane == 0) {
           const int row0 = (int)(tile * 2 * kTileRows + rank * kTileRows + quad * 32);
-          tma_store_2d(&tmEst, res + quad * 32 * 128, colE + half * 64, row0);
+          if (kAddStore) tma_reduce_add_2d(&tmEst, res + quad * 32 * 128, colE + half * 64, row0);
+          else tma_store_2d(&tmEst, res + quad * 32 * 128, colE + half * 64, row0);
           bulk_commit();
           bulk_wait_read<0>();  // the rows have left shared memory: the buffer may be refilled
           if (kResidual) mbar_arrive(&bar->resempty);

@@ -158,6 +158,14 @@ trk_status gemm_row_ln(trk_ctx* ctx, const bf16* A, int64_t a_rows, int64_t lda,
   return launch_gemm<64, tc::EpiRowLn>(ctx, A, a_rows, lda, K, W, 64, rows, ep, st);
 }
 
+// bias vectors of the two layers into the by-value kernel parameter block (layer 2 is absent in the decoder: zeros)
+static void fill_bias(gf::FusedParams& p, const DevLinear& L1, const DevLinear& L2) {
+  for (int c = 0; c < gf::kH; ++c) {
+    p.b1[c] = c < (int)L1.b_host.size() ? L1.b_host[c] : 0.f;
+    p.b2[c] = c < (int)L2.b_host.size() ? L2.b_host[c] : 0.f;
+  }
+}
+
 // Fused edge update / decoder of S4 (gnn_fused.cuh), H = 128: E <- E + LNR(W2 LNR(W1 [h_s ; h_d ; e] + b1) + b2) in place,
 // or score = sigmoid(w_out . LNR(W1 [h_s ; h_d ; e] + b1) + b_out).
 template <int MODE>
@@ -172,7 +180,8 @@ trk_status launch_edge_fused(trk_ctx* ctx, const bf16* X, int64_t ldx, bf16* E, 
   TRK_TRY(make_tmap(ctx, &tw2, L2.w_bf16, gf::kH, gf::kH, gf::kH, 64));
   TRK_TRY(make_tmap(ctx, &te, E, e_rows, gf::kH, gf::kH, 128));
   TRK_TRY(make_tmap(ctx, &test, E, e_rows, gf::kH, gf::kH, 32));
-  gf::FusedParams p{X, ldx, src, dst, L1.b_f32, L2.b_f32, ctx->cfg.gnn_layernorm, w_out, b_out, score, nullptr};
+  gf::FusedParams p{X, ldx, src, dst, {}, {}, ctx->cfg.gnn_layernorm, w_out, b_out, score, nullptr};
+  fill_bias(p, L1, L2);
   const int64_t ptiles = ceil_div(rows.m_cap, 2 * gf::kTileRows);
   const unsigned grid = 2u * (unsigned)std::min<int64_t>(ptiles, ctx->sm_count / 2);
   TRK_LAUNCH(ctx, kern, grid, gf::kFusedThreads, gf::kSmemFused, st, tw1, tw2, te, test, rows, p);
@@ -190,7 +199,8 @@ trk_status launch_node_fused(trk_ctx* ctx, bf16* X, int64_t x_rows, const DevLin
   TRK_TRY(make_tmap(ctx, &tw2, L2.w_bf16, gf::kH, gf::kH, gf::kH, 64));
   TRK_TRY(make_tmap(ctx, &tx, X, x_rows, 3 * gf::kH, 3 * gf::kH, 128));
   TRK_TRY(make_tmap(ctx, &txst, X, x_rows, gf::kH, 3 * gf::kH, 32));
-  gf::FusedParams p{X, 3 * gf::kH, nullptr, nullptr, L1.b_f32, L2.b_f32, ctx->cfg.gnn_layernorm, nullptr, 0.f, nullptr, nullptr};
+  gf::FusedParams p{X, 3 * gf::kH, nullptr, nullptr, {}, {}, ctx->cfg.gnn_layernorm, nullptr, 0.f, nullptr, nullptr};
+  fill_bias(p, L1, L2);
   const int64_t ptiles = ceil_div(rows.m_cap, 2 * gf::kTileRows);
   const unsigned grid = 2u * (unsigned)std::min<int64_t>(ptiles, ctx->sm_count / 2);
   TRK_LAUNCH(ctx, kern, grid, gf::kFusedThreads, gf::kSmemFused, st, tw1, tw2, tx, txst, rows, p);
@@ -208,7 +218,8 @@ trk_status launch_encoder_fused(trk_ctx* ctx, const float* hits, const int32_t* 
   TRK_TRY(make_tmap(ctx, &tw1, w1p, gf::kH, 64, 64, 64));
   TRK_TRY(make_tmap(ctx, &tw2, L2.w_bf16, gf::kH, gf::kH, gf::kH, 64));
   TRK_TRY(make_tmap(ctx, &tout, out, out_rows, gf::kH, ldo, 32));
-  gf::FusedParams p{nullptr, 0, src, dst, L1.b_f32, L2.b_f32, ctx->cfg.gnn_layernorm, nullptr, 0.f, nullptr, hits};
+  gf::FusedParams p{nullptr, 0, src, dst, {}, {}, ctx->cfg.gnn_layernorm, nullptr, 0.f, nullptr, hits};
+  fill_bias(p, L1, L2);
   const int64_t ptiles = ceil_div(rows.m_cap, 2 * gf::kTileRows);
   const unsigned grid = 2u * (unsigned)std::min<int64_t>(ptiles, ctx->sm_count / 2);
   TRK_LAUNCH(ctx, kern, grid, gf::kFusedThreads, gf::kSmemFused, st, tw1, tw2, tout, tout, rows, p);

@@ -138,6 +138,72 @@ def test_frnn_degenerate_caps_and_radii(k, radius):
         trk.close()
 
 
+@pytest.mark.parametrize("scale", [1.0, 1.0e3, 1.0e-3])
+def test_frnn_projection_slack_scales_with_the_data(scale):
+    """The fp32 projection P^T e used for binning and for the level-0 pre-filter is inexact; its slack must scale with |e|
+    (it is taken from max|e| on the device).  An embedding offset far from the origin and scaled by 1e3 / 1e-3, searched with a
+    rotated (non-axis-aligned) orthonormal grid_proj, must still give the oracle's brute-force edge list bit for bit."""
+    run = G.oracle_run("pileup50", "bf16", True, 300)
+    cfg, calib, ev = run["cfg"], run["calib"], run["ev"]
+    hits = ev["hits"]
+    n = len(hits)
+    off = ev["event_offsets"]
+    emb = ((run["out"]["emb"].astype(np.float64) + 37.0) * scale).astype(np.float32)   # |e| ~ 40 scale, neighbours ~0.3 scale apart
+    r = np.float32(calib["frnn_radius"] * scale)
+    d_e = emb.shape[1]
+    rng = np.random.default_rng(5)
+    q, _ = np.linalg.qr(rng.standard_normal((d_e, d_e)))
+    proj = q[:, :3].astype(np.float32)
+    osrc, odst, orow = s2_frnn.frnn_brute(emb, hits, off, r, cfg["frnn_k"])
+    assert len(osrc) > 2 * n                                   # a real graph, with the cap biting somewhere
+    from paper_2501_05520_b200 import Trk
+    trk = Trk(model=run["model"], precision="bf16", frnn_radius=float(r), frnn_k=cfg["frnn_k"], filter_input=cfg["filter_input"],
+              filter_cut=calib["filter_cut"], gnn_hidden=cfg["gnn_hidden"], gnn_iters=cfg["gnn_iters"], gnn_cut=cfg["gnn_cut"],
+              max_hits=n, grid_proj=proj)
+    try:
+        src, dst, rowptr, cnt = trk.stage_frnn(_dev(emb), _dev(hits), off)
+        ec = int(cnt[0])
+        assert int(cnt[1]) == 0 and ec == len(osrc), (ec, len(osrc))
+        assert np.array_equal(src[:ec].cpu().numpy(), osrc) and np.array_equal(dst[:ec].cpu().numpy(), odst)
+        assert np.array_equal(rowptr.cpu().numpy(), orow)
+    finally:
+        trk.close()
+
+
+@pytest.mark.parametrize("width,input_kind", [(256, "raw"), (512, "emb"), (768, "raw")])
+def test_fused_filter_kernel_other_shapes(width, input_kind):
+    """The fused S3 kernel (filter_fused.cuh) on shapes other than 24 -> 1024^3 -> 1: 1, 2 and 3 column tiles per layer, an odd
+    endpoint width (u = 3 raw features, so an operand pair straddles the src | dst boundary) and u = 8 latent features, on a
+    ragged number of edges; every score against the oracle, and against the layer-by-layer path."""
+    import torch
+    from oracle import s3_filter
+    cfg, calib, _ = _toy("bf16")
+    cfg = dict(cfg, filter_input=input_kind)
+    u = 3 if input_kind == "raw" else cfg["embed_dims"][-1]
+    cfg["filter_dims"] = [2 * u, width, width, width, 1]
+    model = G.make_model(cfg)
+    ev = generate_event(120, 0.1, 11)
+    hits = ev["hits"]
+    n = len(hits)
+    rng = np.random.default_rng(1)
+    e = 5 * 256 + 77                                            # several row blocks and a ragged tail
+    src = rng.integers(0, n, e).astype(np.int32)
+    dst = rng.integers(0, n, e).astype(np.int32)
+    feat = hits if input_kind == "raw" else rng.standard_normal((n, u)).astype(np.float32)
+    ref = s3_filter.filter_scores(feat, src, dst, model["filter"]).astype(np.float32)
+    trk = _make(cfg, calib, model, n, max_cand_edges=e)
+    try:
+        fused = trk.stage_filter(_dev(feat), _dev(src), _dev(dst)).clone()
+        trk.set_option("filter_fused", 0)
+        layered = trk.stage_filter(_dev(feat), _dev(src), _dev(dst)).clone()
+        torch.cuda.synchronize()
+        G.check_scores(fused.cpu().numpy(), ref, "bf16", f"fused filter score (W = {width}, {input_kind})")
+        G.check_scores(layered.cpu().numpy(), ref, "bf16", "layer-by-layer filter score")
+        assert float((fused - layered).abs().max()) < 2e-3
+    finally:
+        trk.close()
+
+
 def test_capacity_overflow_is_flagged_and_deterministic():
     import torch
     run = G.oracle_run("toy", "fp32")
