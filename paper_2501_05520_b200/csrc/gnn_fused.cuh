@@ -118,6 +118,32 @@ __device__ __forceinline__ uint32_t pack_relu_bf16(float lo, float hi) {
   return r;
 }
 
+// 32 registers of this thread -> 32 consecutive TMEM columns of its lane
+__device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&r)[32]) {
+  asm volatile(
+      "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], "
+      "{%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, "
+      "%17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31, %32};" ::"r"(taddr),
+      "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]), "r"(r[9]), "r"(r[10]),
+      "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]), "r"(r[16]), "r"(r[17]), "r"(r[18]), "r"(r[19]), "r"(r[20]),
+      "r"(r[21]), "r"(r[22]), "r"(r[23]), "r"(r[24]), "r"(r[25]), "r"(r[26]), "r"(r[27]), "r"(r[28]), "r"(r[29]), "r"(r[30]),
+      "r"(r[31])
+      : "memory");
+}
+__device__ __forceinline__ void tmem_st_wait() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+// D[tmem] (+)= A[tmem] * B[smem desc]^T: the A operand (128 rows per CTA = TMEM lanes, K-major, two bf16 per 32-bit column)
+// is read from tensor memory, so a layer's output can feed the next layer without a trip through shared memory
+__device__ __forceinline__ void tc_mma_bf16_pair_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t idesc, uint32_t accumulate) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "setp.ne.b32 p, %4, 0;\n"
+      "tcgen05.mma.cta_group::2.kind::f16 [%0], [%1], %2, %3, p;\n"
+      "}\n" ::"r"(d_tmem),
+      "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate)
+      : "memory");
+}
+
 constexpr int kFusedThreads = 22 * 32;
 constexpr unsigned kPollSleepNs = 32;           // back-off of the polling TMA / MMA warps when none of their barriers is ready
 constexpr int kOffW1 = 0;                       // 6 K blocks of this CTA's 64 output rows of W1
@@ -125,8 +151,8 @@ constexpr int kOffW2 = kOffW1 + 6 * kWKB;       // 2 K blocks of W2
 constexpr int kOffRing = kOffW2 + 2 * kWKB;     // 4 K blocks: h_src (2), h_dst (2)
 constexpr int kOffEOp = kOffRing + 4 * kKB;     // 2 K blocks: the e tile as layer-1 operand
 constexpr int kOffRes = kOffEOp + 2 * kKB;      // 2 K blocks: the e tile as residual, overwritten in place and stored
-constexpr int kOffT = kOffRes + 2 * kKB;        // 2 K blocks: layer-1 output
-constexpr int kOffVec = kOffT + 2 * kKB;        // b1, b2, w_out: 3 x 128 fp32
+constexpr int kOffXD = kOffRes + 2 * kKB;       // kDecode: partial dots of the upper half rows, 128 fp32
+constexpr int kOffVec = kOffXD + kTileRows * 4; // b1, b2, w_out: 3 x 128 fp32
 constexpr int kOffX1 = kOffVec + 3 * kH * 4;     // epilogue 1: one float2 per row, half-row statistics one way, coefficients back
 constexpr int kOffBar = kOffX1 + kTileRows * 8;
 constexpr int kSmemFused = kOffBar + 256;
@@ -141,9 +167,8 @@ struct Bars {
   uint64_t gfull[2];      // L  8 arrivals (4 gather warps x 2 CTAs), halves: h_src, h_dst (kNode: 1, tx)
   uint64_t gempty[2];     //    own, multicast commit
   uint64_t a1full[2];     //    own, multicast commit
-  uint64_t a1empty[2];    // L  16 arrivals
-  uint64_t tfull;         // L  16 arrivals
-  uint64_t tempty;        //    own, multicast commit
+  uint64_t a1empty[2];    // L  two layers: multicast commit of MMA 2 (T lives in the accumulator's columns); kDecode: 16 arrivals
+  uint64_t tfull[2];      // L  16 arrivals: T of the tile in acc1[b] is in tensor memory
   uint64_t a2full[2];     //    own, multicast commit
   uint64_t a2empty[2];    // L  16 arrivals
   uint32_t tmem_slot;
@@ -235,12 +260,11 @@ gnn_fused_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constant
       mbar_init(&bar->gfull[i], MODE == kNode ? 1 : 8);
       mbar_init(&bar->gempty[i], 1);
       mbar_init(&bar->a1full[i], 1);
-      mbar_init(&bar->a1empty[i], 16);
+      mbar_init(&bar->a1empty[i], kTwoLayers ? 1 : 16);
+      mbar_init(&bar->tfull[i], 16);
       mbar_init(&bar->a2full[i], 1);
       mbar_init(&bar->a2empty[i], 16);
     }
-    mbar_init(&bar->tfull, 16);
-    mbar_init(&bar->tempty, 1);
     fence_barrier_init();
     // this CTA's halves of the weights: output rows [64 rank, 64 rank + 64)
     mbar_arrive_expect_tx(&bar->w_full, (kW1Blocks + 2) * kWKB);
@@ -323,12 +347,17 @@ gnn_fused_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constant
         if (n2 < n2_end && n2 < n1) {
           const int b = n2 & 1;
           const uint32_t ph = (n2 >> 1) & 1;
-          if (mbar_test(&bar->tfull, (uint32_t)(n2 & 1)) && mbar_test(&bar->a2empty[b], ph ^ 1)) {
+          if (mbar_test(&bar->tfull[b], ph) && mbar_test(&bar->a2empty[b], ph ^ 1)) {
             tc_fence_after();
             progressed = true;
             const uint32_t d = tmem_base + (uint32_t)(2 * kH + b * kH);
-            for (int kb = 0; kb < 2; ++kb) kblock(d, sbase + kOffT + kb * kKB, sbase + kOffW2 + kb * kWKB, kb == 0);
-            tc_commit_pair(&bar->tempty);
+            const uint32_t t = tmem_base + (uint32_t)(b * kH);     // T: bf16 pairs in the first 64 columns of acc1[b]
+#pragma unroll
+            for (int k = 0; k < kH / UMMA_K; ++k) {
+              const uint64_t bdesc = make_smem_desc(sbase + kOffW2 + (k / 4) * kWKB) + (uint64_t)((k % 4) * 2);
+              tc_mma_bf16_pair_ts(d, t + (uint32_t)(k * (UMMA_K / 2)), bdesc, idesc, k != 0 ? 1u : 0u);
+            }
+            tc_commit_pair(&bar->a1empty[b]);     // acc1[b] (and the T in it) may be overwritten by layer 1 of tile n2 + 2
             tc_commit_pair(&bar->a2full[b]);
             ++n2;
           }
@@ -452,9 +481,9 @@ gnn_fused_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constant
     const int r = quad * 32 + lane;   // row of this thread inside the CTA's 128-row tile == TMEM lane
     const int bid = 1 + quad;         // named barrier of the two warps that share this quadrant's rows
     const uint32_t a1empty0 = mapa_u32(smem_u32(&bar->a1empty[0]), 0), a1empty1 = mapa_u32(smem_u32(&bar->a1empty[1]), 0);
-    const uint32_t tfull_l = mapa_u32(smem_u32(&bar->tfull), 0);
+    const uint32_t tfull0 = mapa_u32(smem_u32(&bar->tfull[0]), 0), tfull1 = mapa_u32(smem_u32(&bar->tfull[1]), 0);
     float2* slot = reinterpret_cast<float2*>(smem + kOffX1) + r;
-    float* xd = reinterpret_cast<float*>(smem + kOffT + kKB + quad * 32 * 128);   // kDecode only (T is unused there)
+    float* xd = reinterpret_cast<float*>(smem + kOffXD) + quad * 32;               // kDecode only
     for (int tl = 0; tl < n_my; ++tl) {
       const int64_t tile = pair + (int64_t)tl * n_pairs;
       const int b = tl & 1;
@@ -465,8 +494,10 @@ gnn_fused_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constant
       float ps, pq;
       load_half<false>(tmem_base + ((uint32_t)(quad * 32) << 16) + (uint32_t)(b * kH + half * 64), sb1 + half * 64, x, ps, pq);
       tc_fence_before();
-      __syncwarp();
-      if (lane == 0) mbar_arrive_remote(b == 0 ? a1empty0 : a1empty1);     // the accumulator is in registers now
+      if (!kTwoLayers) {
+        __syncwarp();
+        if (lane == 0) mbar_arrive_remote(b == 0 ? a1empty0 : a1empty1);   // the accumulator is in registers now
+      }
       // upper half -> lower half: (sum, sum of squares); lower half -> upper half: (rstd, -mean rstd)
       float2 rs, sh;
       if (half == 1) *slot = f2(ps, pq);
@@ -501,21 +532,21 @@ gnn_fused_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constant
         }
         named_bar_sync(bid, 64);          // the partial dot has been read: the slot may be rewritten for the next tile
       } else {
-        mbar_wait(&bar->tempty, (uint32_t)(tl & 1) ^ 1);   // the layer-2 MMA of the previous tile has read T
+        // T = bf16(LNR(.)) goes back into tensor memory, over the accumulator it came from: row = lane, K index k in the
+        // low / high half of column k / 2, which is the layout tcgen05.mma reads an A operand from.  Both halves of the row
+        // were loaded before the first named barrier above, so the columns are free.  acc1 is double buffered, hence so is T.
+        tc_fence_after();
+        uint32_t w[32];
 #pragma unroll
-        for (int c = 0; c < 64; c += 8) {                  // 8 columns = one 16-byte chunk of the swizzled K block `half`
-          uint32_t w[4];
-#pragma unroll
-          for (int i = 0; i < 4; ++i) {
-            const float2 v = __ffma2_rn(x[c / 2 + i], rs, sh);
-            w[i] = pack_relu_bf16(v.x, v.y);
-          }
-          const int ch = c >> 3;
-          *reinterpret_cast<uint4*>(smem + kOffT + half * kKB + r * 128 + ((ch ^ (r & 7)) << 4)) = make_uint4(w[0], w[1], w[2], w[3]);
+        for (int i = 0; i < 32; ++i) {
+          const float2 v = __ffma2_rn(x[i], rs, sh);
+          w[i] = pack_relu_bf16(v.x, v.y);
         }
-        fence_proxy_async();
+        tmem_st32(tmem_base + ((uint32_t)(quad * 32) << 16) + (uint32_t)(b * kH + half * 32), w);
+        tmem_st_wait();
+        tc_fence_before();
         __syncwarp();
-        if (lane == 0) mbar_arrive_remote(tfull_l);
+        if (lane == 0) mbar_arrive_remote(b == 0 ? tfull0 : tfull1);
       }
     }
   } else {
