@@ -17,17 +17,18 @@
 //   * the 3H-wide first-layer operand is assembled in shared memory as six K blocks: the e rows by TMA, the h rows of the
 //     edge's endpoints by cp.async gathers (256-byte rows) straight into the 128-byte-swizzled UMMA layout; kNode loads
 //     all six K blocks of X = (h | m_in | m_out) by TMA;
-//   * layer-1 accumulator (TMEM) -> LayerNorm + ReLU in registers -> bf16 tile T in shared memory -> layer-2 MMA ->
-//     LayerNorm + ReLU + residual -> TMA store.  The e tile is held twice with separate lifetimes: as the layer-1 operand
-//     (freed as soon as MMA 1 has read it) and as the residual / output staging of epilogue 2 (a second TMA load that hits L2).
+//   * layer-1 accumulator (TMEM) -> LayerNorm + ReLU in registers -> bf16 tile T written back to tensor memory over the
+//     accumulator it came from (tcgen05.st) -> layer-2 MMA with its A operand in TMEM -> LayerNorm + ReLU -> bf16 update
+//     staged in shared memory -> TMA reduce-add store (the residual add happens in global memory).
 // Both LayerNorm epilogues run on EIGHT warps, two per TMEM lane quadrant, each taking one 64-column K block of the row:
 //   * a thread reads 64 accumulator columns, adds the bias, forms the partial (sum, sum of squares) of its half row and
 //     exchanges it with the thread that holds the other half through shared memory (named barriers of 64 threads);
 //     variance = E[x^2] - mean^2 in fp32 (the values are LayerNorm-scale, no cancellation problem);
 //   * epilogue 1 exchanges through one float2 per row (statistics one way, coefficients back); epilogue 2 exchanges inside
-//     the first 16-byte cell of its row of the residual tile (the cell's residual values wait in registers).
+//     the first 16-byte cell of its row of the staging tile.
 // 22 warps: 0 TMA, 1 MMA issuer (leader CTA) + TMEM owner, 2-5 gather, 6-13 epilogue 1, 14-21 epilogue 2.
-// TMEM: acc1[2] (columns 0, 128) and acc2[2] (256, 384), so two tiles are in flight.
+// TMEM: acc1[2] (columns 0, 128; T takes the first 64 columns of its accumulator once that is in registers) and acc2[2]
+// (256, 384), so two tiles are in flight.
 // mbarriers marked L are used in the leader CTA's copy only (both CTAs arrive on it).
 #pragma once
 
@@ -150,7 +151,7 @@ constexpr int kOffW1 = 0;                       // 6 K blocks of this CTA's 64 o
 constexpr int kOffW2 = kOffW1 + 6 * kWKB;       // 2 K blocks of W2
 constexpr int kOffRing = kOffW2 + 2 * kWKB;     // 4 K blocks: h_src (2), h_dst (2)
 constexpr int kOffEOp = kOffRing + 4 * kKB;     // 2 K blocks: the e tile as layer-1 operand
-constexpr int kOffRes = kOffEOp + 2 * kKB;      // 2 K blocks: the e tile as residual, overwritten in place and stored
+constexpr int kOffRes = kOffEOp + 2 * kKB;      // 2 K blocks: staging of the bf16 update for the TMA (reduce-add) store
 constexpr int kOffXD = kOffRes + 2 * kKB;       // kDecode: partial dots of the upper half rows, 128 fp32
 constexpr int kOffVec = kOffXD + kTileRows * 4; // b1, b2, w_out: 3 x 128 fp32
 constexpr int kOffX1 = kOffVec + 3 * kH * 4;     // epilogue 1: one float2 per row, half-row statistics one way, coefficients back
@@ -162,8 +163,6 @@ struct Bars {
   uint64_t w_full;
   uint64_t eopfull;       // L  tx: both CTAs' operand tiles
   uint64_t eopempty;      //    own, multicast commit (MMA 1 has read the operand tile)
-  uint64_t resfull;       //    own, tx: this CTA's residual tile
-  uint64_t resempty;      //    own, 8 arrivals (epilogue-2 warps, after their rows have left shared memory)
   uint64_t gfull[2];      // L  8 arrivals (4 gather warps x 2 CTAs), halves: h_src, h_dst (kNode: 1, tx)
   uint64_t gempty[2];     //    own, multicast commit
   uint64_t a1full[2];     //    own, multicast commit
@@ -242,7 +241,6 @@ gnn_fused_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constant
   // (cp.reduce.async.bulk.tensor .add on bf16: e <- bf16(e + update), one rounding), so the residual tile is never loaded into
   // shared memory again -- a quarter of the kernel's shared-memory traffic in the version that added it in registers
   constexpr bool kAddStore = MODE == kUpdate || MODE == kNode;
-  constexpr bool kResidual = false;
   constexpr int kW1Blocks = MODE == kEncode ? 1 : 6;               // K blocks of W1 resident in shared memory
   // K blocks of W1 that go with the operand tile (e, or h in kNode) and with the two ring halves
   constexpr int kbE = MODE == kNode ? 0 : 4;
@@ -254,8 +252,6 @@ gnn_fused_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constant
     mbar_init(&bar->w_full, 1);
     mbar_init(&bar->eopfull, 1);
     mbar_init(&bar->eopempty, 1);
-    mbar_init(&bar->resfull, 1);
-    mbar_init(&bar->resempty, 8);
     for (int i = 0; i < 2; ++i) {
       mbar_init(&bar->gfull[i], MODE == kNode ? 1 : 8);
       mbar_init(&bar->gempty[i], 1);
@@ -296,11 +292,10 @@ gnn_fused_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constant
       prefetch(2);
       const uint32_t eopfull_leader = mapa_u32(smem_u32(&bar->eopfull), 0);
       const uint32_t gfull_leader[2] = {mapa_u32(smem_u32(&bar->gfull[0]), 0), mapa_u32(smem_u32(&bar->gfull[1]), 0)};
-      int n_op = 0, n_res = 0, n_g[2] = {0, 0};
+      int n_op = 0, n_g[2] = {0, 0};
       const int op_end = MODE == kEncode ? 0 : n_my;
-      const int res_end = kResidual ? n_my : 0;
       const int g_end = MODE == kNode ? n_my : 0;
-      while (n_op < op_end || n_res < res_end || n_g[0] < g_end || n_g[1] < g_end) {
+      while (n_op < op_end || n_g[0] < g_end || n_g[1] < g_end) {
         bool progressed = false;
 #pragma unroll
         for (int h = 0; h < 2; ++h) {              // kNode: m_in | m_out blocks into the ring halves
@@ -318,13 +313,6 @@ gnn_fused_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constant
           for (int kb = 0; kb < 2; ++kb) tma_load_2d_pair(smem + kOffEOp + kb * kKB, &tmE, eopfull_leader, colE + kb * 64, row0_of(n_op));
           prefetch(n_op + 3);
           ++n_op;
-        }
-        // the residual copy of tile t is asked for only after its operand copy, so it finds the rows in L2
-        if (n_res < res_end && n_res < n_op && mbar_test(&bar->resempty, (uint32_t)(n_res & 1) ^ 1)) {
-          progressed = true;
-          mbar_arrive_expect_tx(&bar->resfull, 2 * kKB);
-          for (int kb = 0; kb < 2; ++kb) tma_load_2d(smem + kOffRes + kb * kKB, &tmE, &bar->resfull, colE + kb * 64, row0_of(n_res));
-          ++n_res;
         }
         if (!progressed) __nanosleep(kPollSleepNs);   // nothing was ready: leave the issue slots to the epilogue warps of this scheduler
       }
@@ -569,10 +557,8 @@ gnn_fused_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constant
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive_remote(b == 0 ? a2empty0 : a2empty1);
-        if (kResidual) mbar_wait(&bar->resfull, (uint32_t)(tl & 1));        // the residual copy of this tile has landed
-        // exchange of the half-row statistics through the first cell of this thread's residual row (its values wait in e0)
+        // exchange of the half-row statistics through the first cell of this thread's row of the staging tile
         uint4* cell0 = reinterpret_cast<uint4*>(res + r * 128 + ((0 ^ (r & 7)) << 4));
-        const uint4 e0 = kResidual ? *cell0 : make_uint4(0u, 0u, 0u, 0u);
         *reinterpret_cast<float2*>(cell0) = f2(ps, pq);
         named_bar_sync(bid, 64);
         const float2 other = *reinterpret_cast<const float2*>(smem + kOffRes + (half ^ 1) * kKB + r * 128 + ((0 ^ (r & 7)) << 4));
@@ -583,22 +569,14 @@ gnn_fused_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constant
         for (int c = 0; c < 64; c += 8) {
           const int ch = c >> 3;
           uint4* cell = reinterpret_cast<uint4*>(res + r * 128 + ((ch ^ (r & 7)) << 4));
-          const uint4 e = (c == 0 || !kResidual) ? e0 : *cell;
-          const __nv_bfloat162* e2 = reinterpret_cast<const __nv_bfloat162*>(&e);
           uint32_t w[4];
 #pragma unroll
           for (int i = 0; i < 4; ++i) {
-            // LNR(.) is rounded to bf16 (ReLU inside the conversion) and the residual is added in bf16x2 arithmetic: the sum of two
-            // bf16 values rounded once.  Against adding in fp32 this is one more rounding of the UPDATE (|LNR| <= ~11, ulp 2^-9
-            // relative), far below the rounding of the residual stream itself (|e| grows to ~20) that both forms share.
+            // LNR(.) is rounded to bf16 (ReLU inside the conversion); the TMA store adds it to the row in global memory in bf16
+            // arithmetic: the sum of two bf16 values rounded once.  Against adding in fp32 this is one more rounding of the
+            // UPDATE (|LNR| <= ~11, ulp 2^-9 relative), far below the rounding of the residual stream itself (|e| grows to ~20).
             const float2 v = __ffma2_rn(x[c / 2 + i], rs, sh);
-            const uint32_t u = pack_relu_bf16(v.x, v.y);
-            if (kResidual) {
-              const __nv_bfloat162 t = __hadd2(*reinterpret_cast<const __nv_bfloat162*>(&u), e2[i]);
-              w[i] = *reinterpret_cast<const uint32_t*>(&t);
-            } else {
-              w[i] = u;
-            }
+            w[i] = pack_relu_bf16(v.x, v.y);
           }
           *cell = make_uint4(w[0], w[1], w[2], w[3]);
         }
@@ -610,9 +588,8 @@ gnn_fused_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constant
           else tma_store_2d(&tmEst, res + quad * 32 * 128, colE + half * 64, row0);
           bulk_commit();
           bulk_wait_read<0>();  // the rows have left shared memory: the buffer may be refilled
-          if (kResidual) mbar_arrive(&bar->resempty);
         }
-        if (!kResidual) __syncwarp();   // no residual load orders the next tile's writes after the store's read-out: the warp does
+        __syncwarp();           // orders the next tile's writes of the staging rows after the store's read-out
       }
       if (lane == 0) bulk_wait_all();
     }

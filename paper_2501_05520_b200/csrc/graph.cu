@@ -161,56 +161,6 @@ segment_sum_kernel(const T* __restrict__ E, int H, const int32_t* __restrict__ i
   }
 }
 
-
-// bf16, H = 128 (the pileup configs): a half warp per row (16 lanes x 16 B = one 256-byte row), so one load instruction
-// fetches two rows and eight rows are in flight per warp; the in-edge row indices of up to 32 entries come with one
-// coalesced load and travel by shuffle.  Rows 0, 2, 4, ... of a segment accumulate in the lower half warp, rows 1, 3, 5, ...
-// in the upper one, each in segment order; the two partial sums are added at the end: a fixed order (reading C-14).
-__global__ void __launch_bounds__(256)
-segment_sum_h128_kernel(const __nv_bfloat16* __restrict__ E, const int32_t* __restrict__ in_rowptr, const int32_t* __restrict__ in_perm,
-                        const int32_t* __restrict__ out_rowptr, __nv_bfloat16* __restrict__ X, int64_t n_nodes) {
-  constexpr int H = 128;
-  const int lane = threadIdx.x & 31;
-  const int64_t w = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-  if (w >= 2 * n_nodes) return;
-  const int64_t v = n_nodes - 1 - (w >> 1);   // from the back: the edge kernel's last rows are still in L2
-  const int dir = (int)(w & 1);               // 0: in (dst == v, via perm), 1: out (src == v, contiguous)
-  const int32_t* rp = dir == 0 ? in_rowptr : out_rowptr;
-  const int b = rp[v], e = rp[v + 1];
-  const int half = lane >> 4, c = (lane & 15) * 8;
-  float acc[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-  for (int base = b; base < e; base += 32) {
-    const int cnt = min(32, e - base);
-    const int mine = base + lane < e ? (dir == 0 ? __ldg(in_perm + base + lane) : base + lane) : 0;
-    for (int j = 0; j < cnt; j += 8) {
-      uint4 u[4];
-#pragma unroll
-      for (int t = 0; t < 4; ++t) {
-        const int r = j + 2 * t + half;
-        const int idx = __shfl_sync(0xffffffffu, mine, r & 31);
-        u[t] = r < cnt ? __ldg(reinterpret_cast<const uint4*>(E + (int64_t)idx * H + c)) : make_uint4(0u, 0u, 0u, 0u);
-      }
-#pragma unroll
-      for (int t = 0; t < 4; ++t) {
-        const __nv_bfloat162* h2 = reinterpret_cast<const __nv_bfloat162*>(&u[t]);
-#pragma unroll
-        for (int i = 0; i < 4; ++i) {
-          acc[2 * i] += __low2float(h2[i]);
-          acc[2 * i + 1] += __high2float(h2[i]);
-        }
-      }
-    }
-  }
-#pragma unroll
-  for (int i = 0; i < 8; ++i) acc[i] += __shfl_xor_sync(0xffffffffu, acc[i], 16);
-  if (half == 0) {
-    __nv_bfloat162 o[4];
-#pragma unroll
-    for (int i = 0; i < 4; ++i) o[i] = __floats2bfloat162_rn(acc[2 * i], acc[2 * i + 1]);
-    *reinterpret_cast<uint4*>(X + v * (3 * H) + H + dir * H + c) = *reinterpret_cast<const uint4*>(o);
-  }
-}
-
 }  // namespace
 
 trk_status build_gnn_csr(trk_ctx* ctx, const int32_t* src, const int32_t* dst, const int32_t* n_edges_dev, int64_t n_edges_cap,
@@ -229,10 +179,8 @@ trk_status build_gnn_csr(trk_ctx* ctx, const int32_t* src, const int32_t* dst, c
 trk_status segment_sums(trk_ctx* ctx, const void* E, bool bf16, int64_t n_nodes, void* X, cudaStream_t st) {
   const int H = ctx->H;
   const unsigned blocks = (unsigned)ceil_div(2 * n_nodes * 32, 256);
-  if (bf16 && H == 128 && false) {   // measured slower than the generic kernel (99 vs 80 us per pileup-200 iteration)
-    TRK_LAUNCH(ctx, segment_sum_h128_kernel, blocks, 256, 0, st, (const __nv_bfloat16*)E, ctx->in_rowptr, ctx->in_perm, ctx->out_rowptr,
-               (__nv_bfloat16*)X, n_nodes);
-  } else if (bf16) {
+  // (a half-warp-per-row variant for H = 128 was measured slower: 99 vs 80 us per pileup-200 iteration)
+  if (bf16) {
     TRK_LAUNCH(ctx, segment_sum_kernel<__nv_bfloat16>, blocks, 256, 0, st, (const __nv_bfloat16*)E, H, ctx->in_rowptr,
                ctx->in_perm, ctx->out_rowptr, (__nv_bfloat16*)X, 3 * H, n_nodes);
   } else {
