@@ -14,6 +14,7 @@ namespace trk {
 
 constexpr int kMaxEmbDim = 16;      // d_e is padded to a multiple of 4, at most 16
 constexpr int kMaxEvents = 1024;    // event offsets travel as a kernel parameter
+constexpr int kPhiBins = 1024;           // S4: nodes are visited by phi bin in the segmented sums (graph.cu)
 constexpr int kRBuckets = 16;            // FRNN: radius buckets inside a spatial cell (a tracking detector has ~10 layers)
 constexpr int64_t kMaxCells = 1 << 22;  // FRNN cell-table entries (spatial cells x radius buckets) summed over the events of a call
 constexpr int kFilterChunkTilesPerSm = 64;  // default S3 rows per pass = 128 x sm_count x 64 (trk_config.filter_chunk_rows overrides):
@@ -144,6 +145,8 @@ struct trk_ctx {
   int32_t* in_perm = nullptr;       // [max_kept_edges]
   int32_t* in_fill = nullptr;       // [max_hits]
   int32_t* out_rowptr = nullptr;    // [max_hits+1] CSR by src (edges are src-sorted)
+  int32_t* node_order = nullptr;    // [max_hits] the nodes by phi bin: the order in which the segmented sums visit them (graph.cu)
+  int32_t* phi_bins = nullptr;      // [2 * (kPhiBins + 1)] counts / starts of the phi bins
   // S5
   int32_t* parent = nullptr;        // [max_hits]
   // S6 (tracks.cu): sizes / flags / scans and the (key, value) ping-pong of the radix sort, [max_hits+2] each

@@ -123,18 +123,56 @@ __device__ __forceinline__ void store4<__nv_bfloat16>(__nv_bfloat16* p, float4 v
   *reinterpret_cast<uint2*>(p) = u;
 }
 
+// ---- the order in which the segmented sums visit the nodes ----
+// Every row of E is read twice per iteration: as an out-edge of its source and as an in-edge of its destination.  E (187 MB at
+// pileup-200) does not fit the L2, and in hit-index order (the hits arrive shuffled) the two reads are far apart: 307 MB came
+// from DRAM.  The endpoints of an edge are neighbours in the detector, so with the nodes visited by azimuth the second read of
+// a row follows the first within a few thousand nodes and hits the L2: every row comes from DRAM once (an LRU model of the L2
+// reproduces both figures).  Only the ORDER OF VISITS changes -- each node's sum keeps its fixed order of edges -- so the
+// results are the same bits; the position of a node inside its bin (atomics) is irrelevant for the same reason.
+__device__ __forceinline__ int phi_bin(float phi_over_pi) {
+  const int b = (int)((phi_over_pi + 1.f) * (0.5f * kPhiBins));
+  return min(max(b, 0), kPhiBins - 1);
+}
+__global__ void phi_count_kernel(const float* __restrict__ hits, int64_t n, int32_t* __restrict__ count) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) atomicAdd(&count[phi_bin(hits[i * 3 + 1])], 1);
+}
+// one block of kPhiBins threads: start = exclusive scan of count; count is zeroed for the placement pass
+__global__ void __launch_bounds__(kPhiBins) phi_scan_kernel(int32_t* __restrict__ count, int32_t* __restrict__ start) {
+  __shared__ int32_t s[kPhiBins];
+  const int t = threadIdx.x;
+  const int32_t mine = count[t];
+  s[t] = mine;
+  __syncthreads();
+  for (int o = 1; o < kPhiBins; o <<= 1) {
+    const int32_t add = t >= o ? s[t - o] : 0;
+    __syncthreads();
+    s[t] += add;
+    __syncthreads();
+  }
+  start[t] = s[t] - mine;
+  count[t] = 0;
+}
+__global__ void phi_place_kernel(const float* __restrict__ hits, int64_t n, const int32_t* __restrict__ start, int32_t* __restrict__ fill,
+                                 int32_t* __restrict__ order) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) {
+    const int b = phi_bin(hits[i * 3 + 1]);
+    order[start[b] + atomicAdd(&fill[b], 1)] = (int32_t)i;
+  }
+}
+
 // One warp per (node, direction): X[v][H + dir*H + :] = sum over the segment of E rows (fp32 accumulate).
 // H is a multiple of 4; lanes cover H/4 float4 columns in strides of 32.
 template <typename T>
 __global__ void __launch_bounds__(256)
 segment_sum_kernel(const T* __restrict__ E, int H, const int32_t* __restrict__ in_rowptr, const int32_t* __restrict__ in_perm,
-                   const int32_t* __restrict__ out_rowptr, T* __restrict__ X, int ldx, int64_t n_nodes) {
+                   const int32_t* __restrict__ out_rowptr, const int32_t* __restrict__ order, T* __restrict__ X, int ldx, int64_t n_nodes) {
   const int lane = threadIdx.x & 31;
   const int64_t w = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   if (w >= 2 * n_nodes) return;
-  // nodes from the back: the edge kernel has just written E front to back, so its last rows (the out-edges of the
-  // highest nodes) are still in L2
-  const int64_t v = n_nodes - 1 - (w >> 1);
+  const int64_t v = order[w >> 1];        // nodes by azimuth (see above)
   const int dir = (int)(w & 1);  // 0: in (dst == v, via perm), 1: out (src == v, contiguous)
   const int32_t* rp = dir == 0 ? in_rowptr : out_rowptr;
   const int b = rp[v], e = rp[v + 1];
@@ -163,8 +201,18 @@ segment_sum_kernel(const T* __restrict__ E, int H, const int32_t* __restrict__ i
 
 }  // namespace
 
-trk_status build_gnn_csr(trk_ctx* ctx, const int32_t* src, const int32_t* dst, const int32_t* n_edges_dev, int64_t n_edges_cap,
-                         int64_t n_nodes, cudaStream_t st) {
+trk_status build_gnn_csr(trk_ctx* ctx, const float* hits, const int32_t* src, const int32_t* dst, const int32_t* n_edges_dev,
+                         int64_t n_edges_cap, int64_t n_nodes, cudaStream_t st) {
+  // the visiting order of the segmented sums: nodes counting-sorted by phi bin (hits[:, 1] = phi / pi in (-1, 1])
+  if (n_nodes > 0) {
+    int32_t* count = ctx->phi_bins;
+    int32_t* start = ctx->phi_bins + kPhiBins + 1;
+    const unsigned nb = (unsigned)ceil_div(n_nodes, 256);
+    TRK_TRY(fill_i32(ctx, count, 0, kPhiBins, st));
+    TRK_LAUNCH(ctx, phi_count_kernel, nb, 256, 0, st, hits, n_nodes, count);
+    TRK_LAUNCH(ctx, phi_scan_kernel, 1, kPhiBins, 0, st, count, start);
+    TRK_LAUNCH(ctx, phi_place_kernel, nb, 256, 0, st, hits, n_nodes, start, count, ctx->node_order);
+  }
   const unsigned eb = (unsigned)ceil_div(n_edges_cap + 1, 256);
   TRK_LAUNCH(ctx, rowptr_from_sorted_kernel, eb, 256, 0, st, src, n_edges_dev, n_edges_cap, ctx->out_rowptr, n_nodes);
   TRK_TRY(fill_i32(ctx, ctx->in_fill, 0, n_nodes + 1, st));
@@ -182,10 +230,10 @@ trk_status segment_sums(trk_ctx* ctx, const void* E, bool bf16, int64_t n_nodes,
   // (a half-warp-per-row variant for H = 128 was measured slower: 99 vs 80 us per pileup-200 iteration)
   if (bf16) {
     TRK_LAUNCH(ctx, segment_sum_kernel<__nv_bfloat16>, blocks, 256, 0, st, (const __nv_bfloat16*)E, H, ctx->in_rowptr,
-               ctx->in_perm, ctx->out_rowptr, (__nv_bfloat16*)X, 3 * H, n_nodes);
+               ctx->in_perm, ctx->out_rowptr, ctx->node_order, (__nv_bfloat16*)X, 3 * H, n_nodes);
   } else {
     TRK_LAUNCH(ctx, segment_sum_kernel<float>, blocks, 256, 0, st, (const float*)E, H, ctx->in_rowptr, ctx->in_perm,
-               ctx->out_rowptr, (float*)X, 3 * H, n_nodes);
+               ctx->out_rowptr, ctx->node_order, (float*)X, 3 * H, n_nodes);
   }
   return TRK_OK;
 }

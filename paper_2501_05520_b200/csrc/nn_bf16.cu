@@ -520,7 +520,7 @@ trk_status gnn_forward_bf16(trk_ctx* ctx, const float* hits, int64_t n, const in
   const int64_t x_rows = ctx->cfg.max_hits, e_rows = ctx->cfg.max_kept_edges, t_rows = std::max(x_rows, e_rows);
   tc::Rows nrows{nullptr, 0, n};
   tc::Rows erows{n_edges_dev, 0, n_edges_cap};
-  TRK_TRY(build_gnn_csr(ctx, src, dst, n_edges_dev, n_edges_cap, n, st));
+  TRK_TRY(build_gnn_csr(ctx, hits, src, dst, n_edges_dev, n_edges_cap, n, st));
 
   const bool fused = H == gf::kH && ctx->knobs[kKnobGnnFused] != 0;
   if (fused) {

@@ -222,7 +222,7 @@ trk_status gnn_forward_fp32(trk_ctx* ctx, const float* hits, int64_t n, const in
   float* E = (float*)ctx->E;    // [E][H]
   float* T1 = (float*)ctx->T1;  // scratch, 2 * rows * H floats
   float* cat = ctx->cat;
-  TRK_TRY(build_gnn_csr(ctx, src, dst, n_edges_dev, n_edges_cap, n, st));
+  TRK_TRY(build_gnn_csr(ctx, hits, src, dst, n_edges_dev, n_edges_cap, n, st));
   // encoders
   TRK_TRY(mlp2_lnr_f32(ctx, hits, 3, ctx->node_enc, T1, nullptr, 0, X, 3 * H, nullptr, n, st));
   if (n_edges_cap > 0) {
