@@ -183,6 +183,7 @@ void carve(trk_ctx* c, Carver& k) {
   k.take(&c->out_rowptr, N + 2);
   k.take(&c->node_order, N);
   k.take(&c->phi_bins, 2 * (kPhiBins + 1));
+  k.take(&c->seg_tasks, 2 * N);
   k.take(&c->parent, N);
   for (int32_t** t : {&c->tk_a, &c->tk_b, &c->tk_c, &c->tk_d, &c->tk_e, &c->tk_f, &c->tk_g}) k.take(t, N + 2);
   k.take(&c->tk_hist, (N + 255) / 256 * 256 + 2);

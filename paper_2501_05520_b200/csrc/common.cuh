@@ -147,6 +147,7 @@ struct trk_ctx {
   int32_t* out_rowptr = nullptr;    // [max_hits+1] CSR by src (edges are src-sorted)
   int32_t* node_order = nullptr;    // [max_hits] the nodes by phi bin: the order in which the segmented sums visit them (graph.cu)
   int32_t* phi_bins = nullptr;      // [2 * (kPhiBins + 1)] counts / starts of the phi bins
+  int4* seg_tasks = nullptr;        // [2 max_hits] (node, first entry, end entry, direction) of the segmented sums, in visiting order
   // S5
   int32_t* parent = nullptr;        // [max_hits]
   // S6 (tracks.cu): sizes / flags / scans and the (key, value) ping-pong of the radix sort, [max_hits+2] each

@@ -163,23 +163,45 @@ __global__ void phi_place_kernel(const float* __restrict__ hits, int64_t n, cons
   }
 }
 
+// The work list of the segmented sums, built once per call: task 2 p + dir = (node at position p of the visiting order, its
+// segment bounds), so a warp of segment_sum_kernel starts from ONE coalesced 16-byte load instead of the chain
+// order -> row pointer -> ...
+__global__ void seg_tasks_kernel(const int32_t* __restrict__ order, const int32_t* __restrict__ in_rowptr,
+                                 const int32_t* __restrict__ out_rowptr, int4* __restrict__ tasks, int64_t n_nodes) {
+  const int64_t w = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (w >= 2 * n_nodes) return;
+  const int v = order[w >> 1], dir = (int)(w & 1);
+  const int32_t* rp = dir == 0 ? in_rowptr : out_rowptr;
+  tasks[w] = make_int4(v, rp[v], rp[v + 1], dir);
+}
+
 // One warp per (node, direction): X[v][H + dir*H + :] = sum over the segment of E rows (fp32 accumulate).
 // H is a multiple of 4; lanes cover H/4 float4 columns in strides of 32.
 template <typename T>
 __global__ void __launch_bounds__(256)
-segment_sum_kernel(const T* __restrict__ E, int H, const int32_t* __restrict__ in_rowptr, const int32_t* __restrict__ in_perm,
-                   const int32_t* __restrict__ out_rowptr, const int32_t* __restrict__ order, T* __restrict__ X, int ldx, int64_t n_nodes) {
+segment_sum_kernel(const T* __restrict__ E, int H, const int4* __restrict__ tasks, const int32_t* __restrict__ in_perm,
+                   T* __restrict__ X, int ldx, int64_t n_nodes) {
   const int lane = threadIdx.x & 31;
   const int64_t w = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   if (w >= 2 * n_nodes) return;
-  const int64_t v = order[w >> 1];        // nodes by azimuth (see above)
-  const int dir = (int)(w & 1);  // 0: in (dst == v, via perm), 1: out (src == v, contiguous)
-  const int32_t* rp = dir == 0 ? in_rowptr : out_rowptr;
-  const int b = rp[v], e = rp[v + 1];
+  const int4 task = tasks[w];             // nodes by azimuth (see above)
+  const int64_t v = task.x;
+  const int dir = task.w;        // 0: in (dst == v, via perm), 1: out (src == v, contiguous)
+  const int b = task.y, e = task.z;
   for (int c = lane * 4; c < H; c += 128) {
     float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
     int k = b;
-    for (; k + 4 <= e; k += 4) {               // four independent row loads in flight; the sum keeps its fixed order
+    for (; k + 8 <= e; k += 8) {               // eight independent row loads in flight; the sum keeps its fixed order
+      int64_t r[8];
+#pragma unroll
+      for (int t = 0; t < 8; ++t) r[t] = dir == 0 ? in_perm[k + t] : k + t;
+      float4 x[8];
+#pragma unroll
+      for (int t = 0; t < 8; ++t) x[t] = load4<T>(E + r[t] * H + c);
+#pragma unroll
+      for (int t = 0; t < 8; ++t) { acc.x += x[t].x; acc.y += x[t].y; acc.z += x[t].z; acc.w += x[t].w; }
+    }
+    for (; k + 4 <= e; k += 4) {               // four
       int64_t r0, r1, r2, r3;
       if (dir == 0) { r0 = in_perm[k]; r1 = in_perm[k + 1]; r2 = in_perm[k + 2]; r3 = in_perm[k + 3]; }
       else { r0 = k; r1 = k + 1; r2 = k + 2; r3 = k + 3; }
@@ -221,6 +243,9 @@ trk_status build_gnn_csr(trk_ctx* ctx, const float* hits, const int32_t* src, co
   TRK_TRY(fill_i32(ctx, ctx->in_fill, 0, n_nodes, st));
   TRK_LAUNCH(ctx, place_keys_kernel, eb, 256, 0, st, dst, n_edges_dev, n_edges_cap, ctx->in_rowptr, ctx->in_fill, ctx->in_perm);
   TRK_LAUNCH(ctx, sort_segments_kernel, (unsigned)ceil_div(n_nodes * 32, 256), 256, 0, st, ctx->in_rowptr, ctx->in_perm, n_nodes);
+  if (n_nodes > 0)
+    TRK_LAUNCH(ctx, seg_tasks_kernel, (unsigned)ceil_div(2 * n_nodes, 256), 256, 0, st, ctx->node_order, ctx->in_rowptr, ctx->out_rowptr,
+               ctx->seg_tasks, n_nodes);
   return TRK_OK;
 }
 
@@ -229,11 +254,11 @@ trk_status segment_sums(trk_ctx* ctx, const void* E, bool bf16, int64_t n_nodes,
   const unsigned blocks = (unsigned)ceil_div(2 * n_nodes * 32, 256);
   // (a half-warp-per-row variant for H = 128 was measured slower: 99 vs 80 us per pileup-200 iteration)
   if (bf16) {
-    TRK_LAUNCH(ctx, segment_sum_kernel<__nv_bfloat16>, blocks, 256, 0, st, (const __nv_bfloat16*)E, H, ctx->in_rowptr,
-               ctx->in_perm, ctx->out_rowptr, ctx->node_order, (__nv_bfloat16*)X, 3 * H, n_nodes);
+    TRK_LAUNCH(ctx, segment_sum_kernel<__nv_bfloat16>, blocks, 256, 0, st, (const __nv_bfloat16*)E, H, ctx->seg_tasks,
+               ctx->in_perm, (__nv_bfloat16*)X, 3 * H, n_nodes);
   } else {
-    TRK_LAUNCH(ctx, segment_sum_kernel<float>, blocks, 256, 0, st, (const float*)E, H, ctx->in_rowptr, ctx->in_perm,
-               ctx->out_rowptr, ctx->node_order, (float*)X, 3 * H, n_nodes);
+    TRK_LAUNCH(ctx, segment_sum_kernel<float>, blocks, 256, 0, st, (const float*)E, H, ctx->seg_tasks, ctx->in_perm,
+               (float*)X, 3 * H, n_nodes);
   }
   return TRK_OK;
 }
