@@ -196,6 +196,7 @@ void carve(trk_ctx* c, Carver& k) {
 }
 
 __global__ void finalize_counts_kernel(const int32_t* __restrict__ counts, int64_t edge_cap, int64_t cand_cap, int32_t* __restrict__ out) {
+  TRK_GRID_DEP_WAIT();
   if (threadIdx.x != 0 || blockIdx.x != 0) return;
   int of = counts[3];
   if (edge_cap >= 0 && counts[1] > edge_cap) of = 1;
@@ -207,6 +208,7 @@ __global__ void finalize_counts_kernel(const int32_t* __restrict__ counts, int64
 }
 
 __global__ void zero_counts_kernel(int32_t* counts) {
+  TRK_GRID_DEP_WAIT();
   if (threadIdx.x < 8) counts[threadIdx.x] = 0;
 }
 

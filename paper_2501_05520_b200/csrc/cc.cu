@@ -7,6 +7,7 @@ namespace trk {
 namespace {
 
 __global__ void cc_init_kernel(int32_t* __restrict__ parent, int64_t n, int32_t* __restrict__ pass_count) {
+  TRK_GRID_DEP_WAIT();
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i < n) parent[i] = (int32_t)i;
   if (i == 0 && pass_count) *pass_count = 0;
@@ -38,6 +39,7 @@ __device__ __forceinline__ int32_t find_root(int32_t* parent, int32_t x) {
 __global__ void cc_union_kernel(int32_t* __restrict__ parent, const int32_t* __restrict__ src, const int32_t* __restrict__ dst,
                                 const float* __restrict__ score, const int32_t* __restrict__ n_edges_dev, int64_t n_edges_cap,
                                 float cut, int32_t* __restrict__ pass_count) {
+  TRK_GRID_DEP_WAIT();
   const int64_t n_edges = n_edges_dev ? min((int64_t)*n_edges_dev, n_edges_cap) : n_edges_cap;
   int local = 0;
   for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n_edges; k += (int64_t)gridDim.x * blockDim.x) {
@@ -62,6 +64,7 @@ __global__ void cc_union_kernel(int32_t* __restrict__ parent, const int32_t* __r
 }
 
 __global__ void cc_flatten_kernel(const int32_t* __restrict__ parent, int32_t* __restrict__ labels, int64_t n) {
+  TRK_GRID_DEP_WAIT();
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   int32_t x = (int32_t)i;

@@ -162,6 +162,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsFilter, 1)
 filter_mlp_kernel(const __grid_constant__ CUtensorMap tmS1, const __grid_constant__ CUtensorMap tmS2, const __grid_constant__ CUtensorMap tmW1,
                   const __grid_constant__ CUtensorMap tmW2, const __grid_constant__ CUtensorMap tmW3, const __grid_constant__ CUtensorMap tmS1st,
                   const __grid_constant__ CUtensorMap tmS2st, Rows rows, FilterParams p) {
+  TRK_GRID_DEP_WAIT();
   constexpr int A_BYTES = BM * BK * 2;
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);

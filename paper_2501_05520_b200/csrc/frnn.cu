@@ -30,6 +30,7 @@ __device__ __forceinline__ int float_to_ordered(float f) {
 __device__ __forceinline__ float ordered_to_float(int i) { return __int_as_float(i >= 0 ? i : i ^ 0x7fffffff); }
 
 __global__ void frnn_reset_kernel(int32_t* __restrict__ bbox, int32_t* __restrict__ cell_count, int64_t n_cells_plus1) {
+  TRK_GRID_DEP_WAIT();
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i < 3) {
     bbox[i] = 0x7fffffff;          // min
@@ -46,6 +47,7 @@ __global__ void frnn_reset_kernel(int32_t* __restrict__ bbox, int32_t* __restric
 // proj[i] = P^T e_i  (or the first g coordinates), and the global bounding box.
 __global__ void frnn_project_kernel(const float* __restrict__ emb, const float* __restrict__ hits, int d_e, const float* __restrict__ P, int g,
                                     float* __restrict__ proj, int32_t* __restrict__ bbox, int64_t n) {
+  TRK_GRID_DEP_WAIT();
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   float p[3] = {0.f, 0.f, 0.f};
   float emax = 0.f;
@@ -96,6 +98,7 @@ __global__ void frnn_project_kernel(const float* __restrict__ emb, const float* 
 }
 
 __global__ void frnn_grid_setup_kernel(const int32_t* __restrict__ bbox, float radius, int g, int G, GridParams* __restrict__ gp) {
+  TRK_GRID_DEP_WAIT();
   if (threadIdx.x != 0 || blockIdx.x != 0) return;
   // Rounding slack of the fp32 projection p = sum_k e_k P_ka (an fmaf chain): |p_hat - p| <= d_e 2^-24 sum_k |e_k| |P_ka|
   // <= d_e^1.5 2^-24 max|e| (unit columns), i.e. <= 2^-18 max|e| for d_e <= 16.  Two computed points are at most 2 sqrt(3) of
@@ -149,6 +152,7 @@ __device__ __forceinline__ void cell_coords(const GridParams& gp, const float* p
 __global__ void frnn_count_kernel(const float* __restrict__ proj, const float* __restrict__ hits, const int32_t* __restrict__ ev_of_hit,
                                   const GridParams* __restrict__ gpp, int32_t* __restrict__ cell_of_hit,
                                   int32_t* __restrict__ cell_count, int64_t n) {
+  TRK_GRID_DEP_WAIT();
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   const GridParams gp = *gpp;
@@ -165,6 +169,7 @@ __global__ void frnn_scatter_kernel(const float* __restrict__ emb, const float* 
                                     const int32_t* __restrict__ cell_of_hit, const int32_t* __restrict__ cell_start,
                                     int32_t* __restrict__ cell_fill, float* __restrict__ semb, float4* __restrict__ smeta,
                                     const float* __restrict__ proj, float4* __restrict__ sproj, int64_t n) {
+  TRK_GRID_DEP_WAIT();
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   const int cell = cell_of_hit[i];
@@ -220,6 +225,7 @@ __global__ void __launch_bounds__(kWarpsPerBlock * 32)
 frnn_search_kernel(const float* __restrict__ semb, const float4* __restrict__ smeta, const float4* __restrict__ sproj,
                    const int32_t* __restrict__ cell_start, const GridParams* __restrict__ gpp, double r2_in, float r2_loose_in,
                    float r_proj_in, float proj_scale, int K, int32_t* __restrict__ slots, int32_t* __restrict__ deg, int64_t n) {
+  TRK_GRID_DEP_WAIT();
   constexpr int D = D4 * 4;
   constexpr int PER = CAP / 32;            // buffer entries per lane
   __shared__ unsigned long long s_d2[kWarpsPerBlock][CAP];
@@ -478,6 +484,7 @@ frnn_search_kernel(const float* __restrict__ semb, const float4* __restrict__ sm
 __global__ void frnn_emit_kernel(const int32_t* __restrict__ slots, const int32_t* __restrict__ rowptr, int K,
                                  int32_t* __restrict__ src, int32_t* __restrict__ dst, int32_t* __restrict__ rowptr_out,
                                  int64_t capacity, int32_t* __restrict__ count_out, int32_t* __restrict__ overflow_flag, int64_t n) {
+  TRK_GRID_DEP_WAIT();
   // one warp per hit
   const int lane = threadIdx.x & 31;
   const int64_t i = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
@@ -504,6 +511,7 @@ __global__ void frnn_emit_kernel(const int32_t* __restrict__ slots, const int32_
 // Event offsets travel as a kernel parameter (by value), so trk_infer needs no staging copy and
 // stays graph-capturable.
 __global__ void event_of_hit_kernel(const __grid_constant__ EventOffsets offs, int n_events, int32_t* __restrict__ ev_of_hit, int64_t n) {
+  TRK_GRID_DEP_WAIT();
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   int lo = 0, hi = n_events;  // offsets[lo] <= i < offsets[hi]

@@ -192,6 +192,7 @@ template <int BN, class Epi, int SPLIT = 1, bool GATHER_A = false>
 __global__ void __launch_bounds__(threads_for(SPLIT, GATHER_A), 1)
 gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, const __grid_constant__ CUtensorMap tmC,
                Rows rows, int n_tiles, int k_blocks, typename Epi::Params ep, AGather ag) {
+  TRK_GRID_DEP_WAIT();
   constexpr int STAGES = num_stages(BN, SPLIT);
   constexpr int A_BYTES = BM * BK * 2;
   constexpr int STAGE = stage_bytes(BN);

@@ -99,6 +99,7 @@ template <int BN, class Epi>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
 gemm_tc2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, const __grid_constant__ CUtensorMap tmC,
                 Rows rows, int n_tiles, int k_blocks, typename Epi::Params ep, int row_major_min) {
+  TRK_GRID_DEP_WAIT();
   constexpr int STAGES = num_stages_pair(BN);
   constexpr int A_BYTES = BM * BK * 2;
   constexpr int STAGE = stage_bytes_pair(BN);

@@ -223,6 +223,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kFusedThreads, 1)
 gnn_fused_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constant__ CUtensorMap tmW2,
                        const __grid_constant__ CUtensorMap tmE, const __grid_constant__ CUtensorMap tmEst, Rows rows,
                        const __grid_constant__ FusedParams p) {
+  TRK_GRID_DEP_WAIT();
   extern __shared__ __align__(1024) uint8_t smem[];
   if ((smem_u32(smem) & 1023u) != 0) __trap();   // the swizzled operand layout needs the 1024-byte alignment declared above
   Bars* bar = reinterpret_cast<Bars*>(smem + kOffBar);

@@ -18,6 +18,7 @@ __device__ __forceinline__ int64_t dev_count(const int32_t* n_dev, int64_t cap) 
 // rowptr[v] = first k with key[k] >= v, for sorted keys; rowptr[n_nodes] = n_edges.
 __global__ void rowptr_from_sorted_kernel(const int32_t* __restrict__ key, const int32_t* __restrict__ n_dev, int64_t cap,
                                           int32_t* __restrict__ rowptr, int64_t n_nodes) {
+  TRK_GRID_DEP_WAIT();
   const int64_t n_edges = dev_count(n_dev, cap);
   const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (k > n_edges) return;
@@ -28,6 +29,7 @@ __global__ void rowptr_from_sorted_kernel(const int32_t* __restrict__ key, const
 
 __global__ void count_keys_kernel(const int32_t* __restrict__ key, const int32_t* __restrict__ n_dev, int64_t cap,
                                   int32_t* __restrict__ count) {
+  TRK_GRID_DEP_WAIT();
   const int64_t n_edges = dev_count(n_dev, cap);
   const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (k < n_edges) atomicAdd(&count[key[k]], 1);
@@ -35,6 +37,7 @@ __global__ void count_keys_kernel(const int32_t* __restrict__ key, const int32_t
 
 __global__ void place_keys_kernel(const int32_t* __restrict__ key, const int32_t* __restrict__ n_dev, int64_t cap,
                                   const int32_t* __restrict__ rowptr, int32_t* __restrict__ fill, int32_t* __restrict__ perm) {
+  TRK_GRID_DEP_WAIT();
   const int64_t n_edges = dev_count(n_dev, cap);
   const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (k < n_edges) {
@@ -50,6 +53,7 @@ __global__ void place_keys_kernel(const int32_t* __restrict__ key, const int32_t
 constexpr int kSortChunks = 8;
 constexpr int kSortMaxLen = 32 * kSortChunks;
 __global__ void __launch_bounds__(256) sort_segments_kernel(const int32_t* __restrict__ rowptr, int32_t* __restrict__ perm, int64_t n_nodes) {
+  TRK_GRID_DEP_WAIT();
   const int lane = threadIdx.x & 31;
   const int64_t v = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   if (v >= n_nodes) return;
@@ -135,11 +139,13 @@ __device__ __forceinline__ int phi_bin(float phi_over_pi) {
   return min(max(b, 0), kPhiBins - 1);
 }
 __global__ void phi_count_kernel(const float* __restrict__ hits, int64_t n, int32_t* __restrict__ count) {
+  TRK_GRID_DEP_WAIT();
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i < n) atomicAdd(&count[phi_bin(hits[i * 3 + 1])], 1);
 }
 // one block of kPhiBins threads: start = exclusive scan of count; count is zeroed for the placement pass
 __global__ void __launch_bounds__(kPhiBins) phi_scan_kernel(int32_t* __restrict__ count, int32_t* __restrict__ start) {
+  TRK_GRID_DEP_WAIT();
   __shared__ int32_t s[kPhiBins];
   const int t = threadIdx.x;
   const int32_t mine = count[t];
@@ -156,6 +162,7 @@ __global__ void __launch_bounds__(kPhiBins) phi_scan_kernel(int32_t* __restrict_
 }
 __global__ void phi_place_kernel(const float* __restrict__ hits, int64_t n, const int32_t* __restrict__ start, int32_t* __restrict__ fill,
                                  int32_t* __restrict__ order) {
+  TRK_GRID_DEP_WAIT();
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i < n) {
     const int b = phi_bin(hits[i * 3 + 1]);
@@ -168,6 +175,7 @@ __global__ void phi_place_kernel(const float* __restrict__ hits, int64_t n, cons
 // order -> row pointer -> ...
 __global__ void seg_tasks_kernel(const int32_t* __restrict__ order, const int32_t* __restrict__ in_rowptr,
                                  const int32_t* __restrict__ out_rowptr, int4* __restrict__ tasks, int64_t n_nodes) {
+  TRK_GRID_DEP_WAIT();
   const int64_t w = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (w >= 2 * n_nodes) return;
   const int v = order[w >> 1], dir = (int)(w & 1);
@@ -181,6 +189,7 @@ template <typename T>
 __global__ void __launch_bounds__(256)
 segment_sum_kernel(const T* __restrict__ E, int H, const int4* __restrict__ tasks, const int32_t* __restrict__ in_perm,
                    T* __restrict__ X, int ldx, int64_t n_nodes) {
+  TRK_GRID_DEP_WAIT();
   const int lane = threadIdx.x & 31;
   const int64_t w = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   if (w >= 2 * n_nodes) return;

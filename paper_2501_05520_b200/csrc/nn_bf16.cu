@@ -240,6 +240,7 @@ constexpr int kFirstLayerRowsPerBlock = 64;
 __global__ void __launch_bounds__(256)
 embed_first_layer_kernel(const float* __restrict__ hits, const float* __restrict__ W, const float* __restrict__ b,
                          bf16* __restrict__ out, int64_t M, int N) {
+  TRK_GRID_DEP_WAIT();
   const int groups = N / 8;                       // 16-byte column groups per row
   const int lanes_r = blockDim.x / groups;        // rows in flight per pass (host guarantees groups <= blockDim.x)
   const int g = threadIdx.x % groups, rl = threadIdx.x / groups;
@@ -269,6 +270,7 @@ embed_first_layer_kernel(const float* __restrict__ hits, const float* __restrict
 __global__ void filter_gather_kernel(const float* __restrict__ feat, int u, int cpr_log2, const int32_t* __restrict__ src,
                                      const int32_t* __restrict__ dst, const int32_t* __restrict__ m_dev, int64_t m_off, int64_t m_cap,
                                      bf16* __restrict__ out) {
+  TRK_GRID_DEP_WAIT();
   const int64_t M = rows_of(m_dev, m_off, m_cap);
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   const int64_t row = i >> cpr_log2;
@@ -304,6 +306,7 @@ __global__ void filter_gather_kernel(const float* __restrict__ feat, int u, int 
 
 __global__ void filter_finish_kernel(const float* __restrict__ partial, int n_tiles, float b_last, const int32_t* __restrict__ m_dev,
                                      int64_t m_off, int64_t m_cap, float* __restrict__ score) {
+  TRK_GRID_DEP_WAIT();
   const int64_t M = rows_of(m_dev, m_off, m_cap);
   const int64_t row = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (row >= M) return;
@@ -321,6 +324,7 @@ __global__ void __launch_bounds__(256)
 encoder_first_layer_kernel(const float* __restrict__ hits, const int32_t* __restrict__ src, const int32_t* __restrict__ dst,
                            const float* __restrict__ W, const float* __restrict__ b, int use_ln,
                            const int32_t* __restrict__ m_dev, int64_t m_cap, bf16* __restrict__ out) {
+  TRK_GRID_DEP_WAIT();
   constexpr int K = EDGE ? 4 : 3;
   constexpr int H = PER * 32;
   const int64_t M = rows_of(m_dev, 0, m_cap);

@@ -22,6 +22,7 @@ template <int ACT>
 __global__ void __launch_bounds__(256)
 linear_f32_kernel(const float* __restrict__ A, int lda, const float* __restrict__ W, const float* __restrict__ bias,
                   float* __restrict__ C, int ldc, const int32_t* __restrict__ m_dev, int64_t m_off, int64_t m_cap, int N, int K) {
+  TRK_GRID_DEP_WAIT();
   __shared__ float As[TK][TM + 4];
   __shared__ float Ws[TK][TN + 4];
   const int64_t M = rows_of(m_dev, m_off, m_cap);
@@ -80,6 +81,7 @@ linear_f32_kernel(const float* __restrict__ A, int lda, const float* __restrict_
 __global__ void __launch_bounds__(256)
 ln_relu_f32_kernel(const float* __restrict__ x, int ldx, const float* __restrict__ res, int ldr, float* __restrict__ out, int ldo,
                    const int32_t* __restrict__ m_dev, int64_t m_cap, int N, int use_ln) {
+  TRK_GRID_DEP_WAIT();
   const int64_t M = rows_of(m_dev, 0, m_cap);
   const int lane = threadIdx.x & 31;
   const int64_t row = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
@@ -107,6 +109,7 @@ ln_relu_f32_kernel(const float* __restrict__ x, int ldx, const float* __restrict
 __global__ void gather_pair_f32_kernel(const float* __restrict__ feat, int u, const int32_t* __restrict__ src,
                                        const int32_t* __restrict__ dst, const int32_t* __restrict__ m_dev, int64_t m_off,
                                        int64_t m_cap, float* __restrict__ out) {
+  TRK_GRID_DEP_WAIT();
   const int64_t M = rows_of(m_dev, m_off, m_cap);
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   const int64_t row = i / (2 * u);
@@ -120,6 +123,7 @@ __global__ void gather_pair_f32_kernel(const float* __restrict__ feat, int u, co
 __global__ void gather_edge_cat_f32_kernel(const float* __restrict__ h, int ldh, const float* __restrict__ e, int H,
                                            const int32_t* __restrict__ src, const int32_t* __restrict__ dst,
                                            const int32_t* __restrict__ m_dev, int64_t m_cap, float* __restrict__ cat) {
+  TRK_GRID_DEP_WAIT();
   const int64_t M = rows_of(m_dev, 0, m_cap);
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   const int64_t row = i / (3 * H);
@@ -137,6 +141,7 @@ __global__ void gather_edge_cat_f32_kernel(const float* __restrict__ h, int ldh,
 // (dr, dphi wrapped to (-1,1], dz, deta) per edge; shared with the bf16 path (nn.cuh).
 __global__ void edge_features_kernel(const float* __restrict__ hits, const int32_t* __restrict__ src, const int32_t* __restrict__ dst,
                                      const int32_t* __restrict__ m_dev, int64_t m_cap, float4* __restrict__ out) {
+  TRK_GRID_DEP_WAIT();
   const int64_t M = m_dev ? min((int64_t)max(*m_dev, 0), m_cap) : m_cap;
   const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (k >= M) return;

@@ -27,12 +27,14 @@ __device__ __forceinline__ int32_t label_of(const int32_t* __restrict__ labels, 
 }
 
 __global__ void track_size_kernel(const int32_t* __restrict__ labels, int64_t n, int32_t* __restrict__ size) {
+  TRK_GRID_DEP_WAIT();
   const int64_t v = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (v < n) atomicAdd(&size[label_of(labels, v, n)], 1);
 }
 
 __global__ void track_keep_kernel(const int32_t* __restrict__ labels, const int32_t* __restrict__ size, int64_t n, int min_hits,
                                   int32_t* __restrict__ keep, int32_t* __restrict__ ksize) {
+  TRK_GRID_DEP_WAIT();
   const int64_t v = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (v >= n) return;
   const int k = (label_of(labels, v, n) == (int32_t)v && size[v] >= min_hits) ? 1 : 0;
@@ -44,6 +46,7 @@ __global__ void track_keep_kernel(const int32_t* __restrict__ labels, const int3
 __global__ void track_offsets_kernel(const int32_t* __restrict__ keep, const int32_t* __restrict__ tidx, const int32_t* __restrict__ hoff,
                                      int64_t n, int64_t capacity, int32_t* __restrict__ track_offsets, int32_t* __restrict__ track_counts,
                                      int32_t* __restrict__ overflow_flag) {
+  TRK_GRID_DEP_WAIT();
   const int64_t v = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (v < n && keep[v] && tidx[v] <= capacity) track_offsets[tidx[v]] = hoff[v];
   if (v == 0) {
@@ -62,6 +65,7 @@ __global__ void track_offsets_kernel(const int32_t* __restrict__ keep, const int
 
 __global__ void track_key_kernel(const int32_t* __restrict__ labels, const int32_t* __restrict__ keep, const int32_t* __restrict__ tidx,
                                  int64_t n, int32_t* __restrict__ key, int32_t* __restrict__ val) {
+  TRK_GRID_DEP_WAIT();
   const int64_t v = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (v >= n) return;
   const int32_t r = label_of(labels, v, n);
@@ -73,6 +77,7 @@ __global__ void track_key_kernel(const int32_t* __restrict__ labels, const int32
 // every (digit, block) its first output position)
 __global__ void __launch_bounds__(kRadixThreads)
 radix_hist_kernel(const int32_t* __restrict__ key, int64_t n, int shift, int32_t* __restrict__ hist, int n_blocks) {
+  TRK_GRID_DEP_WAIT();
   __shared__ int cnt[kRadixBins];
   cnt[threadIdx.x] = 0;
   __syncthreads();
@@ -86,6 +91,7 @@ radix_hist_kernel(const int32_t* __restrict__ key, int64_t n, int shift, int32_t
 __global__ void __launch_bounds__(kRadixThreads)
 radix_scatter_kernel(const int32_t* __restrict__ key, const int32_t* __restrict__ val, int64_t n, int shift,
                      const int32_t* __restrict__ hist_scan, int n_blocks, int32_t* __restrict__ key_out, int32_t* __restrict__ val_out) {
+  TRK_GRID_DEP_WAIT();
   constexpr int kWarps = kRadixThreads / 32;
   __shared__ int wcnt[kWarps][kRadixBins];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -117,6 +123,7 @@ radix_scatter_kernel(const int32_t* __restrict__ key, const int32_t* __restrict_
 
 __global__ void track_emit_kernel(const int32_t* __restrict__ val, const int32_t* __restrict__ track_offsets, int64_t n,
                                   int32_t* __restrict__ track_counts, int32_t* __restrict__ track_hits) {
+  TRK_GRID_DEP_WAIT();
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   const int32_t total = track_offsets[track_counts[0]];
   if (i < n) track_hits[i] = i < total ? val[i] : -1;

@@ -39,6 +39,7 @@ __device__ __forceinline__ int block_exclusive_scan(int v, int* total) {
 
 __global__ void __launch_bounds__(kScanThreads) scan_local_kernel(const int32_t* __restrict__ in, int32_t* __restrict__ out,
                                                                   int32_t* __restrict__ block_sums, int64_t n) {
+  TRK_GRID_DEP_WAIT();
   __shared__ int total;
   const int64_t base = (int64_t)blockIdx.x * kScanTile + (int64_t)threadIdx.x * kScanItems;
   int v[kScanItems];
@@ -59,6 +60,7 @@ __global__ void __launch_bounds__(kScanThreads) scan_local_kernel(const int32_t*
 
 // Single block: exclusive scan of the block sums in place; block_sums[n_blocks] = grand total.
 __global__ void __launch_bounds__(kScanThreads) scan_sums_kernel(int32_t* __restrict__ block_sums, int64_t n_blocks) {
+  TRK_GRID_DEP_WAIT();
   __shared__ int total;
   int carry = 0;
   for (int64_t base = 0; base < n_blocks; base += kScanThreads) {
@@ -74,6 +76,7 @@ __global__ void __launch_bounds__(kScanThreads) scan_sums_kernel(int32_t* __rest
 
 __global__ void __launch_bounds__(kScanThreads) scan_add_kernel(int32_t* __restrict__ out, const int32_t* __restrict__ block_sums,
                                                                 int64_t n, int64_t n_blocks) {
+  TRK_GRID_DEP_WAIT();
   const int64_t base = (int64_t)blockIdx.x * kScanTile + (int64_t)threadIdx.x * kScanItems;
   const int add = block_sums[blockIdx.x];
 #pragma unroll
@@ -83,6 +86,7 @@ __global__ void __launch_bounds__(kScanThreads) scan_add_kernel(int32_t* __restr
 }
 
 __global__ void fill_i32_kernel(int32_t* p, int32_t v, int64_t n) {
+  TRK_GRID_DEP_WAIT();
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i < n) p[i] = v;
 }
@@ -90,6 +94,7 @@ __global__ void fill_i32_kernel(int32_t* p, int32_t v, int64_t n) {
 // ---- stable compaction of edges with score > cut ----
 __global__ void __launch_bounds__(kScanThreads) compact_count_kernel(const float* __restrict__ score, const int32_t* __restrict__ n_dev,
                                                                      int64_t n_cap, float cut, int32_t* __restrict__ block_sums) {
+  TRK_GRID_DEP_WAIT();
   __shared__ int total;
   const int64_t n = min((int64_t)*n_dev, n_cap);
   const int64_t base = (int64_t)blockIdx.x * kScanTile + (int64_t)threadIdx.x * kScanItems;
@@ -106,6 +111,7 @@ __global__ void __launch_bounds__(kScanThreads) compact_write_kernel(const int32
                                                                      int64_t n_blocks, int32_t* __restrict__ out_src,
                                                                      int32_t* __restrict__ out_dst, int64_t out_cap,
                                                                      int32_t* __restrict__ count_out, int32_t* __restrict__ overflow_flag) {
+  TRK_GRID_DEP_WAIT();
   __shared__ int total;
   const int64_t n = min((int64_t)*n_dev, n_cap);
   const int64_t base = (int64_t)blockIdx.x * kScanTile + (int64_t)threadIdx.x * kScanItems;
