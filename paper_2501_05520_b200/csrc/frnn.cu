@@ -29,7 +29,8 @@ __device__ __forceinline__ int float_to_ordered(float f) {
 }
 __device__ __forceinline__ float ordered_to_float(int i) { return __int_as_float(i >= 0 ? i : i ^ 0x7fffffff); }
 
-__global__ void frnn_reset_kernel(int32_t* __restrict__ bbox, int32_t* __restrict__ cell_count, int64_t n_cells_plus1) {
+__global__ void frnn_reset_kernel(int32_t* __restrict__ bbox, int32_t* __restrict__ cell_count, int32_t* __restrict__ cell_fill,
+                                  int64_t n_cells_plus1) {
   TRK_GRID_DEP_WAIT();
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i < 3) {
@@ -42,6 +43,7 @@ __global__ void frnn_reset_kernel(int32_t* __restrict__ bbox, int32_t* __restric
     bbox[8] = 0;                   // max |e_k| over all hits and coordinates (bits of a non-negative float)
   }
   if (i < n_cells_plus1) cell_count[i] = 0;
+  if (i + 1 < n_cells_plus1) cell_fill[i] = 0;
 }
 
 // proj[i] = P^T e_i  (or the first g coordinates), and the global bounding box.
@@ -560,12 +562,12 @@ trk_status frnn_build(trk_ctx* ctx, const float* emb, const float* hits, int64_t
   if (n <= 0) return fail(ctx, TRK_ERR_INVALID_ARG, "frnn: empty input");
   const unsigned nb = (unsigned)ceil_div(n, 256);
   // only the cells of this call's events are touched
-  TRK_LAUNCH(ctx, frnn_reset_kernel, (unsigned)ceil_div(n_cells + 1, 256), 256, 0, st, ctx->bbox, ctx->cell_count, n_cells + 1);
+  TRK_LAUNCH(ctx, frnn_reset_kernel, (unsigned)ceil_div(n_cells + 1, 256), 256, 0, st, ctx->bbox, ctx->cell_count, ctx->cell_fill,
+             n_cells + 1);
   TRK_LAUNCH(ctx, frnn_project_kernel, nb, 256, 0, st, emb, hits, ctx->d_e, ctx->grid_proj, g, ctx->proj, ctx->bbox, n);
   TRK_LAUNCH(ctx, frnn_grid_setup_kernel, 1, 32, 0, st, ctx->bbox, ctx->cfg.frnn_radius, g, G, ctx->grid);
   TRK_LAUNCH(ctx, frnn_count_kernel, nb, 256, 0, st, ctx->proj, hits, ctx->ev_of_hit, ctx->grid, ctx->cell_of_hit, ctx->cell_count, n);
   TRK_TRY(exclusive_scan_i32(ctx, ctx->cell_count, ctx->cell_start, n_cells, ctx->scan_tmp, st));
-  TRK_TRY(fill_i32(ctx, ctx->cell_fill, 0, n_cells, st));
   TRK_LAUNCH(ctx, frnn_scatter_kernel, nb, 256, 0, st, emb, hits, ctx->d_e, ctx->d_e_pad, ctx->cell_of_hit, ctx->cell_start,
              ctx->cell_fill, ctx->semb, ctx->smeta, ctx->proj, ctx->sproj, n);
   const double r = (double)ctx->cfg.frnn_radius;

@@ -42,7 +42,7 @@ __global__ void place_keys_kernel(const int32_t* __restrict__ key, const int32_t
   const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (k < n_edges) {
     const int v = key[k];
-    perm[rowptr[v] + atomicAdd(&fill[v], 1)] = (int32_t)k;
+    perm[rowptr[v] + atomicSub(&fill[v], 1) - 1] = (int32_t)k;   // fill still holds the segment's count: back to front
   }
 }
 
@@ -249,7 +249,6 @@ trk_status build_gnn_csr(trk_ctx* ctx, const float* hits, const int32_t* src, co
   TRK_TRY(fill_i32(ctx, ctx->in_fill, 0, n_nodes + 1, st));
   TRK_LAUNCH(ctx, count_keys_kernel, eb, 256, 0, st, dst, n_edges_dev, n_edges_cap, ctx->in_fill);
   TRK_TRY(exclusive_scan_i32(ctx, ctx->in_fill, ctx->in_rowptr, n_nodes, ctx->scan_tmp, st));
-  TRK_TRY(fill_i32(ctx, ctx->in_fill, 0, n_nodes, st));
   TRK_LAUNCH(ctx, place_keys_kernel, eb, 256, 0, st, dst, n_edges_dev, n_edges_cap, ctx->in_rowptr, ctx->in_fill, ctx->in_perm);
   TRK_LAUNCH(ctx, sort_segments_kernel, (unsigned)ceil_div(n_nodes * 32, 256), 256, 0, st, ctx->in_rowptr, ctx->in_perm, n_nodes);
   if (n_nodes > 0)
