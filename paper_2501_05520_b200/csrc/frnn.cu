@@ -68,34 +68,38 @@ __global__ void frnn_project_kernel(const float* __restrict__ emb, const float* 
     proj[i * 3 + 1] = p[1];
     proj[i * 3 + 2] = p[2];
   }
-  // warp-reduce then one atomic per warp and axis
+  // warp-reduce, then block-reduce through shared memory: ONE set of nine atomics per block (the atomics all hit the same nine
+  // words, so their number is the kernel's run time: 22 us with one set per warp)
+  __shared__ int s_red[9][8];
+  const int lane = threadIdx.x & 31, wrp = threadIdx.x >> 5;
+  int red[9];
   for (int a = 0; a < 3; ++a) {
-    int lo = i < n ? float_to_ordered(p[a]) : 0x7fffffff;
-    int hi = i < n ? float_to_ordered(p[a]) : (int)0x80000000;
-    for (int o = 16; o > 0; o >>= 1) {
-      lo = min(lo, __shfl_xor_sync(0xffffffffu, lo, o));
-      hi = max(hi, __shfl_xor_sync(0xffffffffu, hi, o));
-    }
-    if ((threadIdx.x & 31) == 0) {
-      atomicMin(&bbox[a], lo);
-      atomicMax(&bbox[3 + a], hi);
-    }
+    red[a] = i < n ? float_to_ordered(p[a]) : 0x7fffffff;            // min
+    red[3 + a] = i < n ? float_to_ordered(p[a]) : (int)0x80000000;   // max
   }
   {
     const int key = i < n ? float_to_ordered(hits[i * 3]) : 0;
-    int lo = i < n ? key : 0x7fffffff;
-    int hi = i < n ? key : (int)0x80000000;
+    red[6] = i < n ? key : 0x7fffffff;
+    red[7] = i < n ? key : (int)0x80000000;
+    red[8] = __float_as_int(emax);       // non-negative floats order like their bit patterns
+  }
+#pragma unroll
+  for (int q = 0; q < 9; ++q) {
+    const bool is_min = q < 3 || q == 6;
     for (int o = 16; o > 0; o >>= 1) {
-      lo = min(lo, __shfl_xor_sync(0xffffffffu, lo, o));
-      hi = max(hi, __shfl_xor_sync(0xffffffffu, hi, o));
+      const int other = __shfl_xor_sync(0xffffffffu, red[q], o);
+      red[q] = is_min ? min(red[q], other) : max(red[q], other);
     }
-    int em = __float_as_int(emax);       // non-negative floats order like their bit patterns
-    for (int o = 16; o > 0; o >>= 1) em = max(em, __shfl_xor_sync(0xffffffffu, em, o));
-    if ((threadIdx.x & 31) == 0) {
-      atomicMin(&bbox[6], lo);
-      atomicMax(&bbox[7], hi);
-      atomicMax(&bbox[8], em);
-    }
+    if (lane == 0) s_red[q][wrp] = red[q];
+  }
+  __syncthreads();
+  if (threadIdx.x < 9) {
+    const int q = threadIdx.x;
+    const bool is_min = q < 3 || q == 6;
+    int v = s_red[q][0];
+    for (int w = 1; w < (int)(blockDim.x >> 5); ++w) v = is_min ? min(v, s_red[q][w]) : max(v, s_red[q][w]);
+    if (is_min) atomicMin(&bbox[q], v);
+    else atomicMax(&bbox[q], v);
   }
 }
 
