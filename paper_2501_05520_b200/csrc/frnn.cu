@@ -451,16 +451,18 @@ frnn_search_kernel(const float* __restrict__ semb, const float4* __restrict__ sm
     for (int base = lo; base < hi; base += 64) {
       const int pos0 = base + lane, pos1 = base + 32 + lane;
       bool pre0 = false, pre1 = false;
-      float4 cp0, cp1;
+      float4 cp0 = make_float4(0.f, 0.f, 0.f, 0.f), cp1 = cp0;
       if (pos0 < hi) cp0 = __ldg(sproj + pos0);
       if (pos1 < hi) cp1 = __ldg(sproj + pos1);
-      if (pos0 < hi) {
-        const float tx = qp.x - cp0.x, ty = qp.y - cp0.y, tz = qp.z - cp0.z;
-        pre0 = fmaf(tz, tz, fmaf(ty, ty, tx * tx)) <= r2_proj;
-      }
-      if (pos1 < hi) {
-        const float tx = qp.x - cp1.x, ty = qp.y - cp1.y, tz = qp.z - cp1.z;
-        pre1 = fmaf(tz, tz, fmaf(ty, ty, tx * tx)) <= r2_proj;
+      {
+        // both candidates of a lane in packed fp32x2 arithmetic: the same subtractions and fused multiply-adds, component by
+        // component, as the scalar form (stale registers of an out-of-range position are masked by the range test)
+        const float2 tx = __fadd2_rn(make_float2(qp.x, qp.x), make_float2(-cp0.x, -cp1.x));
+        const float2 ty = __fadd2_rn(make_float2(qp.y, qp.y), make_float2(-cp0.y, -cp1.y));
+        const float2 tz = __fadd2_rn(make_float2(qp.z, qp.z), make_float2(-cp0.z, -cp1.z));
+        const float2 d = __ffma2_rn(tz, tz, __ffma2_rn(ty, ty, __fmul2_rn(tx, tx)));
+        pre0 = pos0 < hi && d.x <= r2_proj;
+        pre1 = pos1 < hi && d.y <= r2_proj;
       }
       const unsigned m0 = __ballot_sync(0xffffffffu, pre0), m1 = __ballot_sync(0xffffffffu, pre1);
       if (m0 | m1) {
