@@ -52,8 +52,7 @@ struct FusedParams {
   int64_t ldx;
   const int32_t* src;
   const int32_t* dst;
-  // the two bias vectors travel BY VALUE: kernel parameters live in the constant bank, so the epilogues read them with LDC
-  // (warp-uniform addresses) instead of competing with the tiles for the shared-memory / L1 data pipe
+  // the two bias vectors travel BY VALUE (constant bank); the prologue turns them into the weight blocks of the bias K steps
   float b1[kH];
   float b2[kH];
   int use_ln;
@@ -131,6 +130,11 @@ __device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&r)[32
       "r"(r[31])
       : "memory");
 }
+__device__ __forceinline__ void tmem_st8(uint32_t taddr, const uint32_t (&r)[8]) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"r"(taddr), "r"(r[0]), "r"(r[1]),
+               "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7])
+               : "memory");
+}
 __device__ __forceinline__ void tmem_st_wait() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 // D[tmem] (+)= A[tmem] * B[smem desc]^T: the A operand (128 rows per CTA = TMEM lanes, K-major, two bf16 per 32-bit column)
 // is read from tensor memory, so a layer's output can feed the next layer without a trip through shared memory
@@ -152,9 +156,16 @@ constexpr int kOffW2 = kOffW1 + 6 * kWKB;       // 2 K blocks of W2
 constexpr int kOffRing = kOffW2 + 2 * kWKB;     // 4 K blocks: h_src (2), h_dst (2)
 constexpr int kOffEOp = kOffRing + 4 * kKB;     // 2 K blocks: the e tile as layer-1 operand
 constexpr int kOffRes = kOffEOp + 2 * kKB;      // 2 K blocks: staging of the bf16 update for the TMA (reduce-add) store
-constexpr int kOffXD = kOffRes + 2 * kKB;       // kDecode: partial dots of the upper half rows, 128 fp32
-constexpr int kOffVec = kOffXD + kTileRows * 4; // b1, b2, w_out: 3 x 128 fp32
-constexpr int kOffX1 = kOffVec + 3 * kH * 4;     // epilogue 1: one float2 per row, half-row statistics one way, coefficients back
+// The biases ride on the tensor core: one extra K step per layer multiplies a constant operand whose first two columns are 1
+// with a weight block whose first two columns are hi(b) = bf16(b) and lo(b) = bf16(b - hi(b)) (b = hi + lo to 2^-17 relative,
+// the products with 1 are exact, the accumulator is fp32).  The epilogues then read accumulators that already hold
+// W x + b: no bias loads (16 LDC.128 per thread and tile) and no bias adds (32 packed adds) in their instruction streams.
+constexpr int kOffOnes = kOffRes + 2 * kKB;     // 1 K block: A operand of the bias step of layer 1 (columns 0, 1 = 1.0)
+constexpr int kOffB1 = kOffOnes + kKB;          // 1 K block of this CTA's 64 output rows: columns 0, 1 = hi(b1), lo(b1)
+constexpr int kOffB2 = kOffB1 + kWKB;           // the same for layer 2 (its A operand, the ones, sits next to T in tensor memory)
+constexpr int kOffXD = kOffB2 + kWKB;           // kDecode: partial dots of the upper half rows, 128 fp32
+constexpr int kOffVec = kOffXD + kTileRows * 4; // w_out: 128 fp32
+constexpr int kOffX1 = kOffVec + kH * 4;        // epilogue 1: one float2 per row, half-row statistics one way, coefficients back
 constexpr int kOffBar = kOffX1 + kTileRows * 8;
 constexpr int kSmemFused = kOffBar + 256;
 static_assert(kSmemFused <= 232448, "shared memory budget of one CTA");
@@ -177,24 +188,17 @@ __device__ __forceinline__ void named_bar_sync(int id, int threads) {
   asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(threads) : "memory");
 }
 
-// Half an accumulator row (this thread's TMEM lane, 64 fp32 columns from `taddr`) + bias -> 32 packed pairs, and the
+// Half an accumulator row (this thread's TMEM lane, 64 fp32 columns from `taddr`; the bias is in it already) -> 32 packed pairs, and the
 // partial sum / sum of squares of those 64 values.
-template <bool BIAS_GLOBAL>
-__device__ __forceinline__ void load_half(uint32_t taddr, const float* __restrict__ bias, float2 (&x)[32], float& ps, float& pq) {
+__device__ __forceinline__ void load_half(uint32_t taddr, float2 (&x)[32], float& ps, float& pq) {
   uint32_t u0[32], u1[32];
   tmem_ld32(taddr, u0);
   tmem_ld32(taddr + 32, u1);
-  const float4* b4 = reinterpret_cast<const float4*>(bias);
-  float4 bb[16];
-#pragma unroll
-  for (int j = 0; j < 16; ++j) bb[j] = BIAS_GLOBAL ? __ldg(b4 + j) : b4[j];
   tmem_ld_wait();
 #pragma unroll
-  for (int i = 0; i < 32; i += 4) {
-    x[i / 2] = __fadd2_rn(f2(__uint_as_float(u0[i]), __uint_as_float(u0[i + 1])), f2(bb[i / 4].x, bb[i / 4].y));
-    x[i / 2 + 1] = __fadd2_rn(f2(__uint_as_float(u0[i + 2]), __uint_as_float(u0[i + 3])), f2(bb[i / 4].z, bb[i / 4].w));
-    x[16 + i / 2] = __fadd2_rn(f2(__uint_as_float(u1[i]), __uint_as_float(u1[i + 1])), f2(bb[8 + i / 4].x, bb[8 + i / 4].y));
-    x[16 + i / 2 + 1] = __fadd2_rn(f2(__uint_as_float(u1[i + 2]), __uint_as_float(u1[i + 3])), f2(bb[8 + i / 4].z, bb[8 + i / 4].w));
+  for (int i = 0; i < 32; i += 2) {
+    x[i / 2] = f2(__uint_as_float(u0[i]), __uint_as_float(u0[i + 1]));
+    x[16 + i / 2] = f2(__uint_as_float(u1[i]), __uint_as_float(u1[i + 1]));
   }
   float2 s0 = f2(0.f, 0.f), s1 = s0, q0 = s0, q1 = s0;
 #pragma unroll
@@ -227,9 +231,7 @@ gnn_fused_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constant
   extern __shared__ __align__(1024) uint8_t smem[];
   if ((smem_u32(smem) & 1023u) != 0) __trap();   // the swizzled operand layout needs the 1024-byte alignment declared above
   Bars* bar = reinterpret_cast<Bars*>(smem + kOffBar);
-  const float* sb1 = p.b1;
-  const float* sb2 = p.b2;
-  float* swo = reinterpret_cast<float*>(smem + kOffVec) + 2 * kH;
+  float* swo = reinterpret_cast<float*>(smem + kOffVec);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const uint32_t rank = cluster_ctarank();
   const bool leader = rank == 0;
@@ -272,6 +274,26 @@ gnn_fused_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constant
   if (threadIdx.x >= 128 && threadIdx.x < 128 + kH) {
     const int c = threadIdx.x - 128;
     swo[c] = MODE == kDecode ? p.w_out[c] : 0.f;
+  }
+  {
+    // bias operands in the 128-byte-swizzled K-major layout (16-byte chunk c of row r lives at chunk position c ^ (r & 7));
+    // only the first K step (chunks 0 and 1) is ever read
+    const int t = threadIdx.x;
+    if (t < kTileRows) {
+      uint8_t* row = smem + kOffOnes + t * 128;
+      *reinterpret_cast<uint4*>(row + ((0 ^ (t & 7)) << 4)) = make_uint4(0x3F803F80u, 0u, 0u, 0u);   // bf16 (1, 1, 0, 0, 0, 0, 0, 0)
+      *reinterpret_cast<uint4*>(row + ((1 ^ (t & 7)) << 4)) = make_uint4(0u, 0u, 0u, 0u);
+    } else if (t < kTileRows + 2 * 64) {
+      const int l = (t - kTileRows) >> 6, r = (t - kTileRows) & 63;            // layer, output row of this CTA's half
+      const float b = (l == 0 ? p.b1 : p.b2)[(int)rank * 64 + r];
+      const __nv_bfloat16 hi = __float2bfloat16_rn(b);
+      const __nv_bfloat16 lo = __float2bfloat16_rn(b - __bfloat162float(hi));
+      uint8_t* row = smem + (l == 0 ? kOffB1 : kOffB2) + r * 128;
+      *reinterpret_cast<uint4*>(row + ((0 ^ (r & 7)) << 4)) =
+          make_uint4((uint32_t)__bfloat16_as_ushort(hi) | ((uint32_t)__bfloat16_as_ushort(lo) << 16), 0u, 0u, 0u);
+      *reinterpret_cast<uint4*>(row + ((1 ^ (r & 7)) << 4)) = make_uint4(0u, 0u, 0u, 0u);
+    }
+    fence_proxy_async();
   }
   __syncthreads();
   mbar_wait(&bar->w_full, 0);
@@ -346,6 +368,8 @@ gnn_fused_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constant
               const uint64_t bdesc = make_smem_desc(sbase + kOffW2 + (k / 4) * kWKB) + (uint64_t)((k % 4) * 2);
               tc_mma_bf16_pair_ts(d, t + (uint32_t)(k * (UMMA_K / 2)), bdesc, idesc, k != 0 ? 1u : 0u);
             }
+            // + b2: the ones sit in the eight columns after T (K indices 128..143), written by epilogue 1 with T
+            tc_mma_bf16_pair_ts(d, t + (uint32_t)(kH / 2), make_smem_desc(sbase + kOffB2), idesc, 1u);
             tc_commit_pair(&bar->a1empty[b]);     // acc1[b] (and the T in it) may be overwritten by layer 1 of tile n2 + 2
             tc_commit_pair(&bar->a2full[b]);
             ++n2;
@@ -362,6 +386,7 @@ gnn_fused_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constant
               if constexpr (MODE == kEncode) {
                 // one K step: the 16 columns that hold the hi / lo feature pairs
                 tc_mma_bf16_pair(d, make_smem_desc(sbase + kOffRing), make_smem_desc(sbase + kOffW1), idesc, 0u);
+                tc_mma_bf16_pair(d, make_smem_desc(sbase + kOffOnes), make_smem_desc(sbase + kOffB1), idesc, 1u);   // + b1
                 tc_commit_pair(&bar->gempty[0]);
                 tc_commit_pair(&bar->a1full[b]);
                 ++n1;
@@ -386,6 +411,7 @@ gnn_fused_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constant
               tc_fence_after();
               progressed = true;
               for (int kb = 0; kb < 2; ++kb) kblock(d, sbase + kOffEOp + kb * kKB, sbase + kOffW1 + (kbE + kb) * kWKB, false);
+              tc_mma_bf16_pair(d, make_smem_desc(sbase + kOffOnes), make_smem_desc(sbase + kOffB1), idesc, 1u);     // + b1
               tc_commit_pair(&bar->eopempty);
               tc_commit_pair(&bar->a1full[b]);
               stage1 = 0;
@@ -481,7 +507,7 @@ gnn_fused_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constant
       tc_fence_after();
       float2 x[32];
       float ps, pq;
-      load_half<false>(tmem_base + ((uint32_t)(quad * 32) << 16) + (uint32_t)(b * kH + half * 64), sb1 + half * 64, x, ps, pq);
+      load_half(tmem_base + ((uint32_t)(quad * 32) << 16) + (uint32_t)(b * kH + half * 64), x, ps, pq);
       tc_fence_before();
       if (!kTwoLayers) {
         __syncwarp();
@@ -532,6 +558,11 @@ gnn_fused_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constant
           w[i] = pack_relu_bf16(v.x, v.y);
         }
         tmem_st32(tmem_base + ((uint32_t)(quad * 32) << 16) + (uint32_t)(b * kH + half * 32), w);
+        if (half == 1) {
+          // the A operand of layer 2's bias step: K indices 128, 129 = 1.0 (one 32-bit column), 130..143 = 0
+          const uint32_t ones[8] = {0x3F803F80u, 0u, 0u, 0u, 0u, 0u, 0u, 0u};
+          tmem_st8(tmem_base + ((uint32_t)(quad * 32) << 16) + (uint32_t)(b * kH + kH / 2), ones);
+        }
         tmem_st_wait();
         tc_fence_before();
         __syncwarp();
@@ -554,7 +585,7 @@ gnn_fused_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constant
         tc_fence_after();
         float2 x[32];
         float ps, pq;
-        load_half<false>(tmem_base + ((uint32_t)(quad * 32) << 16) + (uint32_t)(2 * kH + b * kH + half * 64), sb2 + half * 64, x, ps, pq);
+        load_half(tmem_base + ((uint32_t)(quad * 32) << 16) + (uint32_t)(2 * kH + b * kH + half * 64), x, ps, pq);
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive_remote(b == 0 ? a2empty0 : a2empty1);
