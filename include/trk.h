@@ -206,6 +206,27 @@ trk_status trk_stage_gnn(trk_ctx* ctx, const float* hits, int64_t n, const int32
 trk_status trk_stage_cc(trk_ctx* ctx, int64_t n, const int32_t* src, const int32_t* dst, const float* score,
                         int64_t n_edges, float cut, int32_t* labels, void* cuda_stream);
 
+/* S5 without a context and without any allocation (csrc/cc_noalloc.cu).
+ * For callers that may not allocate device memory: a backend that lives inside a memory budget fixed by the serving
+ * framework that owns the GPU, code running where cudaMalloc is forbidden or would stall the
+ * device (while a stream capture is open elsewhere in the process, inside a stream host callback), and loops that cannot
+ * afford the implicit synchronisation of cudaMalloc / cudaFree.  trk_create allocates the whole workspace, so none of
+ * the ctx entry points is usable there; this one computes the same labels as trk_stage_cc (label = smallest hit index of
+ * the component, edges with score > cut kept) with the union-find parent array in a fixed array inside the library image.
+ *   - runs on the caller's CURRENT device; src/dst/score [n_edges] and labels [n] are DEVICE memory of that device and
+ *     stay caller-owned; only kernels are enqueued on cuda_stream (no cudaMalloc, cudaFree, memset, sync or library call).
+ *   - limit: n <= TRK_CC_NOALLOC_MAX_HITS.  A larger n is refused with TRK_ERR_CAPACITY before anything is enqueued
+ *     (text in trk_last_error(NULL)).  The array costs TRK_CC_NOALLOC_MAX_HITS x 4 bytes = 4 MiB on every GPU that
+ *     loads libtrk.so, used or not, until the process exits.
+ *   - the first call on a device looks up the device address of that array (cudaGetSymbolAddress, which may also make
+ *     the runtime load the module): make that first call before starting any stream capture.
+ *   - all calls on a device share the one array, and it keeps what the previous call left there; each call re-initialises
+ *     the n entries it uses, so results never depend on earlier calls -- but two calls that overlap on the same GPU
+ *     (different streams or threads) race on it.  Order them on one stream or with events.                            */
+#define TRK_CC_NOALLOC_MAX_HITS 1048576
+trk_status trk_cc_noalloc(int64_t n, const int32_t* src, const int32_t* dst, const float* score, int64_t n_edges,
+                          float cut, int32_t* labels, void* cuda_stream);
+
 /* S6: track lists from labels [n] (as S5 writes them: label = smallest hit index of the component).
  * track_offsets [capacity+1], track_hits [n], track_counts [3] = {T, hits in tracks, overflow}.    */
 trk_status trk_stage_tracks(trk_ctx* ctx, const int32_t* labels, int64_t n, int32_t min_hits, int32_t* track_offsets,

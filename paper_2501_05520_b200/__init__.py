@@ -3,7 +3,7 @@
     from paper_2501_05520_b200 import Trk
 The CUDA library is loaded lazily by `binding.lib()`; it is required -- there is no CPU fallback.
 """
-from .binding import EXPORTS, LIB_PATH, Trk, TrkError, gemm_bf16, lib  # noqa: F401
+from .binding import CC_NOALLOC_MAX_HITS, EXPORTS, LIB_PATH, Trk, TrkError, cc_noalloc, gemm_bf16, lib  # noqa: F401
 
 
 def trk_from_config(cfg: dict, model: dict, calib: dict, *, max_hits: int, max_events: int = 1, max_cand_edges=None,

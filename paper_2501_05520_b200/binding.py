@@ -20,8 +20,9 @@ EXPORTS = [
     "trk_create", "trk_infer", "trk_destroy", "trk_infer_host", "trk_status_string", "trk_last_error",
     "trk_workspace_bytes", "trk_last_launch_count", "trk_stage_embed", "trk_stage_frnn", "trk_stage_filter",
     "trk_stage_compact", "trk_stage_gnn", "trk_stage_cc", "trk_gemm_bf16", "trk_profile_enable", "trk_profile_stage_ms", "trk_profile_kernel_ms",
-    "trk_set_option", "trk_stage_tracks", "trk_infer_host_tracks",
+    "trk_set_option", "trk_stage_tracks", "trk_infer_host_tracks", "trk_cc_noalloc",
 ]
+CC_NOALLOC_MAX_HITS = 1048576  # TRK_CC_NOALLOC_MAX_HITS of include/trk.h
 
 _f32p = C.POINTER(C.c_float)
 _i32p = C.POINTER(C.c_int32)
@@ -98,6 +99,7 @@ def lib():
     L.trk_profile_kernel_ms.argtypes = [vp, _f32p, i32, _i32p, C.POINTER(i64)]
     L.trk_stage_tracks.argtypes = [vp, vp, i64, i32, vp, i64, vp, vp, vp]
     L.trk_infer_host_tracks.argtypes = [vp, i32, _i32p, vp, vp, vp, vp, vp]
+    L.trk_cc_noalloc.argtypes = [i64, vp, vp, vp, i64, C.c_float, vp, vp]
     for name in EXPORTS:
         if getattr(L, name).restype is C.c_int:
             getattr(L, name).restype = C.c_int
@@ -371,3 +373,15 @@ def gemm_bf16(a, w, bias, relu=True, pair=True, stream=None):
     if st != 0:
         raise TrkError(st, lib().trk_last_error(None).decode())
     return out
+
+
+def cc_noalloc(n, src, dst, score, cut, labels, stream=None):
+    """trk_cc_noalloc: S5 labels for callers that must not allocate device memory (a backend inside a fixed memory budget,
+    code where cudaMalloc is forbidden or stalls the device).  No context: the union-find scratch is a fixed array inside
+    libtrk.so, so n <= CC_NOALLOC_MAX_HITS.  `labels` (CUDA int32 [n]) is the caller's buffer and is written in place --
+    this wrapper allocates nothing either.  Runs on the current device; calls that overlap on one GPU race on the scratch."""
+    st = lib().trk_cc_noalloc(int(n), _ptr(src), _ptr(dst), _ptr(score), 0 if src is None else src.numel(), float(cut), _ptr(labels),
+                              _stream_ptr(stream))
+    if st != 0:
+        raise TrkError(st, lib().trk_last_error(None).decode())
+    return labels
