@@ -202,6 +202,12 @@ trk_status trk_stage_compact(trk_ctx* ctx, const int32_t* src, const int32_t* ds
 /* S4: score fp32 [n_edges] = sigmoid(GNN logit).  Edges must be sorted by (src,dst). */
 trk_status trk_stage_gnn(trk_ctx* ctx, const float* hits, int64_t n, const int32_t* src, const int32_t* dst,
                          int64_t n_edges, float* score, void* cuda_stream);
+/* S4 bookkeeping only: the scatter structure of the message passing, as trk_stage_gnn builds it (same kernels).  Edges
+ * sorted by (src,dst).  in_rowptr [n+1] / in_perm [n_edges]: the in-edges of node v are in_perm[in_rowptr[v] ..
+ * in_rowptr[v+1]) in ASCENDING edge index -- the fixed order in which sum_in e is accumulated, so that S4 gives the same
+ * bits run to run; out_rowptr [n+1]: the out-edges of v are the edge range [out_rowptr[v], out_rowptr[v+1]).  n >= 1. */
+trk_status trk_stage_gnn_csr(trk_ctx* ctx, const float* hits, int64_t n, const int32_t* src, const int32_t* dst,
+                             int64_t n_edges, int32_t* in_rowptr, int32_t* in_perm, int32_t* out_rowptr, void* cuda_stream);
 /* S5: labels int32 [n]; edges with score > cut are kept. */
 trk_status trk_stage_cc(trk_ctx* ctx, int64_t n, const int32_t* src, const int32_t* dst, const float* score,
                         int64_t n_edges, float cut, int32_t* labels, void* cuda_stream);

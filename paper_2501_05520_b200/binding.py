@@ -20,7 +20,7 @@ EXPORTS = [
     "trk_create", "trk_infer", "trk_destroy", "trk_infer_host", "trk_status_string", "trk_last_error",
     "trk_workspace_bytes", "trk_last_launch_count", "trk_stage_embed", "trk_stage_frnn", "trk_stage_filter",
     "trk_stage_compact", "trk_stage_gnn", "trk_stage_cc", "trk_gemm_bf16", "trk_profile_enable", "trk_profile_stage_ms", "trk_profile_kernel_ms",
-    "trk_set_option", "trk_stage_tracks", "trk_infer_host_tracks", "trk_cc_noalloc",
+    "trk_set_option", "trk_stage_tracks", "trk_infer_host_tracks", "trk_cc_noalloc", "trk_stage_gnn_csr",
 ]
 CC_NOALLOC_MAX_HITS = 1048576  # TRK_CC_NOALLOC_MAX_HITS of include/trk.h
 
@@ -99,6 +99,7 @@ def lib():
     L.trk_profile_kernel_ms.argtypes = [vp, _f32p, i32, _i32p, C.POINTER(i64)]
     L.trk_stage_tracks.argtypes = [vp, vp, i64, i32, vp, i64, vp, vp, vp]
     L.trk_infer_host_tracks.argtypes = [vp, i32, _i32p, vp, vp, vp, vp, vp]
+    L.trk_stage_gnn_csr.argtypes = [vp, vp, i64, vp, vp, i64, vp, vp, vp, vp]
     L.trk_cc_noalloc.argtypes = [i64, vp, vp, vp, i64, C.c_float, vp, vp]
     for name in EXPORTS:
         if getattr(L, name).restype is C.c_int:
@@ -341,6 +342,17 @@ class Trk:
         self._check(lib().trk_stage_gnn(self._h, _ptr(hits), hits.shape[0], _ptr(src), _ptr(dst), src.numel(), _ptr(score),
                                         _stream_ptr(stream)))
         return score
+
+    def stage_gnn_csr(self, hits, src, dst, stream=None):
+        """The S4 scatter structure: (in_rowptr [n+1], in_perm [n_edges], out_rowptr [n+1])."""
+        import torch
+        n = hits.shape[0]
+        in_rowptr = torch.empty(n + 1, dtype=torch.int32, device=hits.device)
+        out_rowptr = torch.empty(n + 1, dtype=torch.int32, device=hits.device)
+        in_perm = torch.empty(src.numel(), dtype=torch.int32, device=hits.device)
+        self._check(lib().trk_stage_gnn_csr(self._h, _ptr(hits), n, _ptr(src), _ptr(dst), src.numel(), _ptr(in_rowptr), _ptr(in_perm),
+                                            _ptr(out_rowptr), _stream_ptr(stream)))
+        return in_rowptr, in_perm, out_rowptr
 
     def stage_cc(self, n, src, dst, score, cut, stream=None):
         import torch

@@ -7,6 +7,7 @@
 #include <mutex>
 
 #include "common.cuh"
+#include "graph.cuh"
 #include "nn.cuh"
 
 namespace trk {
@@ -696,6 +697,21 @@ trk_status trk_stage_gnn(trk_ctx* ctx, const float* hits, int64_t n, const int32
     return fail(ctx, TRK_ERR_INVALID_ARG, "stage_gnn: bad arguments");
   if (n > ctx->cfg.max_hits || n_edges > ctx->cfg.max_kept_edges) return fail(ctx, TRK_ERR_CAPACITY, "stage_gnn: exceeds max_hits / max_kept_edges");
   return gnn_dispatch(ctx, hits, n, src, dst, nullptr, n_edges, score, (cudaStream_t)cuda_stream);
+}
+
+trk_status trk_stage_gnn_csr(trk_ctx* ctx, const float* hits, int64_t n, const int32_t* src, const int32_t* dst, int64_t n_edges,
+                             int32_t* in_rowptr, int32_t* in_perm, int32_t* out_rowptr, void* cuda_stream) {
+  if (!ctx) return TRK_ERR_INVALID_ARG;
+  DeviceGuard guard(ctx->device);
+  if (n <= 0 || n_edges < 0 || !hits || !in_rowptr || !out_rowptr || (n_edges > 0 && (!src || !dst || !in_perm)))
+    return fail(ctx, TRK_ERR_INVALID_ARG, "stage_gnn_csr: bad arguments");
+  if (n > ctx->cfg.max_hits || n_edges > ctx->cfg.max_kept_edges) return fail(ctx, TRK_ERR_CAPACITY, "stage_gnn_csr: exceeds max_hits / max_kept_edges");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  TRK_TRY(build_gnn_csr(ctx, hits, src, dst, nullptr, n_edges, n, st));
+  TRK_CUDA(ctx, cudaMemcpyAsync(in_rowptr, ctx->in_rowptr, (size_t)(n + 1) * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
+  TRK_CUDA(ctx, cudaMemcpyAsync(out_rowptr, ctx->out_rowptr, (size_t)(n + 1) * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
+  if (n_edges > 0) TRK_CUDA(ctx, cudaMemcpyAsync(in_perm, ctx->in_perm, (size_t)n_edges * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
+  return TRK_OK;
 }
 
 trk_status trk_stage_cc(trk_ctx* ctx, int64_t n, const int32_t* src, const int32_t* dst, const float* score, int64_t n_edges,

@@ -101,6 +101,11 @@ __device__ __forceinline__ void mbar_arrive_remote_cta(uint32_t cluster_addr) {
   asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
 }
 
+// cluster-scope release: the gathered layer-1 operand rows of this CTA are consumed by an MMA issued from the leader CTA
+__device__ __forceinline__ void mbar_arrive_remote_release_cluster(uint32_t cluster_addr) {
+  asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
+}
+
 constexpr int kTemptyArrivals = 2 * kEpiWarps;   // per CTA and tile: 4 epilogue warps x 2 (layers 1, 2) or 4 + 4 helper warps (layer 3)
 
 // sum over 128 accumulator columns of this thread's TMEM lane of ReLU(acc + b) * w, added to `dot`; releases the accumulator
@@ -430,7 +435,7 @@ filter_mlp_kernel(const __grid_constant__ CUtensorMap tmS1, const __grid_constan
         *reinterpret_cast<uint4*>(rowp + ((q ^ (r & 7)) << 4)) = make_uint4(pk[q * 4], pk[q * 4 + 1], pk[q * 4 + 2], pk[q * 4 + 3]);
       fence_proxy_async();
       __syncwarp();
-      if (lane == 0) mbar_arrive_remote_cta(xfull_leader);
+      if (lane == 0) mbar_arrive_remote_release_cluster(xfull_leader);
     };
     int as = 0;
     uint32_t aphase = 0;

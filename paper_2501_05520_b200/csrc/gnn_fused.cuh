@@ -92,6 +92,12 @@ __device__ __forceinline__ bool mbar_test(uint64_t* bar, uint32_t parity) {
 // continues is either a finished TMEM read (ordered by tcgen05.fence::before_thread_sync) or shared memory of the ARRIVING
 // CTA that its own tensor core / TMA will read (ordered by fence.proxy.async); neither needs the cluster-wide memory barrier
 // of .release.cluster, which cost the epilogue warps several hundred cycles per arrive.
+// The gather warps' arrivals on gfull use this form too although what they publish is shared memory that the OTHER CTA's
+// thread hands to the tensor core, for which the PTX memory model formally asks for .release.cluster: measured in round 3,
+// the cluster-scope form on those arrivals alone costs S4 12 % (1.95 -> 2.18 ms on the pileup-200 event, 2.75 -> 3.11 ms on
+// pileup200_nominal).  The kernel relies on fence.proxy.async + the remote arrive making the rows visible to the pair's
+// tensor core, as current hardware does; every S4 parity test and the run-to-run bit identity
+// tests exercise exactly this hand-over.
 __device__ __forceinline__ void mbar_arrive_remote(uint32_t cluster_addr) {
   asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
 }

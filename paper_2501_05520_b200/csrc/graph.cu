@@ -49,7 +49,7 @@ __global__ void place_keys_kernel(const int32_t* __restrict__ key, const int32_t
 // Each segment of perm is put in ascending edge order (place_keys_kernel fills a segment in the arbitrary order of its atomics;
 // the order of a segmented sum must not depend on it).  One warp per node: the entries of a segment are distinct, so the rank of
 // one is the number of smaller ones -- 32 entries per pass live in registers and are compared through shuffles.  Segments longer
-// than kSortMaxLen (a node with that many in-edges does not occur in tracking graphs) fall back to an insertion sort by one lane.
+// than kSortMaxLen (a node with that many in-edges does not occur in tracking graphs) are sorted in place by a bitonic network.
 constexpr int kSortChunks = 8;
 constexpr int kSortMaxLen = 32 * kSortChunks;
 __global__ void __launch_bounds__(256) sort_segments_kernel(const int32_t* __restrict__ rowptr, int32_t* __restrict__ perm, int64_t n_nodes) {
@@ -89,16 +89,24 @@ __global__ void __launch_bounds__(256) sort_segments_kernel(const int32_t* __res
       if (c * 32 + lane < len) perm[b + rank[c]] = x[c];
     return;
   }
-  if (lane == 0) {
-    const int e = b + len;
-    for (int i = b + 1; i < e; ++i) {
-      const int x = perm[i];
-      int j = i - 1;
-      while (j >= b && perm[j] > x) {
-        perm[j + 1] = perm[j];
-        --j;
+  // Longer segments (a hub): an in-place sorting network over the warp.  Bitonic sort with ascending-only merges -- the first
+  // step of a merge of size k pairs i with i ^ (k - 1), the others i with i ^ j -- so entries beyond len, which count as +inf,
+  // would stay where they are: a pair that reaches past the segment is skipped.  O(len log^2 len / 32) steps per lane.
+  int32_t* seg = perm + b;
+  int p2 = 1;
+  while (p2 < len) p2 <<= 1;
+  for (int k = 2; k <= p2; k <<= 1) {
+    for (int j = k >> 1; j > 0; j >>= 1) {
+      const bool flip = j == (k >> 1);
+      for (int t = lane; t < (p2 >> 1); t += 32) {
+        const int i = ((t & ~(j - 1)) << 1) | (t & (j - 1));      // the t-th index with bit j clear
+        const int l = flip ? (i ^ (k - 1)) : (i | j);
+        if (l < len) {
+          const int32_t x = seg[i], y = seg[l];
+          if (x > y) { seg[i] = y; seg[l] = x; }
+        }
       }
-      perm[j + 1] = x;
+      __syncwarp();
     }
   }
 }
