@@ -292,7 +292,70 @@ def run_concurrency_scan(args):
     ev_s, ms = timed(lambda: tb.infer(hb, evb["event_offsets"], out=ob), 16)
     res["packed_batch16"] = {"events_per_s": ev_s, "ms_per_call": ms, "hits": nb}
     tb.close()
+    res["pileup200"] = scan_headline_size(args, dev)
     print(json.dumps(res))
+
+
+def scan_headline_size(args, dev):
+    """The scan at the headline size: 1, 2, 3 model instances, each on its own stream and each
+    serving its OWN pileup-200 event (seeds 0, 1, 2), then two instances with (i) one stream at high priority and (ii) the fused S3
+    kernel capped below the SM count ("filter_max_pairs") so that the other instance's S1/S2/S4/S5 can co-reside with it.
+    Per row: events/s, the mean per-request latency (event pair on the instance's stream) and the SM clock sampled during the row."""
+    import torch
+    insts = []
+    for r in range(3):
+        cfg, calib, ev, model = build_workload("pileup200", seed_offset=r)
+        t = make_trk(cfg, calib, ev, model, dev.index)
+        hits = torch.from_numpy(ev["hits"]).to(dev)
+        out = t.infer(hits, ev["event_offsets"])
+        torch.cuda.synchronize()
+        insts.append(dict(trk=t, hits=hits, off=ev["event_offsets"], out=out))
+    rounds = max(args.steps, 10)
+
+    def row(k, label, priorities=None, pairs=0):
+        streams = [torch.cuda.Stream(priority=(priorities[i] if priorities else 0)) for i in range(k)]
+        for i in range(k):
+            insts[i]["trk"].set_option("filter_max_pairs", pairs)
+        ev_pairs = [[(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(rounds)] for _ in range(k)]
+
+        def one_round(r, record):
+            for i in range(k):
+                st, x = streams[i], insts[i]
+                if record:
+                    ev_pairs[i][r][0].record(st)
+                x["trk"].infer(x["hits"], x["off"], out=x["out"], stream=st)
+                if record:
+                    ev_pairs[i][r][1].record(st)
+        for _ in range(3):
+            one_round(0, False)
+        torch.cuda.synchronize()
+        sampler = ClockSampler(dev.index)
+        t0 = torch.cuda.Event(enable_timing=True); t1 = torch.cuda.Event(enable_timing=True)
+        cur = torch.cuda.current_stream()
+        t0.record(cur)
+        for st in streams:
+            st.wait_stream(cur)
+        for r in range(rounds):            # every instance streams its requests back to back: no barrier between rounds
+            one_round(r, True)
+        for st in streams:
+            cur.wait_stream(st)
+        t1.record(cur)
+        torch.cuda.synchronize()
+        clocks = sampler.stop()
+        ms = t0.elapsed_time(t1)
+        lat = [float(np.mean([a.elapsed_time(b) for a, b in ev_pairs[i]])) for i in range(k)]
+        return {"row": label, "contexts": k, "filter_max_pairs": pairs, "events_per_s": k * rounds / (ms * 1e-3),
+                "latency_ms_per_request": [round(v, 3) for v in lat], "sm_mhz": clocks.get("sm_mhz"), "reasons": clocks.get("reasons")}
+
+    rows = [row(1, "1 instance"), row(2, "2 instances"), row(3, "3 instances"),
+            row(2, "2 instances, stream 0 high priority", priorities=[-1, 0])]
+    for pairs in (70, 66, 62, 37):
+        rows.append(row(2, f"2 instances, S3 capped at {pairs} CTA pairs", pairs=pairs))
+    rows.append(row(3, "3 instances, S3 capped at 62 CTA pairs", pairs=62))
+    for x in insts:
+        x["trk"].close()
+    return {"workload": "pileup200, instance r serves the event of seed r", "rounds": rounds, "hits": [int(x["hits"].shape[0]) for x in insts],
+            "rows": rows}
 
 
 def make_trk(cfg, calib, ev, model, device):

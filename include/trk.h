@@ -260,6 +260,8 @@ trk_status trk_gemm_bf16(const void* a, const void* w, const float* bias, void* 
  *                     of the S3 filter MLP) run their epilogue on eight warps (two per TMEM lane quadrant); 2: in addition
  *                     that layer's input rows [e_src ; e_dst] are gathered inside the GEMM kernel instead of by a separate
  *                     launch (measured slower on the pileup-200 event, so not the default); 0: four warps.
+ *   "filter_max_pairs" 0 (default): the fused S3 kernel runs one CTA pair per two SMs; v > 0: at most v pairs, which leaves SMs
+ *                     free for the other stages of another model instance on another stream (bench.py --scan).  Same scores.
  *   "gemm_row_major"  16 (default): a CTA pair of the pair GEMM walks all column tiles of one row block before the next
  *                     row block when there are at least 16 row blocks per pair (A rows re-read from L2, no DRAM
  *                     re-reads); 0: tiles in pair strides, column fastest.

@@ -741,7 +741,7 @@ trk_status trk_set_option(trk_ctx* ctx, const char* key, int64_t value) {
   if (!key) return fail(ctx, TRK_ERR_INVALID_ARG, "trk_set_option: key is NULL");
   static const struct { const char* name; int knob; } keys[] = {
       {"gemm_pair", kKnobGemmPair}, {"gnn_fused", kKnobGnnFused}, {"epi_split", kKnobEpiSplit}, {"gemm_row_major", kKnobRowMajor},
-      {"filter_fused", kKnobFilterFused}};
+      {"filter_fused", kKnobFilterFused}, {"filter_max_pairs", kKnobFilterPairs}};
   for (const auto& k : keys)
     if (std::strcmp(key, k.name) == 0) {
       ctx->knobs[k.knob] = value;

@@ -21,7 +21,7 @@ constexpr int kFilterChunkTilesPerSm = 64;  // default S3 rows per pass = 128 x 
                                             // 2.5 GB per activation buffer buys 5 launches per 1.2 M candidate edges
 
 // ---- test / tuning options (trk_set_option), per context ----
-enum { kKnobGemmPair = 0, kKnobGnnFused = 1, kKnobEpiSplit = 2, kKnobRowMajor = 3, kKnobFilterFused = 4, kKnobCount = 5 };
+enum { kKnobGemmPair = 0, kKnobGnnFused = 1, kKnobEpiSplit = 2, kKnobRowMajor = 3, kKnobFilterFused = 4, kKnobFilterPairs = 5, kKnobCount = 6 };
 
 // One Linear layer resident on the device.
 struct DevLinear {
@@ -68,7 +68,7 @@ struct trk_ctx {
   cudaStream_t own_stream = nullptr;
   std::string last_error;
   int64_t launch_count = 0;
-  int64_t knobs[trk::kKnobCount] = {1, 1, 1, 16, 1};   // gemm_pair, gnn_fused, epi_split, gemm_row_major, filter_fused (trk_set_option)
+  int64_t knobs[trk::kKnobCount] = {1, 1, 1, 16, 1, 0};   // gemm_pair, gnn_fused, epi_split, gemm_row_major, filter_fused, filter_max_pairs (trk_set_option)
   std::vector<const void*> smem_attr_set;          // kernels whose dynamic shared-memory limit has been raised on ctx->device
   bool profiling = false;
   cudaEvent_t prof_ev[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};

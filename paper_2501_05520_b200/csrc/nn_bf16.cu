@@ -444,7 +444,10 @@ static trk_status filter_forward_fused(trk_ctx* ctx, const float* feat, const in
   TRK_TRY(make_tmap(ctx, &ts2st, ctx->filter_s2, s_rows, W, W, 32));
   ff::FilterParams p{feat, src, dst, ctx->filter_u, L[0].b_f32, L[1].b_f32, L[2].b_f32, L[3].w_f32, ctx->filter_b_last, score, W};
   const tc::Rows rows{n_edges_dev, 0, n_edges_cap};
-  const unsigned grid = 2u * (unsigned)std::min<int64_t>(ceil_div(n_edges_cap, 256), n_pairs_max);
+  // "filter_max_pairs" (trk_set_option): fewer CTA pairs than the device holds leave SMs to the other stages of another
+  // model instance (a pair walks row blocks pair, pair + n_pairs, ...: the scores do not depend on the number of pairs)
+  const int64_t pair_cap = ctx->knobs[kKnobFilterPairs] > 0 ? std::min<int64_t>(ctx->knobs[kKnobFilterPairs], n_pairs_max) : n_pairs_max;
+  const unsigned grid = 2u * (unsigned)std::min<int64_t>(ceil_div(n_edges_cap, 256), pair_cap);
   // trk_profile_kernel_ms: one CUDA-event pair around the launch
   const bool kprof = ctx->profiling && n_edges_dev == &ctx->counts[0] && ctx->kprof_ev.size() >= 2;
   if (kprof) {

@@ -153,6 +153,10 @@ def test_s3_first_layer_variants_are_bit_identical():
     try:
         feat, src, dst = _dev(o["emb"]), _dev(o["cand_src"]), _dev(o["cand_dst"])
         fused = trk.stage_filter(feat, src, dst).clone()            # default: all layers in one persistent kernel
+        for pairs in (1, 5, 62):                                    # 'filter_max_pairs': fewer CTA pairs, the same bits
+            trk.set_option("filter_max_pairs", pairs)
+            assert torch.equal(trk.stage_filter(feat, src, dst), fused), pairs
+        trk.set_option("filter_max_pairs", 0)
         trk.set_option("filter_fused", 0)                           # layer by layer, chunked
         scores = []
         for v in (0, 1, 2):
