@@ -139,6 +139,24 @@ def oracle_full_event(name, n_particles=None):
     return timing, units, wall
 
 
+def run_cpu_baseline_table(args):
+    """SURVEY.md section 8(d)'s CPU-baseline table: the oracle, as it stands, on the toy and pileup-50 events with BLAS
+    limited to ONE thread and with all cores.  CPU only (no GPU is touched); prints one JSON object, not the bench line."""
+    from threadpoolctl import threadpool_limits
+    table = []
+    for name in ("toy", "pileup50"):
+        for threads in (1, None):
+            with threadpool_limits(limits=threads):
+                oracle_full_event(name, n_particles=20)            # warm-up: imports, BLAS pool
+                timing, units, wall = oracle_full_event(name)
+                used = 1 if threads == 1 else blas_threads()
+            table.append({"config": name, "blas_threads": used, "hits": units["n"], "cand_edges": units["e_c"], "kept_edges": units["e_k"],
+                          "event_s": round(wall, 4), "events_per_s": round(1.0 / wall, 4), "hits_per_s": round(units["n"] / wall, 1),
+                          "stage_s": {k: round(v, 4) for k, v in timing.items()}})
+    print(json.dumps({"cpu_baseline": {"kind": "oracle", "table": table,
+                                       "note": "S2 and S5 are single-threaded NumPy in either row; BLAS threads matter for S1, S3, S4"}}))
+
+
 def reference_units(cfg, calib, ev, model, k):
     """The oracle's pass over ONE event cut into exactly k consecutive pieces of work (the reference arm's steps): S1, S2,
     then S3 in k-4 equal slices of the candidate edges (the filter MLP is row-wise, so slices give the same values as one
@@ -442,11 +460,14 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-all-configs", action="store_true", help="skip the short runs of the other configs (all_configs)")
+    ap.add_argument("--cpu-baseline-all", action="store_true", help="CPU only: the oracle on the toy and pileup-50 events, 1 BLAS thread and all cores")
     ap.add_argument("--scan", action="store_true", help="concurrency scan (model instances x streams, packed batch, CUDA graph)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
     if args.impl == "reference":
         return run_reference(args)
+    if args.cpu_baseline_all:
+        return run_cpu_baseline_table(args)
     if args.scan:
         return run_concurrency_scan(args)
 
