@@ -96,7 +96,7 @@ __device__ __forceinline__ bool mbar_test(uint64_t* bar, uint32_t parity) {
 // thread hands to the tensor core, for which the PTX memory model formally asks for .release.cluster: measured in round 3,
 // the cluster-scope form on those arrivals alone costs S4 12 % (1.95 -> 2.18 ms on the pileup-200 event, 2.75 -> 3.11 ms on
 // pileup200_nominal).  The kernel relies on fence.proxy.async + the remote arrive making the rows visible to the pair's
-// tensor core, as current hardware does; every S4 parity test and the run-to-run bit identity
+// tensor core, as current hardware does (item 3); every S4 parity test and the run-to-run bit identity
 // tests exercise exactly this hand-over.
 __device__ __forceinline__ void mbar_arrive_remote(uint32_t cluster_addr) {
   asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
