@@ -55,3 +55,22 @@ def test_create_fails_loudly_without_a_gpu_or_with_bad_config():
         assert False, "shape error expected"
     except TrkError as e:
         assert e.status in (2, 4, 6)
+
+
+def test_cc_noalloc_refuses_bad_sizes_on_the_host():
+    """trk_cc_noalloc checks its arguments before it touches the CUDA runtime: a size beyond its built-in scratch array is
+    TRK_ERR_CAPACITY with a message that names the limit, bad arguments are TRK_ERR_INVALID_ARG, n == 0 is a no-op --
+    all without a device (the binding's constant must equal the header's)."""
+    import ctypes
+    from paper_2501_05520_b200 import CC_NOALLOC_MAX_HITS, lib
+    header = open(os.path.join(ROOT, "include", "trk.h")).read()
+    assert int(re.search(r"#define\s+TRK_CC_NOALLOC_MAX_HITS\s+(\d+)", header).group(1)) == CC_NOALLOC_MAX_HITS
+    L = lib()
+    null = ctypes.c_void_p(0)
+    junk = ctypes.c_void_p(256)                      # never dereferenced: every call below is refused or empty
+    assert L.trk_cc_noalloc(CC_NOALLOC_MAX_HITS + 1, junk, junk, junk, 1, 0.5, junk, null) == 3
+    assert b"TRK_CC_NOALLOC_MAX_HITS" in L.trk_last_error(None)
+    assert L.trk_cc_noalloc(-1, junk, junk, junk, 0, 0.5, junk, null) == 1
+    assert L.trk_cc_noalloc(10, null, junk, junk, 5, 0.5, junk, null) == 1
+    assert L.trk_cc_noalloc(10, junk, junk, junk, 5, 0.5, null, null) == 1
+    assert L.trk_cc_noalloc(0, null, null, null, 0, 0.5, null, null) == 0
